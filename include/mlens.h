@@ -1,0 +1,200 @@
+/* mlens.h -- C ABI of libmlens: microlensing magnification maps on one NVIDIA B200 (sm_100a).
+ *
+ * Hot path of arXiv 2506.02114 ("P:n" = line n of the paper text):
+ *   lens equation in complex form        w = (1-kappa) z + gamma conj(z) - alpha_star(z) - alpha_s(z)   (eq 12)
+ *   star deflection                      alpha_star = theta^2 sum m_i/(conj z - conj z_i)               (eq 13)
+ *     summed by an adaptive-quadtree fast multipole method (App. C)
+ *   smooth sheet                         disc eq 19 or rectangle eq B7
+ *   shooting window                      eq 14-16, eq A6
+ *   inverse polygon mapping (IPM)        cells -> 2 triangles -> exact area apportioning
+ *   inverse ray shooting (IRS)           ray counts per pixel
+ *
+ * Conventions
+ *   - every call returns an int status (MLENS_OK = 0, negative = error); nothing throws across the ABI;
+ *     mlens_last_error() returns a thread-local message for the last failing call.
+ *   - the library owns the opaque mlens_field; THE CALLER OWNS EVERY ARRAY it passes in or receives
+ *     into.  Arrays are DEVICE pointers (e.g. torch allocations) when ptr_kind = MLENS_PTR_DEVICE and
+ *     HOST pointers when MLENS_PTR_HOST (then the call copies host<->device itself and synchronises).
+ *     Inputs are copied at create time, never aliased.
+ *   - all work is enqueued on the cudaStream_t passed as `stream` (void*, NULL = default stream).
+ *     Calls that return scalars to the host (create, grid_info, stats) synchronise that stream.
+ *   - there is NO CPU fallback: without a CUDA device every compute call fails with MLENS_ECUDA.
+ *   - maps are row-major double[npix2][npix1], row index = x2 (y2) ascending, i.e. map[iy*npix1+ix];
+ *     a pixel owns its lower edges (floor rule).  IPM maps are in magnification units (an identity
+ *     lens gives 1.0); IRS count maps are raw ray counts, the IRS double map is counts / k^2.
+ */
+#ifndef MLENS_H
+#define MLENS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MLENS_VERSION 100 /* 0.1.0 */
+
+enum { MLENS_OK = 0, MLENS_EINVAL = -1, MLENS_ENOMEM = -2, MLENS_ECUDA = -3,
+       MLENS_ERANGE = -4 /* requested accuracy not attainable with order <= MLENS_MAX_ORDER, or tree depth exhausted */,
+       MLENS_ESTATE = -5 };
+
+enum { MLENS_PTR_DEVICE = 0, MLENS_PTR_HOST = 1 };
+enum { MLENS_SHAPE_DISC = 0, MLENS_SHAPE_RECT = 1 };          /* star-region shape */
+enum { MLENS_MASS_EQUAL = 0, MLENS_MASS_POWER = 1 };          /* dN/dm ~ m^-a on [lo,hi] / theoretical mean */
+enum { MLENS_EVAL_FMM = 0, MLENS_EVAL_DIRECT = 1 };           /* DIRECT = the paper's "no FMM" mode (Table 1) */
+enum { MLENS_MAP_IPM = 0, MLENS_MAP_IRS = 1 };
+enum { MLENS_BORDER_EQ16 = 0,      /* dY + 10 theta sqrt(kappa_star)                      (eq 16) */
+       MLENS_BORDER_A6 = 1,        /* dY + theta sqrt(kappa_star <m^2>/(f <m>)), param=f (eq A6) */
+       MLENS_BORDER_MARGIN = 2,    /* dY (1 + param)   (multiplicative margin)                   */
+       MLENS_BORDER_EXPLICIT = 3 };/* window half-sizes He1, He2 given by the caller                    */
+
+#define MLENS_MAX_ORDER 47         /* expansion order p <= 47 (48 coefficients; the paper caps at 31) */
+#define MLENS_MAX_DIRECT 32        /* stars used directly per leaf */
+
+typedef struct mlens_field mlens_field;
+
+/* Lens field from caller-given stars (eq 12).  Exactly one of kappa_star / kappa_smooth may be NaN
+ * and is then derived from kappa_tot (eq 10).  kappa_star is TAKEN AS GIVEN, never recomputed
+ * from the stars (reading G17); mlens_field_get_info reports the actual value of eq 9. */
+typedef struct {
+    double kappa_tot, kappa_star, kappa_smooth, gamma;
+    double theta_star;             /* Einstein radius of unit mass; 1 in all configs */
+    int32_t shape;                 /* MLENS_SHAPE_* of the region the sheet compensates */
+    int32_t ptr_kind;              /* where x, y, m live */
+    double R;                      /* disc radius (shape DISC) */
+    double c1, c2;                 /* rectangle corner (shape RECT), region |x1|<=c1, |x2|<=c2, centred at 0 */
+    int64_t n_stars;               /* may be 0 */
+    const double *x, *y, *m;       /* star positions and masses, length n_stars */
+    double eps_deflection;         /* absolute accuracy wanted for alpha_star, units of theta_star; <=0 -> 1e-8 */
+    int32_t max_direct;            /* <=0 -> 32; at most MLENS_MAX_DIRECT */
+    int32_t order;                 /* expansion order p; <=0 -> chosen from eq C9 and verified on device */
+    void *stream;
+} mlens_field_desc;
+
+/* Seeded star field: n_stars positions uniform in the region, masses equal
+ * or power law.  The region size follows from eq 9 with <m> = 1:  disc R = theta sqrt(N/kappa_star);
+ * rectangle 4 c1 c2 = pi theta^2 N / kappa_star with c1/c2 = rect_aspect.  Generator: DESIGN.md s4. */
+typedef struct {
+    double kappa_tot, kappa_star, kappa_smooth, gamma, theta_star;
+    int32_t shape, mass_law;
+    double rect_aspect;            /* c1/c2 for shape RECT */
+    double mass_a, mass_lo, mass_hi;
+    int64_t n_stars;
+    uint64_t seed;
+    double eps_deflection;
+    int32_t max_direct, order;
+    void *stream;
+} mlens_seed_desc;
+
+typedef struct {
+    int64_t n_stars;
+    int32_t order;                 /* expansion order p in use */
+    int32_t n_levels;              /* deepest level + 1 */
+    int64_t n_nodes, n_leaves;
+    double root_half;              /* half-length of the root square (centred at the origin) */
+    double leaf_half_min;          /* smallest leaf half-length */
+    double kappa_star_actual;      /* theta^2 sum(m) / R^2  or  pi theta^2 sum(m)/(4 c1 c2)   (eq 9) */
+    double mean_m, mean_m2;        /* <m>, <m^2> of the stars */
+    double R, c1, c2;
+    double spot_check_err;         /* max |alpha_fmm - alpha_direct| over the on-device spot check */
+    int32_t max_near;              /* largest near-field list */
+    int32_t max_m2l, max_p2l;      /* largest same-level / coarser-level interaction lists */
+} mlens_field_info;
+
+/* What to shoot.  Cell (i,j), 0<=i<n1, 0<=j<n2, has corners (i,j),(i+1,j),(i+1,j+1),(i,j+1) of the ray
+ * grid z(i,j) = (x0_1 + i h1) + i (x0_2 + j h2); IPM rays are the corners, IRS rays the cell centres. */
+typedef struct {
+    double center_y1, center_y2;   /* map centre (Y1, Y2) in the source plane */
+    double half_y1, half_y2;       /* map half-sizes (dY1, dY2) */
+    int32_t npix1, npix2;
+    double rays_per_pixel_length;  /* k: cell = pixel / k (Table 1 caption) */
+    int32_t map_mode;              /* MLENS_MAP_IPM / MLENS_MAP_IRS */
+    int32_t eval_mode;             /* MLENS_EVAL_FMM / MLENS_EVAL_DIRECT */
+    int32_t border_mode;           /* MLENS_BORDER_* */
+    int32_t accumulate;            /* 0: overwrite map/counts, 1: add to their current contents */
+    double border_param, He1, He2;
+    int64_t i0, i1, j0, j1;        /* cell sub-range [i0,i1) x [j0,j1); i1<=0 or j1<=0 -> whole grid */
+    int32_t ptr_kind;              /* where map / counts / dump live */
+    int32_t sync;                  /* 1: synchronise the stream before returning (always for host pointers) */
+    double *dump_w1, *dump_w2;     /* optional: mapped ray positions of the sub-range, written by the SAME
+                                      kernel that deposits them.  IPM: (j1-j0+1) x (i1-i0+1) corners;
+                                      IRS: (j1-j0) x (i1-i0) centres; row-major, x1 fastest. May be NULL. */
+} mlens_shoot_desc;
+
+typedef struct {
+    double X1, X2;                 /* window centre (eq 14) */
+    double H1, H2;                 /* window half-sizes, grown to whole cells */
+    double h1, h2, p1, p2;         /* cell and pixel sizes */
+    double x0_1, x0_2;             /* position of corner (0,0) */
+    double ylo1, ylo2;             /* lower-left of the map */
+    int64_t n1, n2;                /* cells along x1, x2 */
+    double weight;                 /* magnification carried by one whole triangle: h1 h2/(2 p1 p2) */
+    int32_t order;
+} mlens_grid;
+
+typedef struct {
+    int64_t n_rays;                /* lens-equation evaluations performed (incl. tile-border duplicates) */
+    int64_t n_cells;
+    int64_t n_tri_single;          /* triangles wholly inside one pixel */
+    int64_t n_tri_small;           /* triangles apportioned by the thread that mapped them */
+    int64_t n_tri_queued;          /* large triangles sent through the cooperative queue */
+    int64_t n_queue_chunks;        /* row chunks those were split into */
+    int64_t n_queue_overflow;      /* large triangles processed inline because the queue was full */
+    int64_t n_rays_fallback;       /* rays evaluated outside the tile's cached leaves */
+    int32_t n_bands;               /* row bands the sub-range was processed in */
+    int32_t gpu_launches;          /* kernels launched by this call */
+    float ms_total;                /* device time of the call (CUDA events), only when sync = 1 */
+} mlens_stats;
+
+int mlens_version(void);
+const char *mlens_last_error(void);
+
+int mlens_field_create(const mlens_field_desc *desc, mlens_field **out);
+int mlens_field_create_seeded(const mlens_seed_desc *desc, mlens_field **out);
+int mlens_field_destroy(mlens_field *f);
+int mlens_field_get_info(const mlens_field *f, mlens_field_info *info);
+
+/* Copies the stars, in the caller's original order, into x, y, m (length n_stars each). */
+int mlens_field_get_stars(const mlens_field *f, double *x, double *y, double *m, int32_t ptr_kind, void *stream);
+
+/* alpha_star (eq 13) at n points: FMM (near-field direct sum + local expansion, eq 23-24)
+ * or DIRECT (all stars).  Outputs ax, ay length n. */
+int mlens_deflect(const mlens_field *f, int64_t n, const double *zx, const double *zy,
+                  double *ax, double *ay, int32_t eval_mode, int32_t ptr_kind, void *stream);
+
+/* w of eq 12 at n points (macro + stars + sheet). */
+int mlens_lens_map(const mlens_field *f, int64_t n, const double *zx, const double *zy,
+                   double *wx, double *wy, int32_t eval_mode, int32_t ptr_kind, void *stream);
+
+/* The integers and lengths the shoot call will use (host-side arithmetic only). */
+int mlens_grid_info(const mlens_field *f, const mlens_shoot_desc *desc, mlens_grid *out);
+
+/* Shoots the (sub-range of the) ray grid and builds the map.  map: double[npix2*npix1] or NULL;
+ * counts: uint64[npix2*npix1] (IRS ray counts) or NULL; stats may be NULL. */
+int mlens_shoot(mlens_field *f, const mlens_shoot_desc *desc, double *map, uint64_t *counts,
+                mlens_stats *stats, void *stream);
+
+/* Tree introspection for tests (HOST buffers, any may be NULL).  Node arrays have n_nodes entries;
+ * coefficient arrays n_nodes*(order+1) complex numbers as (re,im) pairs, in units of the node
+ * half-length: multipole eq C1-C3, local eq C4-C7.  Leaf arrays have n_leaves entries;
+ * near_* are n_leaves*MLENS_MAX_DIRECT.  m2l_list is n_nodes*27, p2l_list n_nodes*8 (node indices, -1 pad). */
+typedef struct {
+    int32_t *level, *ix, *iy, *parent, *child0, *star_lo, *star_n, *leaf_id;
+    int32_t *nbr;                  /* n_nodes*8, same-level neighbour node or -1 */
+    int32_t *m2l_cnt, *m2l_list, *p2l_cnt, *p2l_list;
+    double *multipole, *local;
+    int32_t *near_cnt;
+    double *near_x, *near_y, *near_m;
+    double *sorted_x, *sorted_y, *sorted_m;   /* stars in Morton order, n_stars each */
+} mlens_tree_view;
+int mlens_field_get_tree(const mlens_field *f, mlens_tree_view *view);
+
+/* Micro-benchmarks for the roofline denominators: sustained FP64 FMA rate [FLOP/s]
+ * and FP64/u64 global atomic-add rate [adds/s] into a buffer of `n_slots` 8-byte slots. */
+int mlens_bench_dfma(double *flops_per_s, void *stream);
+int mlens_bench_atomics(int64_t n_slots, int32_t use_u64, double *adds_per_s, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MLENS_H */

@@ -1,0 +1,112 @@
+// common.cuh -- internal declarations of libmlens (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+#include <vector>
+#include <new>
+
+#include "../../include/mlens.h"
+
+#define ML_P1MAX (MLENS_MAX_ORDER + 1)   // coefficients per expansion
+#define ML_QBITS 24                      // quantised star / ray coordinate bits per axis
+#define ML_MAXLEV 20                     // deepest tree level
+#define ML_NEAR MLENS_MAX_DIRECT
+
+namespace ml {
+
+void set_error(const char *fmt, ...);
+
+#define ML_CUDA(call)                                                                  \
+    do {                                                                               \
+        cudaError_t e_ = (call);                                                       \
+        if (e_ != cudaSuccess) {                                                       \
+            ml::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return (e_ == cudaErrorMemoryAllocation) ? MLENS_ENOMEM : MLENS_ECUDA;      \
+        }                                                                              \
+    } while (0)
+
+#define ML_TRY(call)                 \
+    do {                             \
+        int rc_ = (call);            \
+        if (rc_ != MLENS_OK) return rc_; \
+    } while (0)
+
+// Growable device array that keeps its contents on reserve().
+template <typename T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t cap = 0;
+    int reserve(size_t n, cudaStream_t s, bool keep = true) {
+        if (n <= cap) return MLENS_OK;
+        size_t ncap = n + n / 4 + 64;
+        T *q = nullptr;
+        ML_CUDA(cudaMalloc(&q, ncap * sizeof(T)));
+        if (p && keep && cap) ML_CUDA(cudaMemcpyAsync(q, p, cap * sizeof(T), cudaMemcpyDeviceToDevice, s));
+        if (p) { ML_CUDA(cudaStreamSynchronize(s)); cudaFree(p); }
+        p = q; cap = ncap;
+        return MLENS_OK;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+struct Tree {
+    int n_nodes = 0, n_leaves = 0, n_levels = 0;
+    int level_off[ML_MAXLEV + 2] = {0};          // nodes of level l are [level_off[l], level_off[l+1])
+    DevBuf<int> level, ix, iy, parent, child0, lo, n, leaf_id, nbr;   // nbr: 8 per node
+    DevBuf<int> m2l_cnt, m2l_list, p2l_cnt, p2l_list;                 // 27 / 8 per node
+    DevBuf<double2> mp, loc;                     // n_nodes * P1
+    DevBuf<int> leaf_node;                       // n_leaves
+    DevBuf<int> near_cnt;                        // n_leaves
+    DevBuf<double> near_x, near_y, near_m;       // n_leaves * ML_NEAR
+    DevBuf<double2> ecoef;                       // n_leaves * P1: (l+1) c_{l+1} theta^2/L, l = 0..p-1
+    void release();
+};
+
+}  // namespace ml
+
+struct mlens_field {
+    // lens
+    double kappa_tot = 0, kappa_star = 0, kappa_smooth = 0, gamma = 0, theta = 1;
+    int shape = 0;
+    double R = 0, c1 = 0, c2 = 0;
+    double eps = 1e-8;
+    int max_direct = 32;
+    int order = 0;                 // p
+    int64_t n_stars = 0;
+    // stars: original order and Morton order
+    ml::DevBuf<double> ox, oy, om, sx, sy, sm;
+    ml::DevBuf<uint32_t> sqx, sqy;
+    double root_half = 1.0;
+    double mean_m = 0, mean_m2 = 0, sum_m = 0;
+    double spot_err = 0;
+    int max_near = 0, max_m2l = 0, max_p2l = 0;
+    ml::Tree tree;
+    // tables
+    ml::DevBuf<double> binom;      // (2*P1MAX) x (2*P1MAX) Pascal triangle
+    ml::DevBuf<double2> tab;       // power tables, see fmm.cu
+    // shoot scratch
+    ml::DevBuf<unsigned long long> acc;  // fixed-point / count accumulator, npix
+    ml::DevBuf<double> queue;            // large-triangle queue
+    ml::DevBuf<unsigned long long> counters;
+    int device = 0;
+};
+
+namespace ml {
+// tree.cu
+int build_tree(mlens_field *f, cudaStream_t s);
+// fmm.cu
+int fmm_prepare_tables(mlens_field *f, cudaStream_t s);
+int fmm_passes(mlens_field *f, cudaStream_t s);     // upward + downward + leaf coefficients for f->order
+// eval.cu
+int deflect_points(const mlens_field *f, int64_t n, const double *zx, const double *zy, double *ox_, double *oy_,
+                   int eval_mode, int full_lens, cudaStream_t s);
+// starfield.cu
+int generate_stars(uint64_t seed, int64_t n, int shape, double a1, double a2, int mass_law, double a,
+                   double lo, double hi, double *x, double *y, double *m, cudaStream_t s);
+// shoot.cu
+int geometry(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid *g);
+int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double *map,
+          unsigned long long *counts, mlens_stats *st, cudaStream_t s);
+}  // namespace ml

@@ -1,0 +1,231 @@
+// fmm.cu -- upward pass (P2M eq C2, M2M eq C3), downward pass (M2L eq C5, P2L eq C6, L2L eq C7) and the
+// per-leaf Taylor coefficients used by the ray evaluator (eq 24 / C4).  App. C2 of the paper.
+// All coefficients are in units of the node half-length.  c_0 and every logarithm are
+// dropped: they never enter a deflection (reading G1).
+#include "device.cuh"
+
+namespace ml {
+
+// table layout inside mlens_field::tab (double2 entries, ML_P1MAX per row)
+static const int TAB_M2M = 0;                  // 4 rows: z0^n, z0 = (+-1 +- i), row = bx + 2 by
+static const int TAB_L2L = 4;                  // 4 rows: (z0/2)^n
+static const int TAB_M2L = 8;                  // 49 rows: (-1/z0)^n, z0 = 2(dx + i dy), row = (dy+3)*7 + dx+3
+static const int TAB_ROWS = 8 + 49;
+static const int BN = 2 * ML_P1MAX;            // Pascal triangle stride
+
+int fmm_prepare_tables(mlens_field *f, cudaStream_t s) {
+    std::vector<double> bin((size_t)BN * BN, 0.0);
+    for (int n = 0; n < BN; ++n) {
+        bin[(size_t)n * BN] = 1.0;
+        for (int k = 1; k <= n; ++k)
+            bin[(size_t)n * BN + k] = bin[(size_t)(n - 1) * BN + k - 1] + (k <= n - 1 ? bin[(size_t)(n - 1) * BN + k] : 0.0);
+    }
+    std::vector<double2> tab((size_t)TAB_ROWS * ML_P1MAX);
+    for (int q = 0; q < 4; ++q) {
+        double2 z0 = make_double2((q & 1) ? 1.0 : -1.0, (q >> 1) ? 1.0 : -1.0);
+        double2 zh = make_double2(0.5 * z0.x, 0.5 * z0.y);
+        for (int n = 0; n < ML_P1MAX; ++n) {
+            tab[(size_t)(TAB_M2M + q) * ML_P1MAX + n] = cpowi(z0, n);
+            tab[(size_t)(TAB_L2L + q) * ML_P1MAX + n] = cpowi(zh, n);
+        }
+    }
+    for (int dy = -3; dy <= 3; ++dy)
+        for (int dx = -3; dx <= 3; ++dx) {
+            int row = TAB_M2L + (dy + 3) * 7 + dx + 3;
+            double2 w = make_double2(0.0, 0.0);
+            if (dx || dy) { double2 z0 = make_double2(2.0 * dx, 2.0 * dy); w = cinv(z0); w.x = -w.x; w.y = -w.y; }
+            for (int n = 0; n < ML_P1MAX; ++n) tab[(size_t)row * ML_P1MAX + n] = cpowi(w, n);
+        }
+    ML_TRY(f->binom.reserve(bin.size(), s, false));
+    ML_TRY(f->tab.reserve(tab.size(), s, false));
+    ML_CUDA(cudaMemcpyAsync(f->binom.p, bin.data(), bin.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+    ML_CUDA(cudaMemcpyAsync(f->tab.p, tab.data(), tab.size() * sizeof(double2), cudaMemcpyHostToDevice, s));
+    ML_CUDA(cudaStreamSynchronize(s));
+    return MLENS_OK;
+}
+
+struct FmmDev {
+    const int *level, *ix, *iy, *parent, *child0, *lo, *n;
+    const int *m2l_cnt, *m2l_list, *p2l_cnt, *p2l_list, *leaf_node;
+    const double *sx, *sy, *sm;
+    const uint32_t *sqx, *sqy;
+    double2 *mp, *loc, *ecoef;
+    const double *binom;
+    const double2 *tab;
+    double root_half, theta2;
+    int p, p1;
+};
+
+__device__ __forceinline__ void node_geom(const FmmDev &F, int node, double &cx, double &cy, double &half) {
+    int lev = F.level[node];
+    half = F.root_half / (double)(1 << lev);
+    cx = -F.root_half + (2.0 * F.ix[node] + 1.0) * half;
+    cy = -F.root_half + (2.0 * F.iy[node] + 1.0) * half;
+}
+
+// P2M, eq C2: a_0 = sum m, a_k = -(1/k) sum m zeta^k.  One block per childless node,
+// thread k owns coefficient k ("done in parallel").  Also serves the childless nodes of the
+// coarser levels.
+__global__ void p2m_kernel(FmmDev F, int n_leaves) {
+    int leaf = blockIdx.x;
+    int k = threadIdx.x;
+    if (leaf >= n_leaves || k > F.p) return;
+    int node = F.leaf_node[leaf];
+    double cx, cy, half;
+    node_geom(F, node, cx, cy, half);
+    double inv = 1.0 / half;
+    int lo = F.lo[node], n = F.n[node];
+    double2 acc = make_double2(0.0, 0.0);
+    for (int i = lo; i < lo + n; ++i) {
+        double m = F.sm[i];
+        if (k == 0) { acc.x += m; continue; }
+        double2 zeta = make_double2((F.sx[i] - cx) * inv, (F.sy[i] - cy) * inv);
+        double2 pw = cpowi(zeta, k);
+        acc.x -= m * pw.x; acc.y -= m * pw.y;
+    }
+    if (k > 0) { acc.x /= (double)k; acc.y /= (double)k; }
+    F.mp[(size_t)node * F.p1 + k] = acc;
+}
+
+// M2M, eq C3: b_l = -a_0 z0^l/l + sum_{k=1}^{l} a_k z0^(l-k) C(l-1,k-1), then / 2^l; the
+// four shifted children are added.  One block per node of the level, thread l owns b_l.
+__global__ void m2m_kernel(FmmDev F, int a, int b) {
+    __shared__ double2 ch[4][ML_P1MAX];
+    int node = a + blockIdx.x;
+    if (node >= b) return;
+    int c0 = F.child0[node];
+    if (c0 < 0) return;                       // childless: P2M already wrote its coefficients
+    int l = threadIdx.x;
+    if (l <= F.p)
+        for (int q = 0; q < 4; ++q) ch[q][l] = F.mp[(size_t)(c0 + q) * F.p1 + l];
+    __syncthreads();
+    if (l > F.p) return;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int q = 0; q < 4; ++q) {
+        const double2 *zp = F.tab + (size_t)(TAB_M2M + q) * ML_P1MAX;
+        if (l == 0) { acc.x += ch[q][0].x; acc.y += ch[q][0].y; continue; }
+        double2 t = cscale(zp[l], -ch[q][0].x / (double)l);       // a_0 is real
+        for (int k = 1; k <= l; ++k) {
+            double bc = F.binom[(size_t)(l - 1) * BN + (k - 1)];
+            double2 u = cmul(ch[q][k], zp[l - k]);
+            t.x = fma(bc, u.x, t.x); t.y = fma(bc, u.y, t.y);
+        }
+        acc.x += t.x; acc.y += t.y;
+    }
+    double sc = scalbn(1.0, -l);
+    F.mp[(size_t)node * F.p1 + l] = cscale(acc, sc);
+}
+
+// Downward pass for the nodes [a, b) of one level: L2L from the parent (eq C7), M2L over the same-level
+// interaction list (eq C5), P2L from the stars of childless coarser nodes (eq C6).  One block per node,
+// thread l owns local coefficient l; source coefficients are staged (pre-scaled) in shared memory.
+__global__ void downward_kernel(FmmDev F, int a, int b) {
+    __shared__ double2 src[ML_P1MAX];
+    int node = a + blockIdx.x;
+    if (node >= b) return;
+    const int l = threadIdx.x, p = F.p;
+    const bool act = (l <= p);
+    int P = F.parent[node];
+    int ix = F.ix[node], iy = F.iy[node], lev = F.level[node];
+    double2 acc = make_double2(0.0, 0.0);
+
+    // ---- L2L (eq C7 with z0 = (child - parent)/L_parent, reading G3): d_l = sum_{k>=l} c_k C(k,l) z0^(k-l) / 2^l
+    if (act) src[l] = F.loc[(size_t)P * F.p1 + l];
+    __syncthreads();
+    if (act && l >= 1) {
+        int q = (ix & 1) + 2 * (iy & 1);
+        const double2 *zp = F.tab + (size_t)(TAB_L2L + q) * ML_P1MAX;
+        double2 t = make_double2(0.0, 0.0);
+        for (int k = l; k <= p; ++k) {
+            double bc = F.binom[(size_t)k * BN + l];
+            double2 u = cmul(src[k], zp[k - l]);
+            t.x = fma(bc, u.x, t.x); t.y = fma(bc, u.y, t.y);
+        }
+        acc = cscale(t, scalbn(1.0, -l));
+    }
+
+    // ---- M2L (eq C5): c_l = z0^-l [ -b_0/l + sum_{k=1}^{p} b_k (-z0)^-k C(l+k-1,k-1) ]
+    int nm = F.m2l_cnt[node];
+    for (int e = 0; e < nm; ++e) {
+        int S = F.m2l_list[(size_t)node * 27 + e];
+        int dx = F.ix[S] - ix, dy = F.iy[S] - iy;
+        const double2 *wp = F.tab + (size_t)(TAB_M2L + (dy + 3) * 7 + dx + 3) * ML_P1MAX;   // (-1/z0)^n
+        __syncthreads();
+        if (act) src[l] = cmul(F.mp[(size_t)S * F.p1 + l], wp[l]);
+        __syncthreads();
+        if (act && l >= 1) {
+            double2 t = make_double2(-src[0].x / (double)l, 0.0);
+            for (int k = 1; k <= p; ++k) {
+                double bc = F.binom[(size_t)(l + k - 1) * BN + (k - 1)];
+                t.x = fma(bc, src[k].x, t.x); t.y = fma(bc, src[k].y, t.y);
+            }
+            double2 zi = wp[l];                                   // (1/z0)^l = (-1)^l (-1/z0)^l
+            if (l & 1) { zi.x = -zi.x; zi.y = -zi.y; }
+            double2 u = cmul(t, zi);
+            acc.x += u.x; acc.y += u.y;
+        }
+    }
+
+    // ---- P2L (eq C6): c_l = sum -m/(l zeta^l) over the stars of coarser childless nodes that lie
+    // outside this node's 3x3 block (those inside are in the near-field list)
+    int np = F.p2l_cnt[node];
+    if (np > 0 && act && l >= 1) {
+        double cx, cy, half;
+        node_geom(F, node, cx, cy, half);
+        int sh = ML_QBITS - lev;
+        for (int e = 0; e < np; ++e) {
+            int Q = F.p2l_list[(size_t)node * 8 + e];
+            int lo = F.lo[Q], n = F.n[Q];
+            for (int i = lo; i < lo + n; ++i) {
+                int cxq = (int)(F.sqx[i] >> sh), cyq = (int)(F.sqy[i] >> sh);
+                if (abs(cxq - ix) <= 1 && abs(cyq - iy) <= 1) continue;
+                double2 zeta = make_double2((F.sx[i] - cx) / half, (F.sy[i] - cy) / half);
+                double2 w = cpowi(cinv(zeta), l);
+                double f = -F.sm[i] / (double)l;
+                acc.x = fma(f, w.x, acc.x); acc.y = fma(f, w.y, acc.y);
+            }
+        }
+    }
+    if (act) F.loc[(size_t)node * F.p1 + l] = (l >= 1) ? acc : make_double2(0.0, 0.0);
+}
+
+// e_l = (l+1) c_{l+1} theta^2 / L for l < p: the derivative series of eq C4 the evaluator sums (eq 24)
+__global__ void leaf_coef_kernel(FmmDev F, int n_leaves) {
+    int leaf = blockIdx.x, l = threadIdx.x;
+    if (leaf >= n_leaves || l > F.p) return;
+    int node = F.leaf_node[leaf];
+    double half = F.root_half / (double)(1 << F.level[node]);
+    double2 v = make_double2(0.0, 0.0);
+    if (l < F.p) v = cscale(F.loc[(size_t)node * F.p1 + l + 1], (double)(l + 1) * F.theta2 / half);
+    F.ecoef[(size_t)leaf * F.p1 + l] = v;
+}
+
+int fmm_passes(mlens_field *f, cudaStream_t s) {
+    Tree &t = f->tree;
+    const int p = f->order, p1 = p + 1;
+    const size_t nn = (size_t)t.n_nodes, nl = (size_t)t.n_leaves;
+    ML_TRY(t.mp.reserve(nn * p1, s, false));
+    ML_TRY(t.loc.reserve(nn * p1, s, false));
+    ML_TRY(t.ecoef.reserve(nl * p1, s, false));
+    ML_CUDA(cudaMemsetAsync(t.loc.p, 0, nn * p1 * sizeof(double2), s));
+    FmmDev F{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p,
+             t.m2l_cnt.p, t.m2l_list.p, t.p2l_cnt.p, t.p2l_list.p, t.leaf_node.p,
+             f->sx.p, f->sy.p, f->sm.p, f->sqx.p, f->sqy.p, t.mp.p, t.loc.p, t.ecoef.p,
+             f->binom.p, f->tab.p, f->root_half, f->theta * f->theta, p, p1};
+    const int T = 64;   // >= ML_P1MAX
+    static_assert(ML_P1MAX <= 64, "one thread per coefficient");
+    p2m_kernel<<<(unsigned)nl, T, 0, s>>>(F, (int)nl);
+    for (int lev = t.n_levels - 2; lev >= 0; --lev) {
+        int a = t.level_off[lev], b = t.level_off[lev + 1];
+        m2m_kernel<<<b - a, T, 0, s>>>(F, a, b);
+    }
+    for (int lev = 2; lev < t.n_levels; ++lev) {
+        int a = t.level_off[lev], b = t.level_off[lev + 1];
+        downward_kernel<<<b - a, T, 0, s>>>(F, a, b);
+    }
+    leaf_coef_kernel<<<(unsigned)nl, T, 0, s>>>(F, (int)nl);
+    ML_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
+}  // namespace ml

@@ -1,0 +1,316 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): |alpha_gpu - alpha_direct| <= 1e-8 theta_E per ray; map pixels
+within 1e-4 relative where mu >= 0.1, at most 1e-4 of the pixels up to 1e-2; IRS counts exact when the
+oracle bins the positions the GPU kernel itself produced.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import synth
+from synth.configs import BORDER_EXPLICIT, MASS_POWER
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ml():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2506_02114_b200 as ml
+    ml.lib()
+    return ml
+
+
+def _cfg_field(ml, orc, idx, n_override=None):
+    cfg = synth.get_config(idx)
+    n = n_override or cfg.n_stars
+    R = cfg.theta_star * math.sqrt(n / cfg.kappa_star)
+    xs, ys, ms = synth.disc_stars(n, R, cfg.seed, cfg)
+    gf = ml.Field.from_stars(cfg.kappa_tot, cfg.gamma, xs, ys, ms, kappa_star=cfg.kappa_star, R=R)
+    of = orc.Field.make(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, xs, ys, ms, R=R)
+    return cfg, gf, of, (xs, ys, ms, R)
+
+
+def _map_check(gpu, ref, label=""):
+    """north_star map tolerance; returns the worst relative deviation."""
+    sel = ref >= 0.1
+    rel = np.abs(gpu[sel] - ref[sel]) / ref[sel]
+    n_loose = int(np.sum(rel > 1e-4))
+    assert rel.max() <= 1e-2, f"{label}: worst pixel off by {rel.max():.3g}"
+    assert n_loose <= max(1, int(1e-4 * ref.size)), f"{label}: {n_loose} pixels beyond 1e-4"
+    small = ~sel
+    if small.any():
+        assert np.max(np.abs(gpu[small] - ref[small])) <= 1e-4
+    return rel.max()
+
+
+# ----------------------------------------------------------------------------- star field
+def test_seeded_field_matches_oracle_generator(ml, orc):
+    f = ml.Field.seeded(0.4, 0.2, 5000, 4242, kappa_star=0.2)
+    x, y, m = f.stars()
+    R = math.sqrt(5000 / 0.2)
+    ox, oy, om = orc.starfield(4242, 5000, shape=0, a1=R)
+    assert f.info()["R"] == R
+    assert np.array_equal(x, ox) and np.array_equal(y, oy) and np.array_equal(m, om)    # bit for bit
+    f2 = ml.Field.seeded(0.6, 0.6, 3000, 7, kappa_star=0.3, mass_law=ml.MASS_POWER)
+    x, y, m = f2.stars()
+    ox, oy, om = orc.starfield(7, 3000, shape=0, a1=math.sqrt(3000 / 0.3), mass_law=1)
+    assert np.array_equal(x, ox) and np.array_equal(y, oy)
+    assert np.max(np.abs(m / om - 1)) < 1e-14                     # pow() differs in the last bits
+    f3 = ml.Field.seeded(0.5, 0.1, 2000, 9, kappa_star=0.25, shape=ml.SHAPE_RECT, rect_aspect=4.0)
+    inf = f3.info()
+    assert 4 * inf["c1"] * inf["c2"] == pytest.approx(math.pi * 2000 / 0.25, rel=1e-14)
+    x, y, m = f3.stars()
+    ox, oy, om = orc.starfield(9, 2000, shape=1, a1=inf["c1"], a2=inf["c2"])
+    assert np.array_equal(x, ox) and np.array_equal(y, oy)
+    assert inf["kappa_star_actual"] == pytest.approx(0.25, rel=1e-12)
+
+
+# ----------------------------------------------------------------------------- tree
+@pytest.mark.parametrize("n", [1, 33, 200, 20000])
+def test_tree_invariants(ml, n):
+    R = math.sqrt(n / 0.3)
+    xs, ys, ms = synth.disc_stars(n, R, 31 + n)
+    f = ml.Field.from_stars(0.5, 0.1, xs, ys, ms, kappa_star=0.3, R=R)
+    t = f.tree()
+    inf = f.info()
+    lev, child0, lo, cnt = t["level"], t["child0"], t["star_lo"], t["star_n"]
+    leaves = np.where(child0 < 0)[0]
+    # every star in exactly one leaf; leaves tile the root (areas sum to 1)
+    assert cnt[leaves].sum() == n
+    assert np.sum(4.0 ** (-lev[leaves].astype(float))) == pytest.approx(1.0, abs=1e-12)
+    # children cover their parent's star range
+    for p in np.where(child0 >= 0)[0][:2000]:
+        c = child0[p]
+        assert lo[c] == lo[p] and cnt[c:c + 4].sum() == cnt[p]
+        assert np.all(t["parent"][c:c + 4] == p) and np.all(lev[c:c + 4] == lev[p] + 1)
+    # sorted stars are a permutation of the input and sit inside their leaf's square
+    assert np.allclose(np.sort(t["sorted_x"]), np.sort(xs), rtol=0, atol=0)
+    rh = t["root_half"]
+    for l in leaves[:3000]:
+        half = rh / 2.0 ** lev[l]
+        cx = -rh + (2 * t["ix"][l] + 1) * half
+        cy = -rh + (2 * t["iy"][l] + 1) * half
+        sl = slice(lo[l], lo[l] + cnt[l])
+        assert np.all(np.abs(t["sorted_x"][sl] - cx) <= half * (1 + 1e-6))
+        assert np.all(np.abs(t["sorted_y"][sl] - cy) <= half * (1 + 1e-6))
+    # list bounds: <= 27 same-level sources, direct list <= 32; 2:1 balance
+    assert inf["max_m2l"] <= 27 and inf["max_near"] <= 32 and t["m2l_cnt"].max() <= 27
+    nb = t["nbr"]
+    for l in leaves[:3000]:
+        for d in range(8):
+            q = nb[l, d]
+            if q <= -2:
+                assert lev[-2 - q] == lev[l] - 1 and child0[-2 - q] < 0
+    # near list = all stars within the 3x3 block of the leaf's own level
+    for l in leaves[:300]:
+        half = rh / 2.0 ** lev[l]
+        cx = -rh + (2 * t["ix"][l] + 1) * half
+        cy = -rh + (2 * t["iy"][l] + 1) * half
+        k = t["leaf_id"][l]
+        got = sorted(zip(t["near_x"][k, :t["near_cnt"][k]], t["near_y"][k, :t["near_cnt"][k]]))
+        inside = (np.abs(xs - cx) < 3 * half * (1 - 1e-6)) & (np.abs(ys - cy) < 3 * half * (1 - 1e-6))
+        outside = (np.abs(xs - cx) > 3 * half * (1 + 1e-6)) | (np.abs(ys - cy) > 3 * half * (1 + 1e-6))
+        gs = set(got)
+        assert all((a, b) in gs for a, b in zip(xs[inside], ys[inside]))
+        assert not any((a, b) in gs for a, b in zip(xs[outside], ys[outside]))
+
+
+def test_fmm_coefficients_against_definitions(ml, orc):
+    # eq C2/C3: multipole coefficients of leaves AND of internal nodes (i.e. after M2M) equal the
+    # definition summed over the node's stars; eq C5-C7: local series + near field = direct sum.
+    n = 3000
+    R = math.sqrt(n / 0.4)
+    xs, ys, ms = synth.disc_stars(n, R, 77, synth.get_config(2))
+    f = ml.Field.from_stars(0.6, 0.2, xs, ys, ms, kappa_star=0.4, R=R, order=30)
+    t = f.tree()
+    p, rh = t["order"], t["root_half"]
+    rng = np.random.default_rng(0)
+    nodes = np.concatenate([[0], rng.choice(len(t["level"]), 60, replace=False)])
+    for nd in nodes:
+        half = rh / 2.0 ** t["level"][nd]
+        cx = -rh + (2 * t["ix"][nd] + 1) * half
+        cy = -rh + (2 * t["iy"][nd] + 1) * half
+        sl = slice(t["star_lo"][nd], t["star_lo"][nd] + t["star_n"][nd])
+        ref = orc.multipole_def(t["sorted_x"][sl], t["sorted_y"][sl], t["sorted_m"][sl], cx, cy, half, p)
+        scale = max(1.0, np.abs(ref[0])) * np.maximum(1.0, np.sqrt(2.0) ** np.arange(p + 1) / np.maximum(1, np.arange(p + 1)))
+        assert np.max(np.abs(t["multipole"][nd] - ref) / scale) < 1e-12, nd
+    of = orc.Field.make(0.6, 0.4, 0.2, xs, ys, ms, R=R)
+    leaves = np.where(t["child0"] < 0)[0]
+    for l in rng.choice(leaves, 40, replace=False):
+        half = rh / 2.0 ** t["level"][l]
+        cx = -rh + (2 * t["ix"][l] + 1) * half
+        cy = -rh + (2 * t["iy"][l] + 1) * half
+        k = t["leaf_id"][l]
+        nf = orc.Field.make(0, 0, 0, t["near_x"][k, :t["near_cnt"][k]], t["near_y"][k, :t["near_cnt"][k]],
+                            t["near_m"][k, :t["near_cnt"][k]], R=R)
+        for (dx, dy) in [(0.0, 0.0), (0.97, -0.97), (-0.5, 0.8)]:
+            zx, zy = cx + dx * half, cy + dy * half
+            fx, fy = orc.local_eval(t["local"][l], cx, cy, half, zx, zy)
+            ax, ay = orc.alpha_star(of, [zx], [zy])
+            if t["near_cnt"][k]:
+                nx, ny = orc.alpha_star(nf, [zx], [zy])
+            else:
+                nx, ny = [0.0], [0.0]
+            assert math.hypot(fx + nx[0] - ax[0], fy + ny[0] - ay[0]) < 1e-8
+
+
+# ----------------------------------------------------------------------------- deflection (the 1e-8 surface)
+@pytest.mark.parametrize("idx,npts", [(0, 100000), (1, 40000), (2, 6000)])
+def test_deflection_parity(ml, orc, idx, npts):
+    cfg, gf, of, (xs, ys, ms, R) = _cfg_field(ml, orc, idx)
+    g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, cfg.npix, cfg.rays_per_pixel_length,
+                     cfg.border_mode, cfg.border_param, m2_over_m=cfg.m2_over_m)
+    inf = gf.info()
+    n1 = npts // 2
+    zx1, zy1 = synth.sample_points_window(n1, g.X1, g.X2, g.H1, g.H2, 10 + idx)
+    # near stars (1e-3 theta_E) and on leaf edges/corners of the finest level
+    zx2, zy2 = synth.sample_points_near_stars(xs, ys, npts // 4, 1e-3, 20 + idx, g.H1, g.H2)
+    L = inf["leaf_half_min"]
+    rng = np.random.default_rng(30 + idx)
+    kx = rng.integers(-int(g.H1 / (2 * L)), int(g.H1 / (2 * L)) + 1, npts // 4)
+    ky = rng.integers(-int(g.H2 / (2 * L)), int(g.H2 / (2 * L)) + 1, npts // 4)
+    zx3 = -inf["root_half"] + (np.floor(inf["root_half"] / (2 * L)) + kx) * 2 * L + rng.choice([0.0, 1e-12, -1e-12], npts // 4)
+    zy3 = -inf["root_half"] + (np.floor(inf["root_half"] / (2 * L)) + ky) * 2 * L + rng.uniform(-L, L, npts // 4) * rng.integers(0, 2, npts // 4)
+    zx, zy = np.concatenate([zx1, zx2, zx3]), np.concatenate([zy1, zy2, zy3])
+    rx, ry = orc.alpha_star(of, zx, zy)
+    ax, ay = gf.deflect(zx, zy, ml.EVAL_FMM)
+    err = np.hypot(ax - rx, ay - ry)
+    assert err.max() <= 1e-8 * cfg.theta_star, (err.max(), inf)
+    dx, dy = gf.deflect(zx[:4000], zy[:4000], ml.EVAL_DIRECT)
+    scale = np.maximum(1.0, np.hypot(rx[:4000], ry[:4000]))
+    assert np.max(np.hypot(dx - rx[:4000], dy - ry[:4000]) / scale) <= 1e-12
+    # full lens equation (macro + sheet terms)
+    wx, wy = gf.lens_map(zx[:4000], zy[:4000])
+    ox, oy = orc.lens_map(of, zx[:4000], zy[:4000])
+    assert np.max(np.hypot(wx - ox, wy - oy)) <= 1e-8
+
+
+def test_rect_sheet_parity(ml, orc):
+    n = 500
+    c1, c2 = 40.0, 10.0
+    ks = math.pi * n / (4 * c1 * c2)
+    xs, ys, ms = synth.rect_stars(n, c1, c2, 3)
+    gf = ml.Field.from_stars(0.5, 0.1, xs, ys, ms, kappa_star=ks, shape=ml.SHAPE_RECT, c1=c1, c2=c2)
+    of = orc.Field.make(0.5, ks, 0.1, xs, ys, ms, shape=1, c1=c1, c2=c2)
+    rng = np.random.default_rng(1)
+    zx = rng.uniform(-60, 60, 20000); zy = rng.uniform(-20, 20, 20000)     # inside and outside the rectangle
+    wx, wy = gf.lens_map(zx, zy)
+    ox, oy = orc.lens_map(of, zx, zy)
+    assert np.max(np.hypot(wx - ox, wy - oy)) <= 1e-8
+
+
+# ----------------------------------------------------------------------------- maps
+def test_ipm_map_config0_whole(ml, orc):
+    cfg, gf, of, _ = _cfg_field(ml, orc, 0)
+    res = gf.shoot(cfg.half_y, cfg.npix, cfg.rays_per_pixel_length, border_mode=cfg.border_mode,
+                   border_param=cfg.border_param)
+    g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, cfg.npix, cfg.rays_per_pixel_length,
+                     cfg.border_mode, cfg.border_param)
+    assert (res.grid.n1, res.grid.n2) == (g.n1, g.n2)
+    assert (res.grid.x0_1, res.grid.x0_2, res.grid.h1, res.grid.h2) == (g.x0_1, g.x0_2, g.h1, g.h2)
+    ref = orc.shoot(of, g, 0)
+    _map_check(res.map, ref, "cfg0 IPM")
+    # total flux is conserved to rounding (integer accumulation: 2^-36 of a triangle per deposit)
+    assert res.map.sum() == pytest.approx(ref.sum(), rel=1e-9)
+    st = res.stats
+    assert st["n_cells"] == g.n1 * g.n2
+    assert st["n_tri_single"] + st["n_tri_small"] + st["n_tri_queued"] + st["n_queue_overflow"] <= 2 * st["n_cells"]
+    # the "no FMM" mode gives the same map
+    res2 = gf.shoot(cfg.half_y, cfg.npix, cfg.rays_per_pixel_length, border_mode=cfg.border_mode,
+                    border_param=cfg.border_param, eval_mode=ml.EVAL_DIRECT)
+    _map_check(res2.map, ref, "cfg0 IPM direct")
+
+
+def test_irs_counts_exact_config0(ml, orc):
+    cfg, gf, of, _ = _cfg_field(ml, orc, 0)
+    res = gf.shoot(cfg.half_y, cfg.npix, 2.0, map_mode=ml.MAP_IRS, border_mode=cfg.border_mode,
+                   border_param=cfg.border_param, dump=True, want_counts=True)
+    g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, cfg.npix, 2.0, cfg.border_mode, cfg.border_param)
+    # exact: the oracle bins the very positions the shooting kernel produced
+    want = orc.bin_irs(res.dump[0], res.dump[1], g)
+    assert np.array_equal(res.counts, want)
+    assert np.array_equal(res.map, want / 4.0)
+    # and those positions are the oracle's rays to 1e-8
+    ox, oy = orc.map_centres(of, g, 0, g.n1, 0, g.n2)
+    assert np.max(np.hypot(res.dump[0] - ox, res.dump[1] - oy)) <= 1e-8
+    # counts from the oracle's own rays differ only for rays within 1e-8 of a pixel edge
+    own = orc.bin_irs(ox, oy, g)
+    assert np.sum(own != want) <= 4
+
+
+@pytest.mark.parametrize("idx", [1, 2])
+def test_ipm_patches_big_configs(ml, orc, idx):
+    cfg, gf, of, (xs, ys, ms, R) = _cfg_field(ml, orc, idx, n_override=20000 if idx == 2 else None)
+    k = cfg.rays_per_pixel_length
+    half, npix = (cfg.half_y, cfg.npix) if idx == 1 else (cfg.half_y * 0.2, cfg.npix // 5)
+    g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, half, npix, k, cfg.border_mode, cfg.border_param,
+                     m2_over_m=cfg.m2_over_m)
+    rng = np.random.default_rng(5)
+    inside = np.where((np.abs(xs) < g.H1 * 0.9) & (np.abs(ys) < g.H2 * 0.9))[0]
+    patches = []
+    s = inside[0]                                     # a patch holding a star
+    patches.append((int((xs[s] - g.x0_1) / g.h1) - 64, int((ys[s] - g.x0_2) / g.h2) - 64))
+    patches.append((0, 0))                            # window corner
+    patches.append((g.n1 - 128, g.n2 - 128))
+    for _ in range(5):
+        patches.append((int(rng.integers(0, g.n1 - 128)), int(rng.integers(0, g.n2 - 128))))
+    for (pi, pj) in patches:
+        pi, pj = max(0, min(pi, g.n1 - 128)), max(0, min(pj, g.n2 - 128))
+        sub = (pi, pi + 128, pj, pj + 128)
+        res = gf.shoot(half, npix, k, border_mode=cfg.border_mode, border_param=cfg.border_param, sub=sub, dump=True)
+        ref = orc.shoot(of, g, 0, sub=sub)
+        ox, oy = orc.map_corners(of, g, *sub)
+        assert np.max(np.hypot(res.dump[0] - ox, res.dump[1] - oy)) <= 1e-8
+        tot = ref.sum()
+        assert np.max(np.abs(res.map - ref)) <= 1e-4 * max(ref.max(), 1e-300) + 1e-12, (pi, pj)
+        assert res.map.sum() == pytest.approx(tot, rel=1e-6, abs=1e-12)
+
+
+def test_closed_forms_on_gpu(ml, orc):
+    # affine maps: exactly 1/|(1-k)^2-g^2| inside (no stars)
+    z = np.zeros(0)
+    for (k, g_) in [(0.0, 0.0), (0.4, 0.2), (0.6, 0.6)]:
+        f = ml.Field.from_stars(k, g_, z, z, z, kappa_star=0.0, R=1e9)
+        res = f.shoot(2.0, 32, 2.0, border_mode=ml.BORDER_MARGIN, border_param=0.25)
+        mu = 1 / abs((1 - k) ** 2 - g_ ** 2)
+        assert np.max(np.abs(res.map - mu)) < 1e-9 * mu
+    # point lens (u^2+2)/(u sqrt(u^2+4)) through the oracle (already pinned to the closed form)
+    f = ml.Field.from_stars(0.0, 0.0, np.zeros(1), np.zeros(1), np.ones(1), kappa_star=0.0, R=1e9)
+    of = orc.Field.make(0.0, 0.0, 0.0, [0.0], [0.0], [1.0], R=1e9)
+    Hw = 2.6
+    res = f.shoot(1.5, 30, 8.0, border_mode=BORDER_EXPLICIT, He=(Hw, Hw))
+    g = orc.geometry(0.0, 0.0, 0.0, 1.5, 30, 8.0, 3, He=(Hw, Hw))
+    _map_check(res.map, orc.shoot(of, g, 0), "point lens")
+
+
+def test_subrange_and_accumulate(ml, orc):
+    cfg, gf, of, _ = _cfg_field(ml, orc, 0)
+    kw = dict(border_mode=cfg.border_mode, border_param=cfg.border_param)
+    whole = gf.shoot(cfg.half_y, 64, 2.0, **kw)
+    g = whole.grid
+    jm = g.n2 // 3
+    part = gf.shoot(cfg.half_y, 64, 2.0, sub=(0, g.n1, 0, jm), **kw)
+    part = gf.shoot(cfg.half_y, 64, 2.0, sub=(0, g.n1, jm, g.n2), out=part.map, accumulate=True, **kw)
+    assert np.allclose(part.map, whole.map, rtol=1e-12, atol=1e-14)
+    # device-resident path (torch tensors in, torch tensors out)
+    import torch
+    dev = gf.shoot(cfg.half_y, 64, 2.0, device=torch.device("cuda"), **kw)
+    assert np.array_equal(dev.map.cpu().numpy(), whole.map)          # integer accumulation: bit-reproducible
+
+
+def test_errors(ml):
+    z = np.zeros(1)
+    with pytest.raises(ml.MlensError):
+        ml.Field.from_stars(0.5, 0.5, z, z, z, kappa_star=0.0, R=1.0).shoot(1.0, 8, 1.0)   # 1-kappa-gamma = 0
+    with pytest.raises(ml.MlensError):
+        ml.Field.from_stars(0.5, 0.1, z, z, z, R=1.0)                                        # no kappa split given
+    with pytest.raises(ml.MlensError):
+        ml.Field.from_stars(0.5, 0.1, z, z, z, kappa_star=0.1, R=-1.0)
+    # more than 32 coincident stars cannot be separated by the tree
+    with pytest.raises(ml.MlensError):
+        ml.Field.from_stars(0.5, 0.1, np.full(40, 0.3), np.full(40, 0.3), np.ones(40), kappa_star=0.1, R=2.0)
