@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement of the hot path (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
+
+One STEP is one pass of the whole hot path over one synthetic workload (BASELINE.json configs[1] by
+default, the configuration the metric is quoted on):
+
+    seeded star field -> Morton sort -> quadtree + lists -> P2M/M2M -> M2L/P2L/L2L -> leaf series
+    -> fused ray evaluation + IPM deposit (map 1)  -> fused ray evaluation + IRS count (map 2)
+
+all of it in libmlens' CUDA kernels, called through the C ABI (include/mlens.h).  `value` is lens-equation
+evaluations per second over the whole step (unique rays of both maps / step time), inputs resident in
+HBM (the star field is generated on the device from the seed).  `e2e` repeats the step with HOST
+buffers: stars handed over as pinned host arrays, maps returned into pinned host arrays, the library
+doing the copies inside the timed region.
+
+N > 1 (torchrun): every rank makes an independent map of the same configuration with its own seed
+(the path shards over realisations: no data-path collective; scaling "weak"); time = max over ranks.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload, on the host cores of this box.  It is a deliberately slow baseline, not the target.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import synth  # noqa: E402
+
+METRIC = "lens_eq_evals_per_s"
+UNIT = "evals/s"
+
+# B200 FP64 vector peak used as the "alu" roofline denominator: 148 SMs x 64 DFMA
+# lanes/SM/clk x 2 flop x 1.965 GHz (clocks.max.sm of MEASURED_PEAKS.json).  The DFMA rate measured
+# by mlens_bench_dfma in the same run is reported beside it as `peak_measured_dfma`.
+FP64_LANES_PER_SM = 64
+# dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
+# (profiles/r01_ncu_full_shoot_ipm.md); None until a capture exists for the current kernel.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(cfg):
+    return (f"{cfg.name}: {cfg.n_stars} stars, kappa_tot={cfg.kappa_tot} kappa_star={cfg.kappa_star} "
+            f"gamma={cfg.gamma}, {cfg.npix}x{cfg.npix} px, half={cfg.half_y}, k={cfg.rays_per_pixel_length:g}")
+
+
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "200", "-i", str(self.index)],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                c = [v.strip() for v in line.split(",")]
+                if len(c) < 9:
+                    continue
+                try:
+                    sm.append(float(c[1])); mx.append(float(c[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, c[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, patch, want_irs=True):
+    """Times the CPU oracle on a patch of `patch` = (ni, nj) cells at the window centre: the whole path
+    (direct sum over all stars + brute-force clipping; IRS binning).  Returns (evals, seconds, threads)."""
+    import oracle
+    oracle.build()
+    R = cfg.R_star
+    xs, ys, ms = oracle.starfield(cfg.seed, cfg.n_stars, shape=0, a1=R, mass_law=cfg.mass_law,
+                                  a=cfg.mass_a, lo=cfg.mass_lo, hi=cfg.mass_hi)
+    of = oracle.Field.make(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, xs, ys, ms, R=R)
+    g = oracle.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, cfg.npix, cfg.rays_per_pixel_length,
+                        cfg.border_mode, cfg.border_param, m2_over_m=cfg.m2_over_m)
+    ni, nj = min(patch[0], g.n1), min(patch[1], g.n2)
+    i0, j0 = (g.n1 - ni) // 2, (g.n2 - nj) // 2
+    sub = (i0, i0 + ni, j0, j0 + nj)
+    t0 = time.perf_counter()
+    oracle.shoot(of, g, 0, sub=sub)
+    evals = (ni + 1) * (nj + 1)
+    if want_irs:
+        oracle.shoot(of, g, 1, sub=sub)
+        evals += ni * nj
+    return evals, time.perf_counter() - t0, oracle.num_threads(), sub
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on this box's host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg = synth.get_config(args.config)
+    patch = (128, 128)
+    for _ in range(args.warmup):
+        oracle_sample(cfg, (32, 32))
+    tot_e, tot_t, thr, sub = 0, 0.0, 1, None
+    for _ in range(args.steps):
+        e, t, thr, sub = oracle_sample(cfg, patch)
+        tot_e += e; tot_t += t
+    v = tot_e / tot_t
+    sample = f"IPM + IRS on the {patch[0]}x{patch[1]}-cell patch {sub} at the window centre, all {cfg.n_stars} stars per ray"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2506_02114_b200 as ml
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libmlens has no CPU fallback")
+    ml.lib()                                         # fail loudly if the extension is missing
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = synth.get_config(args.config)
+    seed = cfg.seed + 7919 * rank                    # one realisation per rank
+    kw = dict(border_mode=cfg.border_mode, border_param=cfg.border_param)
+    half, npix, k = cfg.half_y, cfg.npix, cfg.rays_per_pixel_length
+    stream = torch.cuda.current_stream()
+
+    map_ipm = torch.zeros((npix, npix), dtype=torch.float64, device=dev)
+    map_irs = torch.zeros((npix, npix), dtype=torch.float64, device=dev)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    state = {}
+
+    def step_device():
+        f = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, seed, kappa_star=cfg.kappa_star,
+                            mass_law=cfg.mass_law, mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
+        r1 = f.shoot(half, npix, k, out=map_ipm, map_mode=ml.MAP_IPM, **kw)
+        r2 = f.shoot(half, npix, k, out=map_irs, map_mode=ml.MAP_IRS, **kw)
+        state.update(info=f.info(), ipm=r1, irs=r2)
+        f.close()
+
+    # host-side buffers of the e2e leg: pinned, numpy views handed to the C ABI as HOST pointers
+    R = cfg.R_star
+    hx, hy, hm = (torch.empty(cfg.n_stars, dtype=torch.float64).pin_memory() for _ in range(3))
+    h_ipm = torch.empty((npix, npix), dtype=torch.float64).pin_memory()
+    h_irs = torch.empty((npix, npix), dtype=torch.float64).pin_memory()
+
+    def step_host():
+        f = ml.Field.from_stars(cfg.kappa_tot, cfg.gamma, hx.numpy(), hy.numpy(), hm.numpy(),
+                                kappa_star=cfg.kappa_star, R=R)
+        f.shoot(half, npix, k, out=h_ipm.numpy(), map_mode=ml.MAP_IPM, **kw)
+        f.shoot(half, npix, k, out=h_irs.numpy(), map_mode=ml.MAP_IRS, **kw)
+        f.close()
+        return float(h_ipm[npix // 2, npix // 2])
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        """K steps, each between its own CUDA events on the launching stream; L2 flushed between steps
+        outside the event pairs.  Returns (seconds per step, max over ranks)."""
+        total_ms = 0.0
+        barrier()
+        for _ in range(steps):
+            flush.fill_(1)                           # 512 MiB > 126 MB L2
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            e1.synchronize()
+            total_ms += e0.elapsed_time(e1)
+        barrier()
+        t = torch.tensor([total_ms / steps], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item()) * 1e-3
+
+    for _ in range(max(args.warmup, 3)):
+        step_device()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = ml.launch_count()
+    sec = timed(step_device, args.steps)
+    launches = (ml.launch_count() - l0) // args.steps
+    clocks = sampler.stop() if rank == 0 else None
+
+    g = state["ipm"].grid
+    evals_ipm = (g.n1 + 1) * (g.n2 + 1)
+    evals_irs = g.n1 * g.n2
+    evals = evals_ipm + evals_irs
+    value = world * evals / sec
+
+    e2e = None
+    if not args.no_e2e:
+        # the stars of the e2e leg come from the library's own generator (read back once, outside the timing)
+        f0 = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, seed, kappa_star=cfg.kappa_star,
+                             mass_law=cfg.mass_law, mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
+        sx, sy, sm = f0.stars()
+        f0.close()
+        hx.numpy()[:], hy.numpy()[:], hm.numpy()[:] = sx, sy, sm
+        step_host()
+        sec_h = timed(step_host, args.steps)
+        e2e = {"value": world * evals / sec_h, "unit": UNIT, "ms_per_step": sec_h * 1e3,
+               "h2d_bytes_per_step": 3 * 8 * cfg.n_stars, "d2h_bytes_per_step": 2 * 8 * npix * npix}
+
+    # ---- roofline of the dominant kernel (fused evaluate + IPM deposit), DESIGN.md s7
+    st = state["ipm"].stats
+    p = state["info"]["order"]
+    rays_k = st["n_rays"]                                        # evaluations the kernel performed
+    flop = 10.0 * st["n_near_terms"] + (8.0 * p + 10.0) * rays_k   # 10/near star, 8/Horner term, 10 macro+sheet
+    n_l = max(1, st["n_shoot_launches"])
+    dur = st["ms_shoot"] * 1e-3 / n_l
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    sm_max = peaks.get("sm_max_mhz", 1965.0)
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+    peak_tf = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    achieved_tf = flop / n_l / dur / 1e12 if dur > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "shoot_ipm_kernel", "achieved": achieved_tf, "peak": peak_tf,
+                "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                "peak_source": f"{nsm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz (derived, DESIGN.md s7)",
+                "peak_measured_dfma": ml.bench_dfma() / 1e12,
+                "flop_per_launch": flop / n_l, "launch_ms": dur * 1e3, "launches_per_map": n_l,
+                "share_of_step": st["ms_shoot"] * 1e-3 / sec}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        e, t, thr, sub = oracle_sample(cfg, (384, 384))
+        cpu = {"value": e / t, "unit": UNIT, "cores": thr, "kind": "oracle", "seconds": t,
+               "sample": f"IPM + IRS on the 384x384-cell patch {sub} at the window centre "
+                         f"({e} evaluations, each a direct sum over all {cfg.n_stars} stars)"}
+
+    if rank == 0:
+        irs = state["irs"].stats
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "rays_ipm": evals_ipm, "rays_irs": evals_irs,
+                       "stars_seed": seed, "order_p": p, "border": "eq16",
+                       "l2": "flushed between steps (512 MiB fill outside the per-step events)",
+                       "parallelism": f"{world} independent realisations" if world > 1 else "1 GPU"},
+            "phases_ms": {"ipm_map": st["ms_total"], "ipm_shoot_kernels": st["ms_shoot"], "ipm_drain_kernels": st["ms_drain"],
+                          "irs_map": irs["ms_total"], "irs_shoot_kernels": irs["ms_shoot"],
+                          "create_and_rest": sec * 1e3 - st["ms_total"] - irs["ms_total"]},
+            "ipm_map_wall_ms": st["ms_total"],
+            "evals_per_s_ipm_kernel": rays_k / (st["ms_shoot"] * 1e-3) if st["ms_shoot"] > 0 else None,
+            "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_small", "n_tri_queued", "n_queue_chunks",
+                                                  "n_queue_overflow", "n_rays_fallback")},
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline, "cpu_baseline": cpu,
+        }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

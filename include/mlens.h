@@ -144,10 +144,17 @@ typedef struct {
     int32_t n_bands;               /* row bands the sub-range was processed in */
     int32_t gpu_launches;          /* kernels launched by this call */
     float ms_total;                /* device time of the call (CUDA events), only when sync = 1 */
+    float ms_shoot;                /* summed device time of the fused evaluate+deposit launches (IPM or IRS) */
+    float ms_drain;                /* summed device time of the large-triangle drain launches (IPM) */
+    float ms_finalise;             /* device time of the fixed-point -> double conversion */
+    int32_t n_shoot_launches;      /* launches behind ms_shoot */
+    int64_t n_near_terms;          /* near-field star terms summed over all rays (eq 23 direct part) */
 } mlens_stats;
 
 int mlens_version(void);
 const char *mlens_last_error(void);
+/* Kernels launched by the library in this process so far (every launch site counts itself). */
+int64_t mlens_launch_count(void);
 
 int mlens_field_create(const mlens_field_desc *desc, mlens_field **out);
 int mlens_field_create_seeded(const mlens_seed_desc *desc, mlens_field **out);

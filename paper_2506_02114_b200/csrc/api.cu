@@ -6,6 +6,7 @@
 #include <string.h>
 
 namespace ml {
+std::atomic<long long> g_launches{0};
 static thread_local char g_err[512] = "";
 void set_error(const char *fmt, ...) {
     va_list ap;
@@ -90,11 +91,11 @@ static int spot_check(mlens_field *f, cudaStream_t s, double *err) {
     ML_TRY(b.reserve(6 * NP, s, false)); ML_TRY(bits.reserve(1, s, false));
     double *zx = b.p, *zy = b.p + NP, *ax = b.p + 2 * NP, *ay = b.p + 3 * NP, *bx = b.p + 4 * NP, *by = b.p + 5 * NP;
     double leaf_half = f->root_half / (double)(1 << (f->tree.n_levels - 1));
-    spot_points_kernel<<<(NP + 127) / 128, 128, 0, s>>>(f->sx.p, f->sy.p, f->n_stars, leaf_half, f->root_half, NP, zx, zy);
+    ML_LAUNCH(spot_points_kernel, (NP + 127) / 128, 128, 0, s, f->sx.p, f->sy.p, f->n_stars, leaf_half, f->root_half, NP, zx, zy);
     ML_TRY(deflect_points(f, NP, zx, zy, ax, ay, MLENS_EVAL_FMM, 0, s));
     ML_TRY(deflect_points(f, NP, zx, zy, bx, by, MLENS_EVAL_DIRECT, 0, s));
     ML_CUDA(cudaMemsetAsync(bits.p, 0, 8, s));
-    max_diff_kernel<<<(NP + 127) / 128, 128, 0, s>>>(ax, ay, bx, by, NP, bits.p);
+    ML_LAUNCH(max_diff_kernel, (NP + 127) / 128, 128, 0, s, ax, ay, bx, by, NP, bits.p);
     unsigned long long h = 0;
     ML_CUDA(cudaMemcpyAsync(&h, bits.p, 8, cudaMemcpyDeviceToHost, s));
     ML_CUDA(cudaStreamSynchronize(s));
@@ -150,6 +151,7 @@ extern "C" {
 
 int mlens_version(void) { return MLENS_VERSION; }
 const char *mlens_last_error(void) { return g_err; }
+int64_t mlens_launch_count(void) { return (int64_t)g_launches.load(); }
 
 int mlens_field_create(const mlens_field_desc *d, mlens_field **out) {
     if (!d || !out) { set_error("null argument"); return MLENS_EINVAL; }
@@ -375,11 +377,11 @@ int mlens_bench_dfma(double *flops_per_s, void *stream) {
     double *d = nullptr; ML_CUDA(cudaMalloc(&d, 8));
     const int iters = 1 << 15, blocks = nsm * 8, threads = 256;
     cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    dfma_kernel<<<blocks, threads, 0, s>>>(d, 1024);
+    ML_LAUNCH(dfma_kernel, blocks, threads, 0, s, d, 1024);
     float best = 1e30f;
     for (int r = 0; r < 5; ++r) {
         cudaEventRecord(e0, s);
-        dfma_kernel<<<blocks, threads, 0, s>>>(d, iters);
+        ML_LAUNCH(dfma_kernel, blocks, threads, 0, s, d, iters);
         cudaEventRecord(e1, s);
         ML_CUDA(cudaEventSynchronize(e1));
         float ms; cudaEventElapsedTime(&ms, e0, e1);
@@ -408,11 +410,11 @@ int mlens_bench_atomics(int64_t n_slots, int32_t use_u64, double *adds_per_s, vo
     int nsm = 148; cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
     const int blocks = nsm * 16, threads = 256, per = 256;
     cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    atomics_kernel<<<blocks, threads, 0, s>>>((unsigned long long *)buf, (double *)buf, n_slots, use_u64, 8);
+    ML_LAUNCH(atomics_kernel, blocks, threads, 0, s, (unsigned long long *)buf, (double *)buf, n_slots, use_u64, 8);
     float best = 1e30f;
     for (int r = 0; r < 3; ++r) {
         cudaEventRecord(e0, s);
-        atomics_kernel<<<blocks, threads, 0, s>>>((unsigned long long *)buf, (double *)buf, n_slots, use_u64, per);
+        ML_LAUNCH(atomics_kernel, blocks, threads, 0, s, (unsigned long long *)buf, (double *)buf, n_slots, use_u64, per);
         cudaEventRecord(e1, s);
         ML_CUDA(cudaEventSynchronize(e1));
         float ms; cudaEventElapsedTime(&ms, e0, e1);

@@ -6,6 +6,7 @@
 #include <string>
 #include <vector>
 #include <new>
+#include <atomic>
 
 #include "../../include/mlens.h"
 
@@ -17,6 +18,14 @@
 namespace ml {
 
 void set_error(const char *fmt, ...);
+
+// every kernel the library launches goes through ML_LAUNCH so that mlens_launch_count() is a count, not a guess
+extern std::atomic<long long> g_launches;
+#define ML_LAUNCH(kernel, grid, block, smem, stream, ...)                         \
+    do {                                                                          \
+        ++ml::g_launches;                                                         \
+        kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);               \
+    } while (0)
 
 #define ML_CUDA(call)                                                                  \
     do {                                                                               \

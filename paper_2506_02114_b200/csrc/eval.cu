@@ -78,10 +78,10 @@ int deflect_points(const mlens_field *f, int64_t n, const double *zx, const doub
     LensDev L = make_lens_dev(f);
     if (eval_mode == MLENS_EVAL_FMM) {
         long long blocks = (n + 127) / 128;
-        deflect_fmm_kernel<<<(unsigned)blocks, 128, 0, s>>>(L, n, zx, zy, ox_, oy_, full_lens);
+        ML_LAUNCH(deflect_fmm_kernel, (unsigned)blocks, 128, 0, s, L, n, zx, zy, ox_, oy_, full_lens);
     } else {
         long long blocks = (n + DP_T - 1) / DP_T;
-        deflect_direct_kernel<<<(unsigned)blocks, DP_T, 0, s>>>(L, n, zx, zy, ox_, oy_, full_lens);
+        ML_LAUNCH(deflect_direct_kernel, (unsigned)blocks, DP_T, 0, s, L, n, zx, zy, ox_, oy_, full_lens);
     }
     ML_CUDA(cudaGetLastError());
     return MLENS_OK;
@@ -174,7 +174,7 @@ int generate_stars(uint64_t seed, int64_t n, int shape, double a1, double a2, in
         inv_mean = 1.0 / mean; inv_e = 1.0 / e;
     }
     long long blocks = (n + 255) / 256;
-    starfield_kernel<<<(unsigned)blocks, 256, 0, s>>>(sf, n, shape, a1, a2, mass_law, inv_e, loe, dhe, inv_mean, x, y, m);
+    ML_LAUNCH(starfield_kernel, (unsigned)blocks, 256, 0, s, sf, n, shape, a1, a2, mass_law, inv_e, loe, dhe, inv_mean, x, y, m);
     ML_CUDA(cudaGetLastError());
     return MLENS_OK;
 }

@@ -214,16 +214,16 @@ int fmm_passes(mlens_field *f, cudaStream_t s) {
              f->binom.p, f->tab.p, f->root_half, f->theta * f->theta, p, p1};
     const int T = 64;   // >= ML_P1MAX
     static_assert(ML_P1MAX <= 64, "one thread per coefficient");
-    p2m_kernel<<<(unsigned)nl, T, 0, s>>>(F, (int)nl);
+    ML_LAUNCH(p2m_kernel, (unsigned)nl, T, 0, s, F, (int)nl);
     for (int lev = t.n_levels - 2; lev >= 0; --lev) {
         int a = t.level_off[lev], b = t.level_off[lev + 1];
-        m2m_kernel<<<b - a, T, 0, s>>>(F, a, b);
+        ML_LAUNCH(m2m_kernel, b - a, T, 0, s, F, a, b);
     }
     for (int lev = 2; lev < t.n_levels; ++lev) {
         int a = t.level_off[lev], b = t.level_off[lev + 1];
-        downward_kernel<<<b - a, T, 0, s>>>(F, a, b);
+        ML_LAUNCH(downward_kernel, b - a, T, 0, s, F, a, b);
     }
-    leaf_coef_kernel<<<(unsigned)nl, T, 0, s>>>(F, (int)nl);
+    ML_LAUNCH(leaf_coef_kernel, (unsigned)nl, T, 0, s, F, (int)nl);
     ML_CUDA(cudaGetLastError());
     return MLENS_OK;
 }

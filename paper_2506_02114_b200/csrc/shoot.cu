@@ -20,7 +20,7 @@ static const int SMALL_MAX = 16;      // triangles whose clipped bounding box ha
 static const int CHUNK_PX = 4096;     // pixels of bounding box per queue chunk
 static const int QENT = 8;            // doubles per queue entry
 
-enum { C_QUEUE = 0, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NCOUNTERS };
+enum { C_QUEUE = 0, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR, C_NCOUNTERS };
 
 struct ShootDev {
     LensDev L;
@@ -135,7 +135,7 @@ __device__ __noinline__ void tri_deposit_loop(const ShootDev &S, const TriBox &B
         }
 }
 
-struct ThreadCounters { unsigned int single = 0, small_ = 0, queued = 0, chunks = 0, overflow = 0, fallback = 0, rays = 0; };
+struct ThreadCounters { unsigned int single = 0, small_ = 0, queued = 0, chunks = 0, overflow = 0, fallback = 0, rays = 0, near_ = 0; };
 
 __device__ __forceinline__ void deposit_general(const ShootDev &S, double u0, double v0, double u1, double v1,
                                                 double u2, double v2, ThreadCounters &tc) {
@@ -164,9 +164,9 @@ __device__ __forceinline__ void deposit_general(const ShootDev &S, double u0, do
 }
 
 __device__ __forceinline__ void flush_counters(const ShootDev &S, ThreadCounters &tc) {
-    unsigned int v[7] = {tc.single, tc.small_, tc.queued, tc.chunks, tc.overflow, tc.fallback, tc.rays};
+    unsigned int v[8] = {tc.single, tc.small_, tc.queued, tc.chunks, tc.overflow, tc.fallback, tc.rays, tc.near_};
 #pragma unroll
-    for (int k = 0; k < 7; ++k) {
+    for (int k = 0; k < 8; ++k) {
         unsigned int x = v[k];
         for (int o = 16; o; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
         if ((threadIdx.x & 31) == 0 && x) atomicAdd(&S.counters[C_SINGLE + k], (unsigned long long)x);
@@ -237,6 +237,7 @@ __device__ __forceinline__ void eval_ray(const ShootDev &S, const LeafCache &C, 
         }
         if (slot >= 0) {
             double nx_, ny_, fx, fy;
+            tc.near_ += (unsigned int)C.cnt[slot];
             near_sum(C.nx[slot], C.ny[slot], C.nm[slot], C.cnt[slot], x, y, nx_, ny_);
             far_horner(C.ec[slot], S.L.p, (x - C.cx[slot]) * C.invh[slot], (y - C.cy[slot]) * C.invh[slot], fx, fy);
             ax = fma(S.L.theta2, nx_, fx);
@@ -592,25 +593,36 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     const bool timed = st && (d->sync || d->ptr_kind == MLENS_PTR_HOST);
     if (timed) { ML_CUDA(cudaEventCreate(&e0)); ML_CUDA(cudaEventCreate(&e1)); ML_CUDA(cudaEventRecord(e0, s)); }
     int launches = 0, bands = 0;
+    // per-kernel device times: events between the back-to-back launches of each band (timed calls only)
+    std::vector<cudaEvent_t> ev;
+    auto mark = [&]() -> int {
+        if (!timed) return MLENS_OK;
+        cudaEvent_t e; ML_CUDA(cudaEventCreate(&e)); ML_CUDA(cudaEventRecord(e, s)); ev.push_back(e);
+        return MLENS_OK;
+    };
     for (long long r0 = 0; r0 < nty; r0 += rows_per_band, ++bands) {
         S.tile_row0 = r0;
         S.tile_rows = (nty - r0 < rows_per_band) ? (nty - r0) : rows_per_band;
         long long nt = ntx * S.tile_rows;
         int grid = (int)((nt < (long long)nsm * 16) ? nt : (long long)nsm * 16);
+        ML_TRY(mark());
         if (ipm) {
-            shoot_ipm_kernel<<<grid, NWARP * 32, 0, s>>>(S);
-            drain_kernel<<<nsm * 8, 256, 0, s>>>(S);
+            ML_LAUNCH(shoot_ipm_kernel, grid, NWARP * 32, 0, s, S);
+            ML_TRY(mark());
+            ML_LAUNCH(drain_kernel, nsm * 8, 256, 0, s, S);
+            ML_TRY(mark());
             ML_CUDA(cudaMemsetAsync(f->counters.p, 0, 8, s));     // queue fill count only
             launches += 2;
         } else {
-            shoot_irs_kernel<<<grid, NWARP * 32, 0, s>>>(S);
+            ML_LAUNCH(shoot_irs_kernel, grid, NWARP * 32, 0, s, S);
+            ML_TRY(mark());
             launches += 1;
         }
         ML_CUDA(cudaGetLastError());
     }
     double scale = ipm ? g->weight / (double)(1ull << FIXBITS)
                        : 1.0 / (d->rays_per_pixel_length * d->rays_per_pixel_length);
-    finalise_kernel<<<(unsigned)((npix + 255) / 256), 256, 0, s>>>(f->acc.p, npix, scale, d->accumulate, map,
+    ML_LAUNCH(finalise_kernel, (unsigned)((npix + 255) / 256), 256, 0, s, f->acc.p, npix, scale, d->accumulate, map,
                                                                     ipm ? nullptr : counts);
     ++launches;
     ML_CUDA(cudaGetLastError());
@@ -625,11 +637,24 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         st->n_tri_single = (int64_t)h[C_SINGLE]; st->n_tri_small = (int64_t)h[C_SMALL];
         st->n_tri_queued = (int64_t)h[C_QUEUED]; st->n_queue_chunks = (int64_t)h[C_CHUNKS];
         st->n_queue_overflow = (int64_t)h[C_OVERFLOW]; st->n_rays_fallback = (int64_t)h[C_FALLBACK];
-        st->n_bands = bands; st->gpu_launches = launches;
-        if (timed) { ML_CUDA(cudaEventElapsedTime(&st->ms_total, e0, e1)); cudaEventDestroy(e0); cudaEventDestroy(e1); }
+        st->n_near_terms = (int64_t)h[C_NEAR];
+        st->n_bands = bands; st->gpu_launches = launches; st->n_shoot_launches = bands;
+        if (timed) {
+            ML_CUDA(cudaEventElapsedTime(&st->ms_total, e0, e1)); cudaEventDestroy(e0); cudaEventDestroy(e1);
+            const size_t per = ipm ? 3 : 2;              // events per band
+            for (int b = 0; b < bands; ++b) {
+                float ms = 0;
+                ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per], ev[b * per + 1])); st->ms_shoot += ms;
+                if (ipm) { ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 1], ev[b * per + 2])); st->ms_drain += ms; }
+            }
+            float ms = 0;
+            // the last band's closing event is followed by (memset,) finalise, closing event
+            ML_CUDA(cudaEventElapsedTime(&ms, ev[ev.size() - 2], ev[ev.size() - 1])); st->ms_finalise = ms;
+        }
     } else if (d->sync) {
         ML_CUDA(cudaStreamSynchronize(s));
     }
+    for (cudaEvent_t e : ev) cudaEventDestroy(e);
     return MLENS_OK;
 }
 

@@ -63,10 +63,10 @@ __global__ void scan_add_kernel(int *data, int n, const int *block_offsets) {
 static int exclusive_scan(int *data, int n, int *scratch, cudaStream_t s) {
     if (n <= 0) return MLENS_OK;
     int nb = (n + SCAN_B - 1) / SCAN_B;
-    scan_block_kernel<<<nb, SCAN_T, 0, s>>>(data, n, nb > 1 ? scratch : nullptr);
+    ML_LAUNCH(scan_block_kernel, nb, SCAN_T, 0, s, data, n, nb > 1 ? scratch : nullptr);
     if (nb > 1) {
         ML_TRY(exclusive_scan(scratch, nb, scratch + nb, s));
-        scan_add_kernel<<<nb, SCAN_T, 0, s>>>(data, n, scratch);
+        ML_LAUNCH(scan_add_kernel, nb, SCAN_T, 0, s, data, n, scratch);
     }
     ML_CUDA(cudaGetLastError());
     return MLENS_OK;
@@ -357,8 +357,8 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     double extent = 0.0, mom[2] = {0, 0};
     if (n > 0) {
         int blocks = (int)((N + 255) / 256); if (blocks > 1184) blocks = 1184;
-        extent_kernel<<<blocks, 256, 0, s>>>(f->ox.p, f->oy.p, N, d_bits.p);
-        moments_kernel<<<blocks, 256, 0, s>>>(f->om.p, N, d_mom.p);
+        ML_LAUNCH(extent_kernel, blocks, 256, 0, s, f->ox.p, f->oy.p, N, d_bits.p);
+        ML_LAUNCH(moments_kernel, blocks, 256, 0, s, f->om.p, N, d_mom.p);
         unsigned long long bits = 0;
         ML_CUDA(cudaMemcpyAsync(&bits, d_bits.p, sizeof(bits), cudaMemcpyDeviceToHost, s));
         ML_CUDA(cudaMemcpyAsync(mom, d_mom.p, sizeof(mom), cudaMemcpyDeviceToHost, s));
@@ -384,16 +384,16 @@ int build_tree(mlens_field *f, cudaStream_t s) {
         int nb = (n + RS_CHUNK - 1) / RS_CHUNK;
         ML_TRY(hist.reserve((size_t)256 * nb, s, false));
         ML_TRY(scratch.reserve(scan_scratch_ints((size_t)256 * nb), s, false));
-        keys_kernel<<<(n + 255) / 256, 256, 0, s>>>(f->ox.p, f->oy.p, n, f->root_half, qscale, k0.p, v0.p);
+        ML_LAUNCH(keys_kernel, (n + 255) / 256, 256, 0, s, f->ox.p, f->oy.p, n, f->root_half, qscale, k0.p, v0.p);
         unsigned long long *ka = k0.p, *kb = k1.p; int *va = v0.p, *vb = v1.p;
         for (int shift = 0; shift < 2 * ML_QBITS; shift += 8) {
-            rs_hist_kernel<<<nb, RS_T, 0, s>>>(ka, n, shift, hist.p, nb);
+            ML_LAUNCH(rs_hist_kernel, nb, RS_T, 0, s, ka, n, shift, hist.p, nb);
             ML_TRY(exclusive_scan(hist.p, 256 * nb, scratch.p, s));
-            rs_scatter_kernel<<<nb, RS_T, 0, s>>>(ka, va, n, shift, hist.p, nb, kb, vb);
+            ML_LAUNCH(rs_scatter_kernel, nb, RS_T, 0, s, ka, va, n, shift, hist.p, nb, kb, vb);
             std::swap(ka, kb); std::swap(va, vb);
         }
         ML_CUDA(cudaGetLastError());
-        gather_kernel<<<(n + 255) / 256, 256, 0, s>>>(va, n, f->ox.p, f->oy.p, f->om.p, ka, f->sx.p, f->sy.p, f->sm.p,
+        ML_LAUNCH(gather_kernel, (n + 255) / 256, 256, 0, s, va, n, f->ox.p, f->oy.p, f->om.p, ka, f->sx.p, f->sy.p, f->sm.p,
                                                       f->sqx.p, f->sqy.p);
         if (ka != k0.p) ML_CUDA(cudaMemcpyAsync(k0.p, ka, (size_t)n * sizeof(unsigned long long), cudaMemcpyDeviceToDevice, s));
         ML_CUDA(cudaGetLastError());
@@ -424,7 +424,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
         ML_TRY(flags.reserve(cnt + 1, s, false)); ML_TRY(rank.reserve(cnt + 1, s, false));
         ML_TRY(scratch.reserve(scan_scratch_ints(cnt + 1), s, false));
         TreeDev T{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, t.nbr.p, f->sqx.p, f->sqy.p};
-        link_level_kernel<<<(cnt + 127) / 128, 128, 0, s>>>(T, a, b, lev, f->max_direct, flags.p, d_over.p);
+        ML_LAUNCH(link_level_kernel, (cnt + 127) / 128, 128, 0, s, T, a, b, lev, f->max_direct, flags.p, d_over.p);
         ML_CUDA(cudaMemcpyAsync(rank.p, flags.p, (size_t)cnt * 4, cudaMemcpyDeviceToDevice, s));
         ML_CUDA(cudaMemsetAsync(rank.p + cnt, 0, 4, s));
         ML_TRY(exclusive_scan(rank.p, cnt + 1, scratch.p, s));
@@ -434,7 +434,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
         if ((size_t)b + 4 * (size_t)nsplit > 0x7ffffff0u) { set_error("tree too large"); return MLENS_ERANGE; }
         ML_TRY(reserve_nodes(t, (size_t)b + 4 * (size_t)nsplit + 1, s));
         TreeDev T2{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, t.nbr.p, f->sqx.p, f->sqy.p};
-        make_children_kernel<<<(cnt + 127) / 128, 128, 0, s>>>(T2, a, b, lev, flags.p, rank.p, keys);
+        ML_LAUNCH(make_children_kernel, (cnt + 127) / 128, 128, 0, s, T2, a, b, lev, flags.p, rank.p, keys);
         ML_CUDA(cudaGetLastError());
         if (nsplit == 0) break;
         a = b; b = b + 4 * nsplit; ++lev;
@@ -454,7 +454,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     const int nn = t.n_nodes;
     ML_TRY(t.leaf_id.reserve(nn + 1, s, false));
     ML_TRY(scratch.reserve(scan_scratch_ints(nn + 1), s, false));
-    leaf_flag_kernel<<<(nn + 255) / 256, 256, 0, s>>>(t.child0.p, nn, t.leaf_id.p);
+    ML_LAUNCH(leaf_flag_kernel, (nn + 255) / 256, 256, 0, s, t.child0.p, nn, t.leaf_id.p);
     ML_CUDA(cudaMemsetAsync(t.leaf_id.p + nn, 0, 4, s));
     ML_TRY(exclusive_scan(t.leaf_id.p, nn + 1, scratch.p, s));
     int nleaf = 0;
@@ -472,7 +472,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     ML_CUDA(cudaMemsetAsync(t.near_m.p, 0, (size_t)nleaf * ML_NEAR * 8, s));
     DevBuf<int> maxima; ML_TRY(maxima.reserve(4, s)); ML_CUDA(cudaMemsetAsync(maxima.p, 0, 16, s));
     TreeDev T{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, t.nbr.p, f->sqx.p, f->sqy.p};
-    lists_kernel<<<(nn + 127) / 128, 128, 0, s>>>(T, nn, t.leaf_id.p, t.leaf_node.p, t.m2l_cnt.p, t.m2l_list.p,
+    ML_LAUNCH(lists_kernel, (nn + 127) / 128, 128, 0, s, T, nn, t.leaf_id.p, t.leaf_node.p, t.m2l_cnt.p, t.m2l_list.p,
                                                   t.p2l_cnt.p, t.p2l_list.p, t.near_cnt.p, t.near_x.p, t.near_y.p,
                                                   t.near_m.p, f->sx.p, f->sy.p, f->sm.p, maxima.p);
     int h_max[4];

@@ -73,7 +73,8 @@ class Stats(C.Structure):
     _fields_ = [("n_rays", C.c_int64), ("n_cells", C.c_int64), ("n_tri_single", C.c_int64), ("n_tri_small", C.c_int64),
                 ("n_tri_queued", C.c_int64), ("n_queue_chunks", C.c_int64), ("n_queue_overflow", C.c_int64),
                 ("n_rays_fallback", C.c_int64), ("n_bands", C.c_int32), ("gpu_launches", C.c_int32),
-                ("ms_total", C.c_float)]
+                ("ms_total", C.c_float), ("ms_shoot", C.c_float), ("ms_drain", C.c_float),
+                ("ms_finalise", C.c_float), ("n_shoot_launches", C.c_int32), ("n_near_terms", C.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -96,6 +97,7 @@ def lib():
         L = C.CDLL(_SO)
         L.mlens_version.restype = C.c_int
         L.mlens_last_error.restype = C.c_char_p
+        L.mlens_launch_count.restype = C.c_int64
         vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
         L.mlens_field_create.argtypes = [C.POINTER(FieldDesc), C.POINTER(vp)]
         L.mlens_field_create_seeded.argtypes = [C.POINTER(SeedDesc), C.POINTER(vp)]
@@ -120,6 +122,11 @@ def _check(rc):
 
 def version():
     return lib().mlens_version()
+
+
+def launch_count():
+    """Kernels launched by libmlens in this process so far."""
+    return int(lib().mlens_launch_count())
 
 
 def _is_torch(a):
