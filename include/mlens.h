@@ -149,6 +149,13 @@ typedef struct {
     float ms_finalise;             /* device time of the fixed-point -> double conversion */
     int32_t n_shoot_launches;      /* launches behind ms_shoot */
     int64_t n_near_terms;          /* near-field star terms summed over all rays (eq 23 direct part) */
+    int64_t n_px_small;            /* (triangle, pixel) pairs clipped by the mapping thread itself */
+    int64_t n_px_interior;         /* ... covered by queued triangles as interior pixels (constant deposit) */
+    int64_t n_px_edge;             /* ... clipped exactly by the cooperative drain */
+    int64_t n_rows;                /* pixel rows of queued triangles */
+    int64_t n_tiles_full;          /* tile slots whose truncation bound failed (evaluated with the leaf's full series) */
+    int32_t tile_order;            /* order of the per-tile series */
+    int32_t pad_;
 } mlens_stats;
 
 int mlens_version(void);

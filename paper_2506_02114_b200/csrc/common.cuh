@@ -97,6 +97,7 @@ struct mlens_field {
     ml::DevBuf<double2> tab;       // power tables, see fmm.cu
     // shoot scratch
     ml::DevBuf<unsigned long long> acc;  // fixed-point / count accumulator, npix
+    ml::DevBuf<unsigned long long> diff; // row-difference array of interior runs (IPM), npix
     ml::DevBuf<double> queue;            // large-triangle queue
     ml::DevBuf<unsigned long long> counters;
     int device = 0;

@@ -370,7 +370,9 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     f->sum_m = mom[0];
     f->mean_m = n ? mom[0] / n : 0.0;
     f->mean_m2 = n ? mom[1] / n : 0.0;
-    f->root_half = extent * (1.0 + 1e-6);
+    // The root square is twice the stars' extent: shooting windows reach a little past the star region
+    // (config 1: H2 = 211.4 > R = 210.8), and rays outside the root can only be summed directly.
+    f->root_half = 2.0 * extent * (1.0 + 1e-6);
     if (f->root_half < f->theta) f->root_half = f->theta;
     const double qscale = (double)(1u << ML_QBITS) / (2.0 * f->root_half);
 
