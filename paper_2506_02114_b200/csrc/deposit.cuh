@@ -1,0 +1,393 @@
+// deposit.cuh -- exact area apportioning of mapped triangles (hot loop B) for warp-autonomous kernels.
+//
+// Accumulation is 64-bit fixed point, ONE = 2^FIXBITS per whole triangle: integer adds commute, so maps are
+// bit-reproducible whatever the atomic order.  Two arrays: `acc` holds pixel sums, `diff` the ROW DIFFERENCES
+// of what the large triangles add (map[y][x] = acc[y][x] + sum_{x' <= x} diff[y][x'], finalise_kernel).
+//   - a triangle inside one pixel:            ONE into that pixel                       (run-length merged per warp)
+//   - a triangle over two adjacent pixels:    closed-form split by the area fraction below the pixel line
+//   - a triangle with a small bounding box:   every pixel of the box clipped exactly (Green's theorem form of
+//     Sutherland-Hodgman + shoelace), the pixels of 32 triangles spread evenly over the warp's lanes
+//   - any larger triangle (drain_kernel):     signed-area edge walk.  Every edge is cut into pieces by the
+//     pixel grid lines it crosses; a piece inside pixel (i, j) that rises by dy covers dy (1 - m) of pixel i
+//     and dy of every pixel to its right in row j (m = mean x of the piece within the pixel), i.e.
+//     diff[j][i] += c dy (1 - m), diff[j][i+1] += c dy m  with c = -sign(A) ONE/|A|.  The three edges' covers
+//     cancel to the right of the triangle; they cancel EXACTLY because c dy is computed as G(y_end) - G(y_start)
+//     with G(y) = round(c y) evaluated on values shared by consecutive pieces (vertices, grid lines).
+//     Cost is proportional to the triangle's perimeter in pixels, never to its area, and the result is the same
+//     area of intersection as clipping every pixel, up to rounding.
+#pragma once
+#include "tile.cuh"
+
+namespace ml {
+
+static const int FIXBITS = 36;
+static const unsigned long long FIX_ONE = 1ull << FIXBITS;
+static const int QENT = 6;                 // doubles per giant-queue entry: the 3 vertices in pixel units
+
+enum { C_QUEUE = 0, C_TILE, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR,
+       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_NCOUNTERS };
+
+struct Win {                           // where a warp's deposits go (uniform registers)
+    unsigned int *w32;                 // the warp's shared window viewed as 32-bit halves, or nullptr
+    int ax, ay;
+};
+
+// 64-bit add into shared memory from two native 32-bit atomics (a 64-bit shared atomicAdd is a CAS loop):
+// the low word returns its old value, the carry it produced joins the high word.  Sums commute, so the
+// word pair always ends up holding the exact 64-bit total.
+__device__ __forceinline__ void shared_add64(unsigned int *w32, int idx, unsigned long long v) {
+    unsigned int lo = (unsigned int)v, hi = (unsigned int)(v >> 32);
+    if (lo) {
+        unsigned int old = atomicAdd(&w32[2 * idx], lo);
+        hi += (old + lo < old) ? 1u : 0u;
+    }
+    if (hi) atomicAdd(&w32[2 * idx + 1], hi);
+}
+
+// v into pixel (px, py) of the map (window if it covers the pixel, else L2); pixels outside the map receive nothing
+__device__ __forceinline__ void pix_add(const ShootDev &S, const Win &W, int px, int py, unsigned long long v) {
+    if ((unsigned)px >= (unsigned)S.npix1 || (unsigned)py >= (unsigned)S.npix2 || v == 0ull) return;
+    unsigned int lx = (unsigned int)(px - W.ax), ly = (unsigned int)(py - W.ay);
+    if (W.w32 && lx < (unsigned)WX && ly < (unsigned)WY) shared_add64(W.w32, (int)(ly * WX + lx), v);
+    else atomicAdd(&S.acc[(size_t)py * S.npix1 + px], v);
+}
+// diff[py][px] += v; the caller guarantees 0 <= px < npix1, 0 <= py < npix2
+__device__ __forceinline__ void diff_add(const ShootDev &S, int px, int py, unsigned long long v) {
+    if (v) atomicAdd(&S.diff[(size_t)py * S.npix1 + px], v);
+}
+__device__ __forceinline__ void flush_window(const ShootDev &S, const WarpShared &Ws, const Win &W) {
+    const int lane = threadIdx.x & 31;
+#pragma unroll 4
+    for (int k = lane; k < WY * WX; k += 32) {
+        unsigned long long c = Ws.win[k];
+        if (c) {
+            int px = W.ax + (k % WX), py = W.ay + (k / WX);            // only in-map pixels were ever added
+            atomicAdd(&S.acc[(size_t)py * S.npix1 + px], c);
+        }
+    }
+}
+
+__device__ __forceinline__ int floor_to_int(double u) {
+    return (int)floor(fmin(fmax(u, -1.0e9), 1.0e9));      // NaN -> -1e9
+}
+// pixel coordinates packed as two int16 (values beyond the map on one side collapse: such triangles are outside)
+__device__ __forceinline__ int pack_px(double u, double v) {
+    int a = (int)floor(fmin(fmax(u, -30000.0), 30000.0)), b = (int)floor(fmin(fmax(v, -30000.0), 30000.0));
+    if (u != u) a = -30000;
+    if (v != v) b = -30000;
+    return (b << 16) | (a & 0xffff);
+}
+__device__ __forceinline__ int px_of(int pk) { return (int)(short)(pk & 0xffff); }
+__device__ __forceinline__ int py_of(int pk) { return pk >> 16; }
+
+__device__ __forceinline__ unsigned long long to_fix(double frac) {
+    long long v = __double2ll_rn(frac * (double)FIX_ONE);
+    v = v < 0 ? 0 : v;
+    return v > (long long)FIX_ONE ? FIX_ONE : (unsigned long long)v;
+}
+
+// Fraction of a triangle's area on the negative side of an axis-parallel line, d0..d2 the signed distances
+// of the vertices from it: the lone vertex cuts off a similar corner, ratio t1 t2 of its two edges.
+__device__ __forceinline__ double frac_below(double d0, double d1, double d2) {
+    bool n0 = d0 < 0.0, n1 = d1 < 0.0, n2 = d2 < 0.0;
+    int cnt = (int)n0 + (int)n1 + (int)n2;
+    if (cnt == 0) return 0.0;
+    if (cnt == 3) return 1.0;
+    bool lone_neg = (cnt == 1);
+    double l, o1, o2;
+    if (n0 == lone_neg) { l = d0; o1 = d1; o2 = d2; }
+    else if (n1 == lone_neg) { l = d1; o1 = d0; o2 = d2; }
+    else { l = d2; o1 = d0; o2 = d1; }
+    double f = (l * l) * fast_rcp((l - o1) * (l - o2));
+    return lone_neg ? f : 1.0 - f;
+}
+
+// ---- warp ring buffers of pending work (entries of NW doubles, capacity 64, always < 32 pending before a push)
+struct Ring { int head = 0, count = 0; };
+
+template <int NW>
+__device__ __forceinline__ void ring_push(Ring &R, double (*buf)[NW], bool pred, const double (&v)[NW]) {
+    const unsigned m = __ballot_sync(0xffffffffu, pred);
+    if (pred) {
+        int pos = (R.head + R.count + __popc(m & ((1u << (threadIdx.x & 31)) - 1u))) & 63;
+#pragma unroll
+        for (int k = 0; k < NW; ++k) buf[pos][k] = v[k];
+    }
+    R.count += __popc(m);
+}
+
+// ---- two-pixel strips: entry = signed distances of the vertices from the pixel line, pixel, axis.
+// Out of line (one copy in the instruction cache); lanes [0, n) take one pending entry each.
+static __device__ __noinline__ void strip2_batch(const ShootDev *Sp, unsigned int *w32, int ax, int ay, const double (*ring)[4], int head, int n) {
+    const ShootDev &S = *Sp;
+    const int lane = threadIdx.x & 31;
+    Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
+    __syncwarp();
+    if (lane < n) {
+        const double *q = ring[(head + lane) & 63];
+        const double d0 = q[0], d1 = q[1], d2 = q[2];
+        const int code = __double2loint(q[3]), pk = __double2hiint(q[3]);     // code: bit 0 = axis (1: pixels stacked in y), bit 1 = degenerate
+        const int px = px_of(pk), py = py_of(pk);
+        const unsigned long long a = (code & 2) ? ((d0 < 0.0) ? FIX_ONE : 0ull) : to_fix(frac_below(d0, d1, d2));
+#pragma unroll 1
+        for (int k = 0; k < 2; ++k)                             // rolled: one copy of the add in the instruction stream
+            pix_add(S, W, px + ((code & 1) ? 0 : k), py + ((code & 1) ? k : 0), k ? FIX_ONE - a : a);
+    }
+    __syncwarp();
+}
+
+// ---- the edge walk ------------------------------------------------------------------------------------------
+struct EdgeWalk {                     // one triangle edge, clipped to the map rows and to the columns left of the map's right border
+    double x0, y0, x1, y1, dx, dy, idx, idy, ta, tb;
+    double gx0, gy0, sx, sy;          // first grid line crossed along each axis and the step (+-1)
+    int nX, nY, n;                    // crossings and pieces (n = nX + nY + 1, or 0)
+};
+
+// local coordinates: pixel units relative to the integer point (bx, by); rows [ry0, ry1] and columns <= cx1 are the map
+__device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, double x1, double y1, double ry0, double ry1, double cx1) {
+    E.x0 = x0; E.y0 = y0; E.x1 = x1; E.y1 = y1; E.dx = x1 - x0; E.dy = y1 - y0;
+    E.n = 0; E.nX = 0; E.nY = 0; E.ta = 0.0; E.tb = 1.0; E.idx = 0.0; E.idy = 0.0; E.gx0 = 0.0; E.gy0 = 0.0; E.sx = 1.0; E.sy = 1.0;
+    if (E.dy == 0.0) return;                                   // a horizontal edge covers nothing
+    E.idy = 1.0 / E.dy;
+    double ta = 0.0, tb = 1.0;
+    {
+        double t0 = (ry0 - y0) * E.idy, t1 = (ry1 - y0) * E.idy;
+        ta = fmax(ta, fmin(t0, t1)); tb = fmin(tb, fmax(t0, t1));
+    }
+    if (E.dx != 0.0) {
+        E.idx = 1.0 / E.dx;
+        double tc = (cx1 - x0) * E.idx;
+        if (E.dx > 0.0) tb = fmin(tb, tc); else ta = fmax(ta, tc);
+    } else if (x0 >= cx1) return;
+    if (!(tb > ta)) return;
+    E.ta = ta; E.tb = tb;
+    const double xa = fma(ta, E.dx, x0), xb = fma(tb, E.dx, x0), ya = fma(ta, E.dy, y0), yb = fma(tb, E.dy, y0);
+    double nx, ny;
+    if (E.dx >= 0.0) { E.sx = 1.0; E.gx0 = floor(xa) + 1.0; nx = ceil(xb) - 1.0 - floor(xa); }
+    else { E.sx = -1.0; E.gx0 = ceil(xa) - 1.0; nx = ceil(xa) - 1.0 - floor(xb); }
+    if (E.dy > 0.0) { E.sy = 1.0; E.gy0 = floor(ya) + 1.0; ny = ceil(yb) - 1.0 - floor(ya); }
+    else { E.sy = -1.0; E.gy0 = ceil(ya) - 1.0; ny = ceil(ya) - 1.0 - floor(yb); }
+    E.nX = (E.dx != 0.0 && nx > 0.0) ? (int)fmin(nx, 1.0e6) : 0;
+    E.nY = (ny > 0.0) ? (int)fmin(ny, 1.0e6) : 0;
+    E.n = E.nX + E.nY + 1;
+}
+__device__ __forceinline__ double edge_tx(const EdgeWalk &E, int a) {
+    return fmin(fmax((E.gx0 + E.sx * (double)a - E.x0) * E.idx, E.ta), E.tb);
+}
+__device__ __forceinline__ double edge_ty(const EdgeWalk &E, int b) {
+    return fmin(fmax((E.gy0 + E.sy * (double)b - E.y0) * E.idy, E.ta), E.tb);
+}
+
+// Piece q of the edge (0 <= q < E.n): pieces [0, nX) start at the x-crossings, [nX, nX+nY) at the y-crossings,
+// the last one at the edge's (clipped) start.  At equal parameter an x-crossing comes before a y-crossing.
+// cs = -sign(A) ONE/|A|; (bx, by) = integer origin of the local coordinates.
+__device__ __forceinline__ void edge_piece(const ShootDev &S, const EdgeWalk &E, int q, double cs, int bx, int by) {
+    double ts, xs, ys, te;
+    int an, bn;                                                // next crossing of each family after the start
+    if (q < E.nX) {
+        ts = edge_tx(E, q);
+        xs = E.gx0 + E.sx * (double)q; ys = fma(ts, E.dy, E.y0);
+        an = q + 1;
+        bn = (int)fmin(fmax(((E.sy > 0.0) ? floor(ys) - E.gy0 : E.gy0 - ceil(ys)) + 1.0, 0.0), (double)E.nY);
+        while (bn > 0 && edge_ty(E, bn - 1) >= ts) --bn;
+        while (bn < E.nY && edge_ty(E, bn) < ts) ++bn;
+    } else if (q < E.nX + E.nY) {
+        const int b = q - E.nX;
+        ts = edge_ty(E, b);
+        ys = E.gy0 + E.sy * (double)b; xs = fma(ts, E.dx, E.x0);
+        bn = b + 1;
+        an = (int)fmin(fmax(((E.sx > 0.0) ? floor(xs) - E.gx0 : E.gx0 - ceil(xs)) + 1.0, 0.0), (double)E.nX);
+        while (an > 0 && edge_tx(E, an - 1) > ts) --an;
+        while (an < E.nX && edge_tx(E, an) <= ts) ++an;
+    } else {
+        ts = E.ta; xs = fma(ts, E.dx, E.x0); ys = fma(ts, E.dy, E.y0);
+        an = 0; bn = 0;
+    }
+    const double tX = (an < E.nX) ? edge_tx(E, an) : E.tb, tY = (bn < E.nY) ? edge_ty(E, bn) : E.tb;
+    double xe, ye;
+    if (tX <= tY && an < E.nX) { te = tX; xe = E.gx0 + E.sx * (double)an; ye = fma(te, E.dy, E.y0); }
+    else if (bn < E.nY) { te = tY; ye = E.gy0 + E.sy * (double)bn; xe = fma(te, E.dx, E.x0); }
+    else if (E.tb == 1.0) { te = 1.0; xe = E.x1; ye = E.y1; }      // the vertex itself: shared bit for bit with the next edge
+    else { te = E.tb; xe = fma(te, E.dx, E.x0); ye = fma(te, E.dy, E.y0); }
+    const long long tcov = __double2ll_rn(cs * ye) - __double2ll_rn(cs * ys);
+    if (tcov == 0) return;
+    const double ym = 0.5 * (ys + ye), xm = 0.5 * (xs + xe);
+    const int jr = (int)floor(ym) + by;
+    if ((unsigned)jr >= (unsigned)S.npix2) return;
+    const double fi = floor(xm);
+    const int ic = (int)fi + bx;
+    if (ic >= S.npix1) return;
+    long long r = tcov;                                        // left of the map: the whole cover enters at column 0
+    int c0 = 0;
+    if (ic >= 0) {
+        const double m = fmin(fmax(xm - fi, 0.0), 1.0);
+        r = __double2ll_rn((double)tcov * m);
+        c0 = ic + 1;
+        diff_add(S, ic, jr, (unsigned long long)(tcov - r));
+    }
+    if (c0 < S.npix1) diff_add(S, c0, jr, (unsigned long long)r);
+}
+
+struct TriSetup {
+    double x[3], y[3];                // local coordinates
+    double cs, ry0, ry1, cx1;
+    int bx, by;
+    int status;                       // 0: nothing to deposit, 1: walk the edges
+};
+
+// Reading G12: a triangle of zero area puts its whole weight into the pixel of vertex 0.  The same is done
+// when ONE/|A| times the triangle's height would leave the 63-bit range (aspect ratio beyond ~2^26).
+__device__ __forceinline__ void tri_setup(const ShootDev &S, const Win &W, const double *v, TriSetup &T) {
+    T.status = 0;
+    const double u0 = v[0], v0 = v[1], u1 = v[2], v1 = v[3], u2 = v[4], v2 = v[5];
+    const double mnx = fmin(u0, fmin(u1, u2)), mxx = fmax(u0, fmax(u1, u2));
+    const double mny = fmin(v0, fmin(v1, v2)), mxy = fmax(v0, fmax(v1, v2));
+    if (!(mxx >= 0.0) || !(mxy >= 0.0) || !(mnx < (double)S.npix1) || !(mny < (double)S.npix2)) return;   // also NaN
+    if (!(mnx > -1.0e9) || !(mny > -1.0e9) || !(mxx < 1.0e9) || !(mxy < 1.0e9)) return;                     // inf / absurd
+    const double fbx = floor(mnx), fby = floor(mny);
+    T.bx = (int)fbx; T.by = (int)fby;
+    T.x[0] = u0 - fbx; T.y[0] = v0 - fby; T.x[1] = u1 - fbx; T.y[1] = v1 - fby; T.x[2] = u2 - fbx; T.y[2] = v2 - fby;
+    const double A2 = (T.x[1] - T.x[0]) * (T.y[2] - T.y[0]) - (T.x[2] - T.x[0]) * (T.y[1] - T.y[0]);
+    const double hgt = mxy - fby + 1.0;
+    const double c = (A2 != 0.0) ? 2.0 * (double)FIX_ONE / fabs(A2) : 0.0;
+    if (A2 == 0.0 || !(c * hgt < 4.0e18)) {
+        pix_add(S, W, floor_to_int(u0), floor_to_int(v0), FIX_ONE);
+        return;
+    }
+    T.cs = (A2 > 0.0) ? -c : c;
+    T.ry0 = fmax(0.0, -fby); T.ry1 = fmin(hgt, (double)S.npix2 - fby); T.cx1 = (double)S.npix1 - fbx;
+    T.status = 1;
+}
+
+// Exact area of (triangle  intersect  unit pixel [qx, qx+1] x [qy, qy+1]) by Green's theorem: area = closed
+// integral of clamp(x - qx, 0, 1) dy over the part of the boundary with y in the pixel's row.  Same value as
+// Sutherland-Hodgman clipping + shoelace up to rounding; no polygon arrays, no data-dependent vertex
+// counts.  Signed like the triangle.  (x, y)[3] = vertices, (idx, idy)[3] = reciprocal edge vectors (0 if the
+// component is 0), edge k runs from vertex k to vertex k+1.
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }     // operands are never NaN here
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double clamp01(double v) { return dmin(dmax(v, 0.0), 1.0); }
+__device__ __forceinline__ double tri_pixel_area(const double (&x)[3], const double (&y)[3], const double (&idx)[3], const double (&idy)[3],
+                                                 double qx, double qy) {
+    double s = 0.0;
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+        const int e1 = (e == 2) ? 0 : e + 1;
+        const double dy = y[e1] - y[e];
+        if (dy == 0.0) continue;
+        const double px = x[e] - qx, py = y[e] - qy, dx = x[e1] - x[e];
+        const double ta = -py * idy[e], tb = (1.0 - py) * idy[e];
+        const double t0 = dmax(0.0, dmin(ta, tb)), t1 = dmin(1.0, dmax(ta, tb));
+        if (!(t1 > t0)) continue;
+        double integ;
+        if (dx == 0.0) {
+            integ = (t1 - t0) * clamp01(px);
+        } else {
+            const double sa = -px * idx[e], sb = (1.0 - px) * idx[e];
+            const double ua = dmax(t0, dmin(sa, sb)), ub = dmin(t1, dmax(sa, sb));
+            const double mid = (ub > ua) ? (ub - ua) * clamp01(fma(0.5 * (ua + ub), dx, px)) : 0.0;
+            const double over = (dx > 0.0) ? dmax(0.0, t1 - dmax(sb, t0)) : dmax(0.0, dmin(sb, t1) - t0);
+            integ = mid + over;
+        }
+        s = fma(dy, integ, s);
+    }
+    return s;
+}
+
+// Apportions n <= 32 pending general triangles of the warp's ring.  Lane = triangle for the set-up; then the
+// pixels of all the (clipped) bounding boxes of the batch are spread evenly over the lanes, each clipped
+// exactly against its triangle.  Triangles whose box holds more than S.small_px pixels go to the global queue
+// (edge walk in drain_kernel: cost ~ perimeter).  Out of line.  Returns the pixels this lane clipped.
+static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w32, int ax, int ay, WarpShared *Wsp, int head, int n) {
+    const ShootDev &S = *Sp;
+    WarpShared &Ws = *Wsp;
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
+    __syncwarp();
+    int npx = 0, done = 0;
+    if (lane < n) {
+        const double *v = Ws.ringE[(head + lane) & 63];
+        const double u0 = v[0], v0 = v[1], u1 = v[2], v1 = v[3], u2 = v[4], v2 = v[5];
+        const double mnx = fmin(u0, fmin(u1, u2)), mxx = fmax(u0, fmax(u1, u2));
+        const double mny = fmin(v0, fmin(v1, v2)), mxy = fmax(v0, fmax(v1, v2));
+        const bool sane = (mxx >= 0.0) && (mxy >= 0.0) && (mnx < (double)S.npix1) && (mny < (double)S.npix2) &&
+                          (mnx > -1.0e9) && (mny > -1.0e9) && (mxx < 1.0e9) && (mxy < 1.0e9);      // false for NaN too
+        if (sane) {
+            const double fbx = floor(mnx), fby = floor(mny);
+            const double x0 = u0 - fbx, y0 = v0 - fby, x1 = u1 - fbx, y1 = v1 - fby, x2 = u2 - fbx, y2 = v2 - fby;
+            const double A2 = (x1 - x0) * (y2 - y0) - (x2 - x0) * (y1 - y0);
+            if (A2 == 0.0) {                                    // reading G12: whole weight to the pixel of vertex 0
+                pix_add(S, W, floor_to_int(u0), floor_to_int(v0), FIX_ONE);
+            } else {
+                const int lox = max((int)fbx, 0), hix = min((int)floor(mxx), S.npix1 - 1);
+                const int loy = max((int)fby, 0), hiy = min((int)floor(mxy), S.npix2 - 1);
+                const long long wc = (long long)hix - lox + 1, hc = (long long)hiy - loy + 1;
+                if (wc > 0 && hc > 0) {
+                    bool big = false;
+                    if (wc * hc > (long long)S.small_px) {
+                        unsigned long long slot = atomicAdd(&S.counters[C_QUEUE], 1ull);
+                        if ((long long)slot < S.queue_cap) {
+                            double *qd = S.queue + (size_t)slot * QENT;
+#pragma unroll
+                            for (int k = 0; k < QENT; ++k) qd[k] = v[k];
+                            atomicAdd(&S.counters[C_QUEUED], 1ull);
+                            big = true;
+                        } else atomicAdd(&S.counters[C_OVERFLOW], 1ull);   // queue full: clipped here, pixel by pixel
+                    }
+                    if (!big) {
+                        npx = (int)((wc * hc < (1ll << 26)) ? wc * hc : (1ll << 26));   // (only a full queue can bring such boxes here)
+                        double *rc = Ws.rec[lane];
+                        rc[0] = 2.0 / A2;
+                        rc[1] = __hiloint2double(loy, lox);
+                        rc[2] = __hiloint2double((int)fby, (int)fbx);
+                        rc[3] = __hiloint2double(0, (int)wc);
+                        const double dx0 = x1 - x0, dx1 = x2 - x1, dx2 = x0 - x2, dy0 = y1 - y0, dy1 = y2 - y1, dy2 = y0 - y2;
+                        rc[4] = (dx0 != 0.0) ? fast_rcp(fabs(dx0)) * (dx0 < 0.0 ? -1.0 : 1.0) : 0.0;
+                        rc[5] = (dx1 != 0.0) ? fast_rcp(fabs(dx1)) * (dx1 < 0.0 ? -1.0 : 1.0) : 0.0;
+                        rc[6] = (dx2 != 0.0) ? fast_rcp(fabs(dx2)) * (dx2 < 0.0 ? -1.0 : 1.0) : 0.0;
+                        rc[7] = (dy0 != 0.0) ? fast_rcp(fabs(dy0)) * (dy0 < 0.0 ? -1.0 : 1.0) : 0.0;
+                        rc[8] = (dy1 != 0.0) ? fast_rcp(fabs(dy1)) * (dy1 < 0.0 ? -1.0 : 1.0) : 0.0;
+                        rc[9] = (dy2 != 0.0) ? fast_rcp(fabs(dy2)) * (dy2 < 0.0 ? -1.0 : 1.0) : 0.0;
+                    }
+                }
+            }
+        }
+    }
+    int inc = npx;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(full, inc, o); if (lane >= o) inc += t; }
+    const int total = __shfl_sync(full, inc, 31);
+    __syncwarp();
+#pragma unroll 1
+    for (int k0 = 0; k0 < total; k0 += 32) {
+        const int k = k0 + lane;
+        int i = 0;                                              // first triangle whose inclusive prefix exceeds k
+#pragma unroll
+        for (int step = 16; step; step >>= 1) {
+            int v = __shfl_sync(full, inc, (i + step - 1) & 31);
+            if (v <= k) i += step;
+        }
+        i &= 31;
+        const int incl = __shfl_sync(full, inc, i), cnt = __shfl_sync(full, npx, i);
+        if (k < total) {
+            const int m = k - (incl - cnt);
+            const double *v = Ws.ringE[(head + i) & 63];
+            const double *rc = Ws.rec[i];
+            const int lox = __double2loint(rc[1]), loy = __double2hiint(rc[1]);
+            const int bx = __double2loint(rc[2]), by = __double2hiint(rc[2]);
+            const int wc = __double2loint(rc[3]);
+            const int py = loy + m / wc, px = lox + m % wc;
+            const double fbx = (double)bx, fby = (double)by;
+            const double x[3] = {v[0] - fbx, v[2] - fbx, v[4] - fbx}, y[3] = {v[1] - fby, v[3] - fby, v[5] - fby};
+            const double idx[3] = {rc[4], rc[5], rc[6]}, idy[3] = {rc[7], rc[8], rc[9]};
+            const double a = tri_pixel_area(x, y, idx, idy, (double)(px - bx), (double)(py - by));
+            pix_add(S, W, px, py, to_fix(a * rc[0]));
+            ++done;
+        }
+    }
+    __syncwarp();
+    return done;
+}
+
+}  // namespace ml

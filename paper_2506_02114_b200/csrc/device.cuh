@@ -24,6 +24,15 @@ __host__ __device__ __forceinline__ double2 cpowi(double2 a, int n) {     // a^n
     return r;
 }
 
+// 1/a to double precision from the 20-bit hardware seed: one cubic step, e^3 ~ 2^-60 (a normal, finite, > 0)
+__device__ __forceinline__ double fast_rcp(double a) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    double e = fma(-a, y, 1.0);
+    double t = fma(e, e, e);
+    return fma(y, t, y);
+}
+
 // ---- everything a kernel needs to evaluate the lens equation (eq 12)
 struct LensDev {
     double one_minus_kappa, gamma, kappa_star, theta2;
@@ -99,15 +108,8 @@ __device__ __forceinline__ double2 zlogz(double2 v) {
     return cmul(v, lg);
 }
 
-// Smooth-sheet deflection alpha_s: disc eq 19 (P:176), rectangle eq B7 (P:588-593).
-__device__ __forceinline__ void sheet(const LensDev &L, double x, double y, double &ax, double &ay) {
-    if (L.shape == MLENS_SHAPE_DISC) {
-        double r2 = x * x + y * y;
-        if (r2 <= L.R2) { ax = -L.kappa_star * x; ay = -L.kappa_star * y; }
-        else { double q = L.kappa_star * L.R2 / r2; ax = -q * x; ay = -q * y; }
-        return;
-    }
-    const double c1 = L.c1, c2 = L.c2, ks = L.kappa_star;
+// Smooth-sheet deflection alpha_s of a rectangle, eq B7.  Kept out of line: four complex logarithms.
+static __device__ __noinline__ double2 sheet_rect(double c1, double c2, double ks, double x, double y) {
     // conj z = (x, -y); corners c = (c1, c2), conj c = (c1, -c2)
     double2 t1 = zlogz(make_double2(c1 - x, c2 + y));       //  c - conj z
     double2 t2 = zlogz(make_double2(c1 - x, -c2 + y));      //  conj c - conj z
@@ -120,7 +122,19 @@ __device__ __forceinline__ void sheet(const LensDev &L, double x, double y, doub
     bool in2 = (y >= -c2) && (y <= c2);
     if (in2 && x >= -c1 && x <= c1) rx -= ks * (2.0 * c1 + 2.0 * x);
     if (in2 && x - c1 >= 0.0) rx -= ks * 4.0 * c1;
-    ax = rx; ay = ry;
+    return make_double2(rx, ry);
+}
+
+// Smooth-sheet deflection alpha_s: disc eq 19 (P:176), rectangle eq B7 (P:588-593).
+__device__ __forceinline__ void sheet(const LensDev &L, double x, double y, double &ax, double &ay) {
+    if (L.shape == MLENS_SHAPE_DISC) {
+        double r2 = x * x + y * y;
+        if (r2 <= L.R2) { ax = -L.kappa_star * x; ay = -L.kappa_star * y; }
+        else { double q = L.kappa_star * L.R2 * fast_rcp(r2); ax = -q * x; ay = -q * y; }
+        return;
+    }
+    double2 a = sheet_rect(L.c1, L.c2, L.kappa_star, x, y);
+    ax = a.x; ay = a.y;
 }
 
 // All stars, for DIRECT mode and rays outside the root square.
@@ -157,6 +171,18 @@ __device__ __forceinline__ void alpha_fmm_global(const LensDev &L, double x, dou
     far_horner(L.ecoef + (size_t)leaf * L.p1, L.p, (x - cx) * inv, (y - cy) * inv, fx, fy);
     ax = fma(L.theta2, nx_, fx);
     ay = fma(L.theta2, ny_, fy);
+}
+
+// Out-of-line copies for the shooting kernels' rare paths (keeps their hot loops inside the instruction cache).
+static __device__ __noinline__ double2 alpha_fmm_global_ool(const LensDev *L, double x, double y) {
+    double ax, ay;
+    alpha_fmm_global(*L, x, y, ax, ay);
+    return make_double2(ax, ay);
+}
+static __device__ __noinline__ double2 direct_all_ool(const LensDev *L, double x, double y) {
+    double ax, ay;
+    direct_all(*L, x, y, ax, ay);
+    return make_double2(ax * L->theta2, ay * L->theta2);
 }
 
 // w of eq 12 from alpha_star: w = (1-kappa) z + gamma conj z - alpha_star - alpha_s

@@ -1,0 +1,323 @@
+// tile.cuh -- warp-autonomous ray-tile evaluator (hot loop A): every warp owns a 32 x 32 tile of rays,
+// builds the tile's own expansion with warp-level primitives only (no block barrier anywhere) and then
+// evaluates eq 12 for four rays per lane at a time.
+//
+// Targets outnumber sources by 10^4..10^5, so the FMM hierarchy is continued on the target side
+// (DESIGN.md s5.4): for every ray tile the leaf's local series is shifted to the tile centre (eq C7 once
+// more) and the leaf's near-field stars that are far from the tile on the tile's scale are added to it
+// (eq C6); what is left per ray is a ~13-term Horner sum plus the few stars within ~10 tile radii.  Both
+// truncations are bounded per tile from the coefficients themselves; a tile whose bound fails evaluates
+// the leaf's full series and full star list instead.
+#pragma once
+#include "device.cuh"
+
+namespace ml {
+
+static const int TCX = 32;            // rays per tile row (= warp width, one column per lane)
+static const int TCY = 32;            // ray rows per tile
+static const int RPT = 4;             // rays a lane evaluates together (independent Horner chains)
+static const int NGRP = TCY / RPT;
+static const int TQMAX = 15;          // highest order of the tile series
+static const int NSLOT = 2;           // leaves a tile keeps a series for (rays in further leaves go through the tree)
+static const int WX = 32, WY = 16;    // per-warp shared-memory pixel window
+static const int FOLDJ = WX * WY * 8 / (32 * 16);   // series terms per pass of the star folding (scratch = the window)
+static const int BN = 2 * ML_P1MAX;   // stride of the Pascal triangle
+
+// What a shooting kernel needs besides the lens: the ray grid, the map, the accumulators.
+struct ShootDev {
+    LensDev L;
+    double x0_1, x0_2, h1, h2;
+    long long i0, i1, j0, j1;          // cell sub-range
+    double ylo1, ylo2, p1, p2, inv_p1, inv_p2;
+    int npix1, npix2;
+    unsigned long long *acc;           // fixed-point pixel sums (IPM) or ray counts (IRS)
+    unsigned long long *diff;          // IPM: row-difference array written by the edge walk of large triangles
+    double *queue;                     // giant-triangle queue, QENT doubles per entry
+    unsigned long long *counters;
+    long long queue_cap;
+    double *dump1, *dump2;
+    const double *binom;               // Pascal triangle, stride BN
+    int eval_mode;
+    int ntx;                           // tiles along x1
+    long long tile_row0, tile_rows;    // band of tile rows handled by this launch
+    int tq;                            // order of the tile series
+    double eps_far, eps_star;          // truncation budgets of the tile series (absolute, units of theta)
+    int dbg;
+    int small_px;                      // triangles whose bounding box has more pixels than this go to the global queue
+};
+
+__device__ __forceinline__ double corner_x(const ShootDev &S, long long i) { return __dadd_rn(S.x0_1, __dmul_rn((double)i, S.h1)); }
+__device__ __forceinline__ double corner_y(const ShootDev &S, long long j) { return __dadd_rn(S.x0_2, __dmul_rn((double)j, S.h2)); }
+
+// Per-warp shared memory.  `win` doubles as the scratch of the tile set-up (fold terms), which is why it
+// is zeroed at the end of the set-up and not by the flush.
+struct WarpShared {
+    unsigned long long win[WY * WX];                         // 4 KB
+    double2 t[NSLOT][TQMAX + 1];                                 // conj(alpha)(u) = sum_j t_j u^j, theta^2 included
+    double sx[NSLOT][ML_NEAR], sy[NSLOT][ML_NEAR], sm[NSLOT][ML_NEAR];   // direct stars (absolute positions, m theta^2)
+    double2 e[ML_P1MAX];                                     // the leaf's derivative series (set-up scratch)
+    uint32_t bx0[NSLOT], bx1[NSLOT], by0[NSLOT], by1[NSLOT];
+    int leaf[NSLOT], node[NSLOT], nd[NSLOT], mode[NSLOT];
+    double ringE[64][6];                                     // pending general triangles (3 vertices, pixel units)
+    double ringS[64][4];                                     // pending two-pixel strips
+    double rec[32][10];                                      // per-triangle records of the batch being apportioned
+    double stu[RPT + 1][32], stv[RPT + 1][32];               // mapped corners of the row group in pixel units (row 0 = last row of the previous group)
+    int stp[RPT + 1][32];                                    // their packed pixels
+};
+static_assert(FOLDJ >= 4 && ML_NEAR == 32, "fold scratch must fit the window");
+
+struct TileCtx {                       // warp-uniform registers
+    double zt_x, zt_y, inv_rt;
+    bool fast;                         // the whole tile sits in one leaf whose tile series passed its bound
+};
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Builds slot `s` of the warp's tile: shifted series + folded stars + direct-star list.
+__device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &W, const TileCtx &C, int s, double rt) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int p = S.L.p, Q = S.tq;
+    const int leaf = W.leaf[s], node = W.node[s];
+    const int lev = __ldg(&S.L.level[node]);
+    const double half = S.L.root_half / (double)(1 << lev);
+    const double cx = -S.L.root_half + (2.0 * __ldg(&S.L.ix[node]) + 1.0) * half;
+    const double cy = -S.L.root_half + (2.0 * __ldg(&S.L.iy[node]) + 1.0) * half;
+    const int cnt = __ldg(&S.L.near_cnt[leaf]);
+    for (int j = lane; j < p; j += 32) W.e[j] = S.L.ecoef[(size_t)leaf * S.L.p1 + j];
+    __syncwarp();
+    // ---- shift of the derivative series to the tile centre: T_j = rho^j sum_m e_{j+m} C(j+m, j) zeta_t^m   (eq C7)
+    const double rho = rt / half;
+    const double zr = (C.zt_x - cx) / half, zi = (C.zt_y - cy) / half;
+    double tail = 0.0;
+    for (int j = lane; j < p; j += 32) {
+        double ar = 0.0, ai = 0.0;
+        for (int m = p - 1 - j; m >= 0; --m) {
+            double bc = __ldg(&S.binom[(size_t)(j + m) * BN + j]);
+            double2 c = W.e[j + m];
+            double tr = fma(ar, zr, fma(-ai, zi, bc * c.x));
+            double ti = fma(ar, zi, fma(ai, zr, bc * c.y));
+            ar = tr; ai = ti;
+        }
+        double sc = 1.0;
+        for (int k = 0; k < j; ++k) sc *= rho;
+        ar *= sc; ai *= sc;
+        if (j <= Q) W.t[s][j] = make_double2(ar, ai);
+        else tail += fabs(ar) + fabs(ai);
+    }
+    for (int j = p + lane; j <= Q; j += 32) W.t[s][j] = make_double2(0.0, 0.0);
+    tail = warp_sum(tail);
+    // ---- near-field stars (lane k = star k): far from the tile on the tile's scale -> series (eq C6), else direct
+    double2 *fold = reinterpret_cast<double2 *>(W.win);          // [FOLDJ][32]
+    {
+        const int k = lane;
+        bool have = k < cnt, direct = false;
+        double x = 0, y = 0, m = 0;
+        double2 term = make_double2(0.0, 0.0), w = make_double2(0.0, 0.0);
+        if (have) {
+            size_t o = (size_t)leaf * ML_NEAR + k;
+            x = S.L.near_x[o]; y = S.L.near_y[o]; m = S.L.near_m[o] * S.L.theta2;
+            double dx = x - C.zt_x, dy = y - C.zt_y;
+            double d2 = dx * dx + dy * dy, d = sqrt(d2);
+            double r = (d > 0.0) ? rt / d : 2.0;
+            direct = true;
+            if (r < 0.5) {
+                double rq = r;
+                for (int k2 = 0; k2 < Q; ++k2) rq *= r;                  // r^(Q+1)
+                double bound = (m / d) * rq / (1.0 - r);
+                if (bound <= S.eps_star) {
+                    direct = false;
+                    // conj(alpha_i) = m/(eta - d) = -(m/d) sum_j (eta/d)^j ; with eta = rt u: term_j = -(m/d)(rt/d)^j
+                    double id2 = 1.0 / d2;
+                    term = make_double2(-m * dx * id2, m * dy * id2);     // -m/d = -m conj(d)/|d|^2
+                    w = make_double2(rt * dx * id2, -rt * dy * id2);      // rt/d
+                }
+            }
+        }
+        const unsigned fm = __ballot_sync(full, have && !direct);
+        const unsigned dm = __ballot_sync(full, direct);
+        if (direct) {
+            int pos = __popc(dm & ((1u << k) - 1u));
+            W.sx[s][pos] = x; W.sy[s][pos] = y; W.sm[s][pos] = m;
+        }
+        if (k == 0) { W.nd[s] = __popc(dm); W.mode[s] = (tail <= S.eps_far) ? 0 : 1; }
+        if (fm) {
+            // FOLDJ series terms per pass: lane = star writes its terms, lane = term sums over the stars
+            for (int j0 = 0; j0 <= Q; j0 += FOLDJ) {
+                __syncwarp();
+#pragma unroll
+                for (int j = 0; j < FOLDJ; ++j) { fold[j * 32 + k] = term; term = cmul(term, w); }
+                __syncwarp();
+                if (lane < FOLDJ && j0 + lane <= Q) {
+                    double2 a = W.t[s][j0 + lane];
+#pragma unroll 8
+                    for (int kk = 0; kk < 32; ++kk) { double2 f = fold[lane * 32 + kk]; a.x += f.x; a.y += f.y; }
+                    W.t[s][j0 + lane] = a;
+                }
+            }
+        }
+    }
+    __syncwarp();
+}
+
+__device__ __forceinline__ void zero_window(WarpShared &W) {
+    const int lane = threadIdx.x & 31;
+    ulonglong2 *w2 = reinterpret_cast<ulonglong2 *>(W.win);
+#pragma unroll
+    for (int k = 0; k < WY * WX / 64; ++k) w2[k * 32 + lane] = make_ulonglong2(0ull, 0ull);
+}
+
+// Sets up the warp's tile: centre, radius, leaves of the four extreme rays, one slot per distinct leaf.
+// off = offset of the rays from the grid corners in cells (0 for IPM, 0.5 for IRS).  Leaves the window zeroed.
+__device__ __forceinline__ void wtile_setup(const ShootDev &S, WarpShared &W, TileCtx &C, long long ci0, long long cj0,
+                                            long long ci1, long long cj1, double off, unsigned long long *full_counter) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    C.inv_rt = 1.0; C.fast = false; C.zt_x = 0.0; C.zt_y = 0.0;
+    if (S.eval_mode != MLENS_EVAL_FMM) { zero_window(W); __syncwarp(); return; }
+    const double rt = 0.5 * sqrt((double)((TCX - 1) * (TCX - 1)) * S.h1 * S.h1 + (double)((TCY - 1) * (TCY - 1)) * S.h2 * S.h2) * (1.0 + 1e-9);
+    C.zt_x = corner_x(S, ci0) + (0.5 * (TCX - 1) + off) * S.h1;
+    C.zt_y = corner_y(S, cj0) + (0.5 * (TCY - 1) + off) * S.h2;
+    C.inv_rt = 1.0 / rt;
+    int leaf = -1, node = -1;
+    uint32_t b0x = 0, b1x = 0, b0y = 0, b1y = 0;
+    if (lane < 4) {
+        double x = corner_x(S, (lane & 1) ? ci1 : ci0) + off * S.h1, y = corner_y(S, (lane & 2) ? cj1 : cj0) + off * S.h2;
+        uint32_t qx, qy;
+        if (quantise(S.L, x, y, qx, qy)) {
+            node = find_leaf_node(S.L, qx, qy);
+            int lev = __ldg(&S.L.level[node]), ix = __ldg(&S.L.ix[node]), iy = __ldg(&S.L.iy[node]);
+            int sh = ML_QBITS - lev;
+            leaf = __ldg(&S.L.leaf_id[node]);
+            b0x = (uint32_t)ix << sh; b1x = (uint32_t)(ix + 1) << sh;
+            b0y = (uint32_t)iy << sh; b1y = (uint32_t)(iy + 1) << sh;
+        }
+    }
+    const int l0 = __shfl_sync(full, leaf, 0), l1 = __shfl_sync(full, leaf, 1), l2 = __shfl_sync(full, leaf, 2), l3 = __shfl_sync(full, leaf, 3);
+    const bool one_leaf = l0 >= 0 && l1 == l0 && l2 == l0 && l3 == l0;
+    {
+        // one slot per distinct leaf, in corner order, at most NSLOT of them
+        bool dup = (lane > 0 && leaf == l0) || (lane > 1 && leaf == l1) || (lane > 2 && leaf == l2);
+        const bool keep = lane < 4 && leaf >= 0 && !dup;
+        const unsigned km = __ballot_sync(full, keep);
+        const int slot = __popc(km & ((1u << lane) - 1u));
+        if (lane < NSLOT) { W.leaf[lane] = -1; W.node[lane] = -1; W.nd[lane] = 0; W.mode[lane] = -1; }
+        __syncwarp();
+        if (keep && slot < NSLOT) {
+            W.leaf[slot] = leaf; W.node[slot] = node;
+            W.bx0[slot] = b0x; W.bx1[slot] = b1x; W.by0[slot] = b0y; W.by1[slot] = b1y;
+        }
+    }
+    __syncwarp();
+    for (int s = 0; s < NSLOT; ++s) {
+        if (W.leaf[s] < 0) continue;                              // warp-uniform
+        wtile_build_slot(S, W, C, s, rt);
+        if (lane == 0 && W.mode[s] == 1 && full_counter) atomicAdd(full_counter, 1ull);
+    }
+    zero_window(W);
+    __syncwarp();
+    C.fast = one_leaf && W.mode[0] == 0;
+}
+
+struct ThreadCounters { unsigned int single = 0, small_ = 0, queued = 0, chunks = 0, overflow = 0, fallback = 0, rays = 0, near_ = 0, px_small = 0; };
+
+// One ray of a tile that straddles leaves (or whose series failed its bound), out of line: the slot of the
+// ray's leaf if the tile has one for it, else the tree.  Returns alpha_star.
+static __device__ __noinline__ double2 eval_one_ool(const ShootDev *Sp, const WarpShared *T, double x, double y, double ux, double uy, int *kind) {
+    int s = -1;
+    uint32_t qx, qy;
+    if (quantise(Sp->L, x, y, qx, qy)) {
+#pragma unroll 1
+        for (int k = 0; k < NSLOT; ++k)
+            if (T->leaf[k] >= 0 && qx >= T->bx0[k] && qx < T->bx1[k] && qy >= T->by0[k] && qy < T->by1[k]) s = k;
+    }
+    if (s >= 0 && T->mode[s] != 0) s = -1;
+    if (s < 0) { *kind = -1; return alpha_fmm_global_ool(&Sp->L, x, y); }
+    const int Q = Sp->tq;
+    double sr = T->t[s][Q].x, si = T->t[s][Q].y;
+    for (int j = Q - 1; j >= 0; --j) {
+        double2 c = T->t[s][j];
+        double tr = fma(sr, ux, fma(-si, uy, c.x));
+        double ti = fma(sr, uy, fma(si, ux, c.y));
+        sr = tr; si = ti;
+    }
+    const int nd = T->nd[s];
+    for (int k = 0; k < nd; ++k) {
+        double dx = x - T->sx[s][k], dy = y - T->sy[s][k];
+        double r2 = fma(dx, dx, dy * dy);
+        double q = (__double2hiint(r2) >= 0x00100000) ? T->sm[s][k] * fast_rcp(r2) : 0.0;
+        sr = fma(q, dx, sr);
+        si = fma(-q, dy, si);
+    }
+    *kind = nd;
+    return make_double2(sr, -si);
+}
+
+// w(z) of eq 12 for the RPT rays of one lane (same column, consecutive rows).
+__device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T, const TileCtx &C, const double (&x)[RPT],
+                                          const double (&y)[RPT], const double (&ux)[RPT], const double (&uy)[RPT],
+                                          const bool (&valid)[RPT], double (&wx)[RPT], double (&wy)[RPT], ThreadCounters &tc) {
+    double ax[RPT], ay[RPT];
+    bool all = true;
+#pragma unroll
+    for (int r = 0; r < RPT; ++r) all = all && valid[r];
+    if (C.fast && all) {
+        // the common case: the whole tile in one leaf, RPT independent Horner chains share every coefficient load
+        const int Q = S.tq;
+        const double2 *t = T.t[0];
+        double sr[RPT], si[RPT];
+        double2 c = t[Q];
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { sr[r] = c.x; si[r] = c.y; }
+        for (int j = Q - 1; j >= 0; --j) {
+            c = t[j];
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                double tr = fma(sr[r], ux[r], fma(-si[r], uy[r], c.x));
+                double ti = fma(sr[r], uy[r], fma(si[r], ux[r], c.y));
+                sr[r] = tr; si[r] = ti;
+            }
+        }
+        const int nd = T.nd[0];
+        tc.rays += RPT;
+        tc.near_ += (unsigned int)(nd * RPT);
+        for (int k = 0; k < nd; ++k) {
+            double X = T.sx[0][k], Y = T.sy[0][k], M = T.sm[0][k];
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                double dx = x[r] - X, dy = y[r] - Y;
+                double r2 = fma(dx, dx, dy * dy);
+                double q = (__double2hiint(r2) >= 0x00100000) ? M * fast_rcp(r2) : 0.0;   // reading G11: skip r = 0
+                sr[r] = fma(q, dx, sr[r]);
+                si[r] = fma(-q, dy, si[r]);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { ax[r] = sr[r]; ay[r] = -si[r]; }
+    } else {
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) {
+            ax[r] = ay[r] = 0.0;
+            if (!valid[r]) continue;
+            ++tc.rays;
+            double2 a;
+            if (S.eval_mode == MLENS_EVAL_DIRECT) a = direct_all_ool(&S.L, x[r], y[r]);
+            else {
+                int kind;
+                a = eval_one_ool(&S, &T, x[r], y[r], ux[r], uy[r], &kind);
+                if (kind >= 0) tc.near_ += (unsigned int)kind; else ++tc.fallback;
+            }
+            ax[r] = a.x; ay[r] = a.y;
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < RPT; ++r)
+        if (valid[r]) lens_w(S.L, x[r], y[r], ax[r], ay[r], wx[r], wy[r]);
+        else { wx[r] = 0.0; wy[r] = 0.0; }
+}
+
+}  // namespace ml
