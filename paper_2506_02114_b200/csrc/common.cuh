@@ -98,7 +98,9 @@ struct mlens_field {
     // shoot scratch
     ml::DevBuf<unsigned long long> acc;  // fixed-point / count accumulator, npix
     ml::DevBuf<unsigned long long> diff; // row-difference array of interior runs (IPM), npix
-    ml::DevBuf<double> queue;            // large-triangle queue
+    ml::DevBuf<double> queue;            // general-triangle queue
+    ml::DevBuf<int> qcount;              // entries per queue chunk
+    ml::DevBuf<unsigned int> biglist;    // queue entries to be walked edge by edge
     ml::DevBuf<unsigned long long> counters;
     int device = 0;
 };

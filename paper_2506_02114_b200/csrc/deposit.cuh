@@ -22,10 +22,11 @@ namespace ml {
 
 static const int FIXBITS = 36;
 static const unsigned long long FIX_ONE = 1ull << FIXBITS;
-static const int QENT = 6;                 // doubles per giant-queue entry: the 3 vertices in pixel units
+static const int QENT = 6;                 // doubles per queue entry: the 3 vertices in pixel units
+static const int QCHUNK = 256;             // queue entries a warp reserves at a time
 
 enum { C_QUEUE = 0, C_TILE, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR,
-       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_NCOUNTERS };
+       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_BIG, C_WALK, C_NCOUNTERS };
 
 struct Win {                           // where a warp's deposits go (uniform registers)
     unsigned int *w32;                 // the warp's shared window viewed as 32-bit halves, or nullptr
@@ -137,16 +138,20 @@ static __device__ __noinline__ void strip2_batch(const ShootDev *Sp, unsigned in
 }
 
 // ---- the edge walk ------------------------------------------------------------------------------------------
+// An edge is walked along its MAJOR axis: between two consecutive grid lines of that axis it stays inside one
+// row (or column) of pixels and, its slope being <= 1, crosses at most one grid line of the other axis -- so a
+// step yields one or two pieces, found without any search, and the steps are independent (one per lane).
 struct EdgeWalk {                     // one triangle edge, clipped to the map rows and to the columns left of the map's right border
     double x0, y0, x1, y1, dx, dy, idx, idy, ta, tb;
-    double gx0, gy0, sx, sy;          // first grid line crossed along each axis and the step (+-1)
-    int nX, nY, n;                    // crossings and pieces (n = nX + nY + 1, or 0)
+    double g0, sg;                    // first grid line crossed along the major axis and the step (+-1)
+    int majorY;                       // 1: walk rows (|dy| >= |dx|), 0: walk columns
+    int n;                            // steps = crossings of major-axis grid lines + 1, or 0
 };
 
 // local coordinates: pixel units relative to the integer point (bx, by); rows [ry0, ry1] and columns <= cx1 are the map
 __device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, double x1, double y1, double ry0, double ry1, double cx1) {
     E.x0 = x0; E.y0 = y0; E.x1 = x1; E.y1 = y1; E.dx = x1 - x0; E.dy = y1 - y0;
-    E.n = 0; E.nX = 0; E.nY = 0; E.ta = 0.0; E.tb = 1.0; E.idx = 0.0; E.idy = 0.0; E.gx0 = 0.0; E.gy0 = 0.0; E.sx = 1.0; E.sy = 1.0;
+    E.n = 0; E.ta = 0.0; E.tb = 1.0; E.idx = 0.0; E.idy = 0.0; E.g0 = 0.0; E.sg = 1.0; E.majorY = 1;
     if (E.dy == 0.0) return;                                   // a horizontal edge covers nothing
     E.idy = 1.0 / E.dy;
     double ta = 0.0, tb = 1.0;
@@ -161,54 +166,18 @@ __device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, do
     } else if (x0 >= cx1) return;
     if (!(tb > ta)) return;
     E.ta = ta; E.tb = tb;
-    const double xa = fma(ta, E.dx, x0), xb = fma(tb, E.dx, x0), ya = fma(ta, E.dy, y0), yb = fma(tb, E.dy, y0);
-    double nx, ny;
-    if (E.dx >= 0.0) { E.sx = 1.0; E.gx0 = floor(xa) + 1.0; nx = ceil(xb) - 1.0 - floor(xa); }
-    else { E.sx = -1.0; E.gx0 = ceil(xa) - 1.0; nx = ceil(xa) - 1.0 - floor(xb); }
-    if (E.dy > 0.0) { E.sy = 1.0; E.gy0 = floor(ya) + 1.0; ny = ceil(yb) - 1.0 - floor(ya); }
-    else { E.sy = -1.0; E.gy0 = ceil(ya) - 1.0; ny = ceil(ya) - 1.0 - floor(yb); }
-    E.nX = (E.dx != 0.0 && nx > 0.0) ? (int)fmin(nx, 1.0e6) : 0;
-    E.nY = (ny > 0.0) ? (int)fmin(ny, 1.0e6) : 0;
-    E.n = E.nX + E.nY + 1;
-}
-__device__ __forceinline__ double edge_tx(const EdgeWalk &E, int a) {
-    return fmin(fmax((E.gx0 + E.sx * (double)a - E.x0) * E.idx, E.ta), E.tb);
-}
-__device__ __forceinline__ double edge_ty(const EdgeWalk &E, int b) {
-    return fmin(fmax((E.gy0 + E.sy * (double)b - E.y0) * E.idy, E.ta), E.tb);
+    E.majorY = fabs(E.dy) >= fabs(E.dx);
+    const double d = E.majorY ? E.dy : E.dx, c0 = E.majorY ? y0 : x0;
+    const double a = fma(ta, d, c0), b = fma(tb, d, c0);       // major coordinate at the clipped ends
+    double nc;
+    if (d > 0.0) { E.sg = 1.0; E.g0 = floor(a) + 1.0; nc = ceil(b) - 1.0 - floor(a); }
+    else { E.sg = -1.0; E.g0 = ceil(a) - 1.0; nc = ceil(a) - 1.0 - floor(b); }
+    E.n = ((nc > 0.0) ? (int)fmin(nc, 1.0e7) : 0) + 1;
 }
 
-// Piece q of the edge (0 <= q < E.n): pieces [0, nX) start at the x-crossings, [nX, nX+nY) at the y-crossings,
-// the last one at the edge's (clipped) start.  At equal parameter an x-crossing comes before a y-crossing.
-// cs = -sign(A) ONE/|A|; (bx, by) = integer origin of the local coordinates.
-__device__ __forceinline__ void edge_piece(const ShootDev &S, const EdgeWalk &E, int q, double cs, int bx, int by) {
-    double ts, xs, ys, te;
-    int an, bn;                                                // next crossing of each family after the start
-    if (q < E.nX) {
-        ts = edge_tx(E, q);
-        xs = E.gx0 + E.sx * (double)q; ys = fma(ts, E.dy, E.y0);
-        an = q + 1;
-        bn = (int)fmin(fmax(((E.sy > 0.0) ? floor(ys) - E.gy0 : E.gy0 - ceil(ys)) + 1.0, 0.0), (double)E.nY);
-        while (bn > 0 && edge_ty(E, bn - 1) >= ts) --bn;
-        while (bn < E.nY && edge_ty(E, bn) < ts) ++bn;
-    } else if (q < E.nX + E.nY) {
-        const int b = q - E.nX;
-        ts = edge_ty(E, b);
-        ys = E.gy0 + E.sy * (double)b; xs = fma(ts, E.dx, E.x0);
-        bn = b + 1;
-        an = (int)fmin(fmax(((E.sx > 0.0) ? floor(xs) - E.gx0 : E.gx0 - ceil(xs)) + 1.0, 0.0), (double)E.nX);
-        while (an > 0 && edge_tx(E, an - 1) > ts) --an;
-        while (an < E.nX && edge_tx(E, an) <= ts) ++an;
-    } else {
-        ts = E.ta; xs = fma(ts, E.dx, E.x0); ys = fma(ts, E.dy, E.y0);
-        an = 0; bn = 0;
-    }
-    const double tX = (an < E.nX) ? edge_tx(E, an) : E.tb, tY = (bn < E.nY) ? edge_ty(E, bn) : E.tb;
-    double xe, ye;
-    if (tX <= tY && an < E.nX) { te = tX; xe = E.gx0 + E.sx * (double)an; ye = fma(te, E.dy, E.y0); }
-    else if (bn < E.nY) { te = tY; ye = E.gy0 + E.sy * (double)bn; xe = fma(te, E.dx, E.x0); }
-    else if (E.tb == 1.0) { te = 1.0; xe = E.x1; ye = E.y1; }      // the vertex itself: shared bit for bit with the next edge
-    else { te = E.tb; xe = fma(te, E.dx, E.x0); ye = fma(te, E.dy, E.y0); }
+// One piece of an edge, from (xs, ys) to (xe, ye), inside one pixel.  cs = -sign(A) ONE/|A|; (bx, by) = integer
+// origin of the local coordinates.  The cover G(ye) - G(ys) telescopes exactly along the triangle's boundary.
+__device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, double ys, double xe, double ye, double cs, int bx, int by) {
     const long long tcov = __double2ll_rn(cs * ye) - __double2ll_rn(cs * ys);
     if (tcov == 0) return;
     const double ym = 0.5 * (ys + ye), xm = 0.5 * (xs + xe);
@@ -226,6 +195,36 @@ __device__ __forceinline__ void edge_piece(const ShootDev &S, const EdgeWalk &E,
         diff_add(S, ic, jr, (unsigned long long)(tcov - r));
     }
     if (c0 < S.npix1) diff_add(S, c0, jr, (unsigned long long)r);
+}
+
+// Step k of the edge (0 <= k < E.n): from major-axis grid line k-1 (or the clipped start) to grid line k (or the
+// clipped end).  End points on a grid line take its exact value and an unclipped end the vertex itself, so
+// consecutive steps and consecutive edges share their end points bit for bit.
+__device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, int k, double cs, int bx, int by) {
+    const double d = E.majorY ? E.dy : E.dx, c0 = E.majorY ? E.y0 : E.x0, id = E.majorY ? E.idy : E.idx;
+    const double od = E.majorY ? E.dx : E.dy, oc0 = E.majorY ? E.x0 : E.y0, oid = E.majorY ? E.idx : E.idy;
+    // start and end in (major, other) coordinates
+    double ms, os, me, oe, ts, te;
+    if (k == 0) { ts = E.ta; ms = (ts == 0.0) ? c0 : fma(ts, d, c0); os = (ts == 0.0) ? oc0 : fma(ts, od, oc0); }
+    else { ms = E.g0 + E.sg * (double)(k - 1); ts = fmin(fmax((ms - c0) * id, E.ta), E.tb); os = fma(ts, od, oc0); }
+    if (k == E.n - 1) {
+        te = E.tb;
+        const bool vtx = (te == 1.0);
+        me = vtx ? (E.majorY ? E.y1 : E.x1) : fma(te, d, c0);
+        oe = vtx ? (E.majorY ? E.x1 : E.y1) : fma(te, od, oc0);
+    } else { me = E.g0 + E.sg * (double)k; te = fmin(fmax((me - c0) * id, E.ta), E.tb); oe = fma(te, od, oc0); }
+    // at most one grid line of the other axis lies strictly between os and oe
+    const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
+    const bool cross = (od != 0.0) && ((oe > os) ? (gl < oe) : (gl > oe)) && (oe != os);
+    if (cross) {
+        const double tg = fmin(fmax((gl - oc0) * oid, ts), te);
+        const double mg = fma(tg, d, c0);
+        if (E.majorY) { piece_deposit(S, os, ms, gl, mg, cs, bx, by); piece_deposit(S, gl, mg, oe, me, cs, bx, by); }
+        else { piece_deposit(S, ms, os, mg, gl, cs, bx, by); piece_deposit(S, mg, gl, me, oe, cs, bx, by); }
+    } else {
+        if (E.majorY) piece_deposit(S, os, ms, oe, me, cs, bx, by);
+        else piece_deposit(S, ms, os, me, oe, cs, bx, by);
+    }
 }
 
 struct TriSetup {
@@ -294,20 +293,20 @@ __device__ __forceinline__ double tri_pixel_area(const double (&x)[3], const dou
     return s;
 }
 
-// Apportions n <= 32 pending general triangles of the warp's ring.  Lane = triangle for the set-up; then the
-// pixels of all the (clipped) bounding boxes of the batch are spread evenly over the lanes, each clipped
-// exactly against its triangle.  Triangles whose box holds more than S.small_px pixels go to the global queue
-// (edge walk in drain_kernel: cost ~ perimeter).  Out of line.  Returns the pixels this lane clipped.
-static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w32, int ax, int ay, WarpShared *Wsp, int head, int n) {
-    const ShootDev &S = *Sp;
-    WarpShared &Ws = *Wsp;
+// Apportions n <= 32 general triangles, entry i at ent + ((head + i) & mask) * QENT.  Lane = triangle for the
+// set-up; then the pixels of all the (clipped) bounding boxes of the batch are spread evenly over the lanes,
+// each clipped exactly against its triangle.  With WALK_BIG, triangles whose box holds more than S.small_px
+// pixels are left out and reported in the returned lane mask (the caller walks their edges: cost ~ perimeter).
+// `done` counts the pixels this lane clipped.
+template <bool WALK_BIG>
+__device__ __forceinline__ unsigned apportion_batch(const ShootDev &S, const Win &W, double (*rec)[10], const double *ent, int head, int mask,
+                                                    int n, int &done) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
-    __syncwarp();
-    int npx = 0, done = 0;
+    int npx = 0;
+    bool big = false;
     if (lane < n) {
-        const double *v = Ws.ringE[(head + lane) & 63];
+        const double *v = ent + (size_t)((head + lane) & mask) * QENT;
         const double u0 = v[0], v0 = v[1], u1 = v[2], v1 = v[3], u2 = v[4], v2 = v[5];
         const double mnx = fmin(u0, fmin(u1, u2)), mxx = fmax(u0, fmax(u1, u2));
         const double mny = fmin(v0, fmin(v1, v2)), mxy = fmax(v0, fmax(v1, v2));
@@ -324,20 +323,10 @@ static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w
                 const int loy = max((int)fby, 0), hiy = min((int)floor(mxy), S.npix2 - 1);
                 const long long wc = (long long)hix - lox + 1, hc = (long long)hiy - loy + 1;
                 if (wc > 0 && hc > 0) {
-                    bool big = false;
-                    if (wc * hc > (long long)S.small_px) {
-                        unsigned long long slot = atomicAdd(&S.counters[C_QUEUE], 1ull);
-                        if ((long long)slot < S.queue_cap) {
-                            double *qd = S.queue + (size_t)slot * QENT;
-#pragma unroll
-                            for (int k = 0; k < QENT; ++k) qd[k] = v[k];
-                            atomicAdd(&S.counters[C_QUEUED], 1ull);
-                            big = true;
-                        } else atomicAdd(&S.counters[C_OVERFLOW], 1ull);   // queue full: clipped here, pixel by pixel
-                    }
+                    big = WALK_BIG && (wc * hc > (long long)S.small_px);
                     if (!big) {
                         npx = (int)((wc * hc < (1ll << 26)) ? wc * hc : (1ll << 26));   // (only a full queue can bring such boxes here)
-                        double *rc = Ws.rec[lane];
+                        double *rc = rec[lane];
                         rc[0] = 2.0 / A2;
                         rc[1] = __hiloint2double(loy, lox);
                         rc[2] = __hiloint2double((int)fby, (int)fbx);
@@ -358,6 +347,7 @@ static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(full, inc, o); if (lane >= o) inc += t; }
     const int total = __shfl_sync(full, inc, 31);
+    const unsigned bigmask = __ballot_sync(full, big);
     __syncwarp();
 #pragma unroll 1
     for (int k0 = 0; k0 < total; k0 += 32) {
@@ -372,8 +362,8 @@ static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w
         const int incl = __shfl_sync(full, inc, i), cnt = __shfl_sync(full, npx, i);
         if (k < total) {
             const int m = k - (incl - cnt);
-            const double *v = Ws.ringE[(head + i) & 63];
-            const double *rc = Ws.rec[i];
+            const double *v = ent + (size_t)((head + i) & mask) * QENT;
+            const double *rc = rec[i];
             const int lox = __double2loint(rc[1]), loy = __double2hiint(rc[1]);
             const int bx = __double2loint(rc[2]), by = __double2hiint(rc[2]);
             const int wc = __double2loint(rc[3]);
@@ -387,6 +377,51 @@ static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w
         }
     }
     __syncwarp();
+    return bigmask;
+}
+
+// Warp-cooperative edge walk of one large triangle (v = its 3 vertices in pixel units, same in all lanes).
+__device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT]) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
+    TriSetup T;
+    T.status = 0;
+    if (lane == 0) tri_setup(S, W, v, T);                      // the degenerate case deposits: one lane only
+    const int status = __shfl_sync(full, T.status, 0);
+    if (status != 1) return 0ull;
+    const double cs = __shfl_sync(full, T.cs, 0);
+    const int bx = __shfl_sync(full, T.bx, 0), by = __shfl_sync(full, T.by, 0);
+    const double fbx = (double)bx, fby = (double)by;
+    const double hgt = fmax(v[1], fmax(v[3], v[5])) - fby + 1.0;
+    const double ry0 = fmax(0.0, -fby), ry1 = fmin(hgt, (double)S.npix2 - fby), cx1 = (double)S.npix1 - fbx;
+    unsigned long long n_pieces = 0;
+#pragma unroll 1
+    for (int ed = 0; ed < 3; ++ed) {
+        const int ia = 2 * ed, ib = (ed == 2) ? 0 : 2 * ed + 2;
+        EdgeWalk E;
+        edge_setup(E, v[ia] - fbx, v[ia + 1] - fby, v[ib] - fbx, v[ib + 1] - fby, ry0, ry1, cx1);
+        for (int k = lane; k < E.n; k += 32) edge_step(S, E, k, cs, bx, by);
+        n_pieces += (unsigned long long)E.n;
+    }
+    return n_pieces;
+}
+
+// The shooting kernel's own copy, for the triangles it could not hand to the global queue (queue full).
+// Out of line, cold.
+static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w32, int ax, int ay, WarpShared *Wsp, int head, int n) {
+    Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
+    int done = 0;
+    __syncwarp();
+    unsigned big = apportion_batch<true>(*Sp, W, Wsp->rec, &Wsp->ringE[0][0], head, 63, n, done);
+    while (big) {
+        const int i = __ffs(big) - 1;
+        big &= big - 1;
+        double v[QENT];
+#pragma unroll
+        for (int k = 0; k < QENT; ++k) v[k] = Wsp->ringE[(head + i) & 63][k];
+        walk_triangle(*Sp, v);
+    }
     return done;
 }
 

@@ -34,7 +34,11 @@ __device__ __forceinline__ long long fetch_tile(const ShootDev &S) {
     return __shfl_sync(0xffffffffu, t, 0);
 }
 
-struct Pend { Ring E, S2; };
+struct Pend {
+    Ring E, S2;                        // E: only what the global queue could not take
+    long long chunk = -1;              // queue chunk this warp is filling
+    int used = 0;
+};
 
 // Runs the pending-work rings down to fewer than `keep` entries (keep = 32 inside a tile, 1 at the end).
 __device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, WarpShared &Ws, Pend &P, int keep, ThreadCounters &tc) {
@@ -51,6 +55,39 @@ __device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, War
         if (lane < n) ++tc.small_;
         P.E.head = (P.E.head + n) & 63; P.E.count -= n;
     }
+}
+
+// General triangles go to the global queue, which drain_kernel apportions at full occupancy.  A warp reserves
+// QCHUNK entries at a time (one atomic per chunk); if the queue is full they stay in the warp's own ring and
+// are clipped by the (cold) in-kernel copy.
+__device__ __forceinline__ void queue_push(const ShootDev &S, WarpShared &Ws, Pend &P, bool pred, const double (&e)[6], ThreadCounters &tc) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const unsigned m = __ballot_sync(full, pred);
+    if (!m) return;
+    const int n = __popc(m);
+    if (P.chunk < 0 || P.used + n > QCHUNK) {
+        long long c = 0;
+        if (lane == 0) {
+            if (P.chunk >= 0) S.qcount[P.chunk] = P.used;
+            c = (long long)atomicAdd(&S.counters[C_QUEUE], 1ull);
+        }
+        c = __shfl_sync(full, c, 0);
+        P.chunk = (c < S.queue_cap) ? c : -1;
+        P.used = 0;
+    }
+    if (P.chunk < 0) {                                          // queue full
+        if (pred) ++tc.overflow;
+        ring_push<6>(P.E, Ws.ringE, pred, e);
+        return;
+    }
+    if (pred) {
+        double *q = S.queue + ((size_t)P.chunk * QCHUNK + (size_t)(P.used + __popc(m & ((1u << lane) - 1u)))) * QENT;
+#pragma unroll
+        for (int k = 0; k < QENT; ++k) q[k] = e[k];
+        ++tc.queued;
+    }
+    P.used += n;
 }
 
 // The cell row between corner rows `prev` and `cur` of the staged group: lane = cell column.
@@ -97,7 +134,7 @@ __device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSh
             e[2] = Ws.stu[r2][c2]; e[3] = Ws.stv[r2][c2];
             e[4] = Ws.stu[r3][c3]; e[5] = Ws.stv[r3][c3];
         }
-        ring_push<6>(P.E, Ws.ringE, act && !strip, e);
+        queue_push(S, Ws, P, act && !strip, e, tc);
         {
             const bool ay = (h == 1);                                        // pixels stacked in y
             const double line = ay ? (double)(mny + 1) : (double)(mnx + 1);
@@ -185,45 +222,78 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32) shoot_ipm_kernel(const __gri
     // pending work of the last tiles goes straight to the map
     W.w32 = nullptr;
     run_batches(S, W, Ws, P, 1, tc);
+    if (lane == 0 && P.chunk >= 0) S.qcount[P.chunk] = P.used;
     flush_counters(S, tc);
 }
 
-// Giant triangles (the faint images of the whole map that every star in the window produces): one warp per
-// queued triangle, edge by edge, the lanes striding over the edge's pieces.  Work ~ perimeter in pixels.
-__global__ void __launch_bounds__(256) drain_kernel(const __grid_constant__ ShootDev S) {
+// Apportions the queued general triangles at full occupancy: a warp takes a chunk, 32 entries at a time.
+// Small boxes are clipped pixel by pixel, the pixels of the 32 triangles spread evenly over the lanes; the
+// large ones (among them the faint images of the whole map that every star in the window produces) are
+// walked edge by edge by the whole warp, cost ~ perimeter.
+static const int DRAIN_WARPS = 8;
+__global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_constant__ ShootDev S) {
+    __shared__ double rec_s[DRAIN_WARPS][32][10];
+    double (*rec)[10] = rec_s[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     long long nq = (long long)S.counters[C_QUEUE];
     if (nq > S.queue_cap) nq = S.queue_cap;
     Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
     unsigned long long n_pieces = 0;
+    int n_clipped = 0;
     while (true) {
-        long long q = 0;
-        if (lane == 0) q = (long long)atomicAdd(&S.counters[C_DRAIN], 1ull);
-        q = __shfl_sync(full, q, 0);
-        if (q >= nq) break;
-        const double *e = S.queue + (size_t)q * QENT;
+        long long c = 0;
+        if (lane == 0) c = (long long)atomicAdd(&S.counters[C_DRAIN], 1ull);
+        c = __shfl_sync(full, c, 0);
+        if (c >= nq) break;
+        const int cnt = S.qcount[c];
+        const double *base = S.queue + (size_t)c * QCHUNK * QENT;
+#pragma unroll 1
+        for (int b0 = 0; b0 < cnt; b0 += 32) {
+            unsigned big = apportion_batch<true>(S, W, rec, base, b0, 0x7fffffff, min(32, cnt - b0), n_clipped);
+            if (big) {
+                // large triangles are handed on one by one (walk_kernel): a chunk from a star's tile is full of them
+                const int nb = __popc(big);
+                unsigned long long at = 0;
+                if (lane == 0) at = atomicAdd(&S.counters[C_BIG], (unsigned long long)nb);
+                at = __shfl_sync(full, at, 0);
+                if ((long long)(at + nb) <= S.big_cap) {
+                    if (big & (1u << lane)) S.biglist[at + __popc(big & ((1u << lane) - 1u))] = (unsigned int)(c * QCHUNK + b0 + lane);
+                    big = 0;
+                }
+            }
+            while (big) {                                       // list full: walked here
+                const int i = __ffs(big) - 1;
+                big &= big - 1;
+                double v[QENT];
+#pragma unroll
+                for (int k = 0; k < QENT; ++k) v[k] = base[(size_t)(b0 + i) * QENT + k];
+                n_pieces += walk_triangle(S, v);
+            }
+        }
+    }
+    if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
+    for (int o = 16; o; o >>= 1) n_clipped += __shfl_xor_sync(full, n_clipped, o);
+    if (lane == 0 && n_clipped) atomicAdd(&S.counters[C_PX_INT], (unsigned long long)n_clipped);
+}
+
+// Edge walk of the large triangles the drain set aside: one warp per triangle, handed out one at a time.
+__global__ void __launch_bounds__(256) walk_kernel(const __grid_constant__ ShootDev S) {
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    long long nb = (long long)S.counters[C_BIG];
+    if (nb > S.big_cap) nb = S.big_cap;
+    unsigned long long n_pieces = 0;
+    while (true) {
+        long long i = 0;
+        if (lane == 0) i = (long long)atomicAdd(&S.counters[C_WALK], 1ull);
+        i = __shfl_sync(full, i, 0);
+        if (i >= nb) break;
+        const double *e = S.queue + (size_t)S.biglist[i] * QENT;
         double v[QENT];
 #pragma unroll
         for (int k = 0; k < QENT; ++k) v[k] = __ldg(&e[k]);
-        TriSetup T;
-        T.status = 0;
-        if (lane == 0) tri_setup(S, W, v, T);                  // the degenerate case deposits: one lane only
-        const int status = __shfl_sync(full, T.status, 0);
-        if (status != 1) continue;
-        const double cs = __shfl_sync(full, T.cs, 0);
-        const int bx = __shfl_sync(full, T.bx, 0), by = __shfl_sync(full, T.by, 0);
-        const double fbx = (double)bx, fby = (double)by;
-        const double hgt = fmax(v[1], fmax(v[3], v[5])) - fby + 1.0;
-        const double ry0 = fmax(0.0, -fby), ry1 = fmin(hgt, (double)S.npix2 - fby), cx1 = (double)S.npix1 - fbx;
-#pragma unroll 1
-        for (int ed = 0; ed < 3; ++ed) {
-            const int ia = 2 * ed, ib = (ed == 2) ? 0 : 2 * ed + 2;
-            EdgeWalk E;
-            edge_setup(E, v[ia] - fbx, v[ia + 1] - fby, v[ib] - fbx, v[ib + 1] - fby, ry0, ry1, cx1);
-            for (int k = lane; k < E.n; k += 32) edge_piece(S, E, k, cs, bx, by);
-            n_pieces += (unsigned long long)E.n;
-        }
+        n_pieces += walk_triangle(S, v);
     }
     if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
 }
@@ -409,9 +479,11 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if (ipm) {
         ML_TRY(f->diff.reserve((size_t)npix, s, false));
         ML_CUDA(cudaMemsetAsync(f->diff.p, 0, (size_t)npix * 8, s));
-        long long qmb = env_ll("MLENS_QUEUE_MB", 512);
-        qcap = qmb * (1ll << 20) / (QENT * 8);
-        ML_TRY(f->queue.reserve((size_t)qcap * QENT, s, false));
+        long long qmb = env_ll("MLENS_QUEUE_MB", 1024);
+        qcap = qmb * (1ll << 20) / (QCHUNK * QENT * 8);              // chunks
+        ML_TRY(f->queue.reserve((size_t)qcap * QCHUNK * QENT, s, false));
+        ML_TRY(f->qcount.reserve((size_t)qcap, s, false));
+        ML_TRY(f->biglist.reserve((size_t)qcap * QCHUNK / 4, s, false));
     }
     ShootDev S;
     S.L = make_lens_dev(f);
@@ -419,7 +491,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     S.i0 = i0; S.i1 = i1; S.j0 = j0; S.j1 = j1;
     S.ylo1 = g->ylo1; S.ylo2 = g->ylo2; S.p1 = g->p1; S.p2 = g->p2; S.inv_p1 = 1.0 / g->p1; S.inv_p2 = 1.0 / g->p2;
     S.npix1 = d->npix1; S.npix2 = d->npix2;
-    S.acc = f->acc.p; S.diff = f->diff.p; S.queue = f->queue.p; S.counters = f->counters.p; S.queue_cap = qcap;
+    S.acc = f->acc.p; S.diff = f->diff.p; S.queue = f->queue.p; S.qcount = f->qcount.p; S.biglist = f->biglist.p; S.big_cap = qcap * QCHUNK / 4; S.counters = f->counters.p; S.queue_cap = qcap;
     S.dump1 = d->dump_w1; S.dump2 = d->dump_w2;
     S.binom = f->binom.p;
     if ((S.dump1 == nullptr) != (S.dump2 == nullptr)) { set_error("dump_w1 and dump_w2 go together"); return MLENS_EINVAL; }
@@ -427,7 +499,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     S.tq = (int)env_ll("MLENS_TILE_ORDER", 12);
     if (S.tq > TQMAX) S.tq = TQMAX;
     if (S.tq < 2) S.tq = 2;
-    S.small_px = (int)env_ll("MLENS_SMALL_PX", 32);
+    S.small_px = (int)env_ll("MLENS_SMALL_PX", 64);
     S.dbg = (int)env_ll("MLENS_DBG", 0);
     // truncation budget of the tile series: 5 % of the deflection accuracy the field was built for
     S.eps_far = 0.02 * f->eps * f->theta;
@@ -439,7 +511,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 27);
+    long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 26);
     long long rows_per_band = band_cells / (ntx * stepx * stepy);
     if (rows_per_band < 1) rows_per_band = 1;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -472,14 +544,15 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         const long long want = (nt + SHOOT_WARPS - 1) / SHOOT_WARPS;
         int grid = (int)((want < resident) ? want : resident);
         ML_CUDA(cudaMemsetAsync(f->counters.p, 0, 16, s));         // queue fill count and tile counter
-        ML_CUDA(cudaMemsetAsync(f->counters.p + C_DRAIN, 0, 8, s));
+        ML_CUDA(cudaMemsetAsync(f->counters.p + C_DRAIN, 0, 3 * 8, s));   // drain, big-list and walk counters
         ML_TRY(mark());
         if (ipm) {
             ML_LAUNCH(shoot_ipm_kernel, grid, SHOOT_WARPS * 32, smem, s, S);
             ML_TRY(mark());
-            ML_LAUNCH(drain_kernel, nsm * 8, 256, 0, s, S);
+            ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
+            ML_LAUNCH(walk_kernel, nsm * 8, 256, 0, s, S);
             ML_TRY(mark());
-            launches += 2;
+            launches += 3;
         } else {
             ML_LAUNCH(shoot_irs_kernel, grid, SHOOT_WARPS * 32, smem, s, S);
             ML_TRY(mark());
@@ -506,7 +579,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         st->n_tri_queued = (int64_t)h[C_QUEUED]; st->n_queue_chunks = (int64_t)h[C_QUEUED];
         st->n_queue_overflow = (int64_t)h[C_OVERFLOW]; st->n_rays_fallback = (int64_t)h[C_FALLBACK];
         st->n_near_terms = (int64_t)h[C_NEAR];
-        st->n_px_small = (int64_t)h[C_PX_SMALL]; st->n_px_interior = 0;
+        st->n_px_small = (int64_t)h[C_PX_SMALL]; st->n_px_interior = (int64_t)h[C_PX_INT];
         st->n_px_edge = (int64_t)h[C_PX_EDGE]; st->n_rows = 0;
         st->n_tiles_full = (int64_t)h[C_TILES_FULL];
         st->tile_order = S.tq;

@@ -32,9 +32,12 @@ struct ShootDev {
     int npix1, npix2;
     unsigned long long *acc;           // fixed-point pixel sums (IPM) or ray counts (IRS)
     unsigned long long *diff;          // IPM: row-difference array written by the edge walk of large triangles
-    double *queue;                     // giant-triangle queue, QENT doubles per entry
+    double *queue;                     // general-triangle queue: chunks of QCHUNK entries of QENT doubles
+    int *qcount;                       // entries in each chunk
+    unsigned int *biglist;             // queue entries whose triangles are walked edge by edge (walk_kernel)
+    long long big_cap;
     unsigned long long *counters;
-    long long queue_cap;
+    long long queue_cap;               // chunks
     double *dump1, *dump2;
     const double *binom;               // Pascal triangle, stride BN
     int eval_mode;
