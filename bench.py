@@ -15,8 +15,10 @@ HBM (the star field is generated on the device from the seed).  `e2e` repeats th
 buffers: stars handed over as pinned host arrays, maps returned into pinned host arrays, the library
 doing the copies inside the timed region.
 
-N > 1 (torchrun): every rank makes an independent map of the same configuration with its own seed
-(the path shards over realisations: no data-path collective; scaling "weak"); time = max over ranks.
+N > 1 (torchrun): the SAME map on N GPUs: stars and tree replicated, the cell grid cut
+into star-weighted row slabs (paper_2506_02114_b200/multi.py), one all-reduce (sum, float64) of each
+map over NCCL -- the path's only exchange step; total work is fixed, so scaling is "strong";
+time = max over ranks.
 
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
 workload, on the host cores of this box.  It is a deliberately slow baseline, not the target.
@@ -159,7 +161,7 @@ def run_reference(args):
     sample = f"IPM + IRS on the {patch[0]}x{patch[1]}-cell patch {sub} at the window centre, all {cfg.n_stars} stars per ray"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg), "sample": sample},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle", "sample": sample},
@@ -173,6 +175,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     import paper_2506_02114_b200 as ml
+    from paper_2506_02114_b200 import multi
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: libmlens has no CPU fallback")
@@ -185,7 +188,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     cfg = synth.get_config(args.config)
-    seed = cfg.seed + 7919 * rank                    # one realisation per rank
+    seed = cfg.seed                                  # N > 1: the same field on every rank, one slab of rays each
     kw = dict(border_mode=cfg.border_mode, border_param=cfg.border_param)
     half, npix, k = cfg.half_y, cfg.npix, cfg.rays_per_pixel_length
     stream = torch.cuda.current_stream()
@@ -198,9 +201,24 @@ def run_ours(args):
     def step_device():
         f = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, seed, kappa_star=cfg.kappa_star,
                             mass_law=cfg.mass_law, mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
-        r1 = f.shoot(half, npix, k, out=map_ipm, map_mode=ml.MAP_IPM, **kw)
-        r2 = f.shoot(half, npix, k, out=map_irs, map_mode=ml.MAP_IRS, **kw)
-        state.update(info=f.info(), ipm=r1, irs=r2)
+        if world > 1 and "weights" not in state:     # slab cost model from the star rows (same on every rank; cached)
+            g0 = f.grid(half, npix, k, **kw)
+            state["weights"] = multi.star_row_weights(f.stars()[1], g0.x0_2, g0.h2, int(g0.n2))
+        _, slab, s1 = multi.shoot_distributed(f, half, npix, k, weights=state.get("weights"), out=map_ipm,
+                                              map_mode=ml.MAP_IPM, **kw)
+        _, _, s2 = multi.shoot_distributed(f, half, npix, k, weights=state.get("weights"), out=map_irs,
+                                           map_mode=ml.MAP_IRS, **kw)
+        state.update(info=f.info(), ipm=s1, irs=s2, slab=slab, grid=f.grid(half, npix, k, **kw))
+        if "near_mean" not in state:                 # mean near-field list of a ray's leaf (area-weighted over the window)
+            t = f.tree()
+            g_ = state["grid"]
+            leaves = np.where(t["child0"] < 0)[0]
+            half_l = t["root_half"] / 2.0 ** t["level"][leaves]
+            cx = -t["root_half"] + (2 * t["ix"][leaves] + 1) * half_l
+            cy = -t["root_half"] + (2 * t["iy"][leaves] + 1) * half_l
+            inside = (np.abs(cx - g_.X1) < g_.H1) & (np.abs(cy - g_.X2) < g_.H2)
+            wgt = (half_l ** 2) * inside
+            state["near_mean"] = float(np.sum(wgt * t["near_cnt"][t["leaf_id"][leaves]]) / max(np.sum(wgt), 1e-300))
         f.close()
 
     # host-side buffers of the e2e leg: pinned, numpy views handed to the C ABI as HOST pointers
@@ -212,8 +230,14 @@ def run_ours(args):
     def step_host():
         f = ml.Field.from_stars(cfg.kappa_tot, cfg.gamma, hx.numpy(), hy.numpy(), hm.numpy(),
                                 kappa_star=cfg.kappa_star, R=R)
-        f.shoot(half, npix, k, out=h_ipm.numpy(), map_mode=ml.MAP_IPM, **kw)
-        f.shoot(half, npix, k, out=h_irs.numpy(), map_mode=ml.MAP_IRS, **kw)
+        if world == 1:
+            f.shoot(half, npix, k, out=h_ipm.numpy(), map_mode=ml.MAP_IPM, **kw)
+            f.shoot(half, npix, k, out=h_irs.numpy(), map_mode=ml.MAP_IRS, **kw)
+        else:                                        # slabs on the device, all-reduce, then the result back to the host
+            multi.shoot_distributed(f, half, npix, k, weights=state.get("weights"), out=map_ipm, map_mode=ml.MAP_IPM, **kw)
+            multi.shoot_distributed(f, half, npix, k, weights=state.get("weights"), out=map_irs, map_mode=ml.MAP_IRS, **kw)
+            h_ipm.copy_(map_ipm, non_blocking=True); h_irs.copy_(map_irs, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
         f.close()
         return float(h_ipm[npix // 2, npix // 2])
 
@@ -251,11 +275,11 @@ def run_ours(args):
     launches = (ml.launch_count() - l0) // args.steps
     clocks = sampler.stop() if rank == 0 else None
 
-    g = state["ipm"].grid
-    evals_ipm = (g.n1 + 1) * (g.n2 + 1)
+    g = state["grid"]
+    evals_ipm = (g.n1 + 1) * (g.n2 + 1)              # unique rays of the whole map, whatever N
     evals_irs = g.n1 * g.n2
     evals = evals_ipm + evals_irs
-    value = world * evals / sec
+    value = evals / sec
 
     e2e = None
     if not args.no_e2e:
@@ -267,14 +291,20 @@ def run_ours(args):
         hx.numpy()[:], hy.numpy()[:], hm.numpy()[:] = sx, sy, sm
         step_host()
         sec_h = timed(step_host, args.steps)
-        e2e = {"value": world * evals / sec_h, "unit": UNIT, "ms_per_step": sec_h * 1e3,
+        e2e = {"value": evals / sec_h, "unit": UNIT, "ms_per_step": sec_h * 1e3,
                "h2d_bytes_per_step": 3 * 8 * cfg.n_stars, "d2h_bytes_per_step": 2 * 8 * npix * npix}
 
     # ---- roofline of the dominant kernel (fused evaluate + IPM deposit), DESIGN.md s7
-    st = state["ipm"].stats
+    # Algorithmic work per lens-equation evaluation: the leaf's near-field list summed directly
+    # (10 flop per star) + the leaf's order-p Taylor series by Horner (8 flop per term) + 10 flop macro and sheet.
+    # The kernel itself does less (it re-expands the series per 32x32-ray tile, order 12, and folds the distant
+    # near-field stars into it): `flop_executed` counts what it really issues for the evaluation.
+    st = state["ipm"]
     p = state["info"]["order"]
+    n_near_leaf = state["near_mean"]
     rays_k = st["n_rays"]                                        # evaluations the kernel performed
-    flop = 10.0 * st["n_near_terms"] + (8.0 * p + 10.0) * rays_k   # 10/near star, 8/Horner term, 10 macro+sheet
+    flop_alg = rays_k * (10.0 * n_near_leaf + 8.0 * (p - 1) + 10.0)
+    flop_exec = 10.0 * st["n_near_terms"] + (8.0 * st["tile_order"] + 10.0) * rays_k
     n_l = max(1, st["n_shoot_launches"])
     dur = st["ms_shoot"] * 1e-3 / n_l
     peaks = {}
@@ -285,13 +315,16 @@ def run_ours(args):
     sm_max = peaks.get("sm_max_mhz", 1965.0)
     nsm = torch.cuda.get_device_properties(dev).multi_processor_count
     peak_tf = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-    achieved_tf = flop / n_l / dur / 1e12 if dur > 0 else 0.0
+    achieved_tf = flop_alg / n_l / dur / 1e12 if dur > 0 else 0.0
     roofline = {"bound": "alu", "kernel": "shoot_ipm_kernel", "achieved": achieved_tf, "peak": peak_tf,
                 "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
                 "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
                 "peak_source": f"{nsm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz (derived, DESIGN.md s7)",
                 "peak_measured_dfma": ml.bench_dfma() / 1e12,
-                "flop_per_launch": flop / n_l, "launch_ms": dur * 1e3, "launches_per_map": n_l,
+                "flop_per_eval_algorithmic": flop_alg / rays_k, "near_stars_per_leaf_mean": n_near_leaf,
+                "flop_per_launch": flop_alg / n_l, "flop_executed_per_launch": flop_exec / n_l,
+                "achieved_executed": flop_exec / n_l / dur / 1e12 if dur > 0 else 0.0,
+                "launch_ms": dur * 1e3, "launches_per_map": n_l,
                 "share_of_step": st["ms_shoot"] * 1e-3 / sec}
 
     cpu = None
@@ -302,22 +335,23 @@ def run_ours(args):
                          f"({e} evaluations, each a direct sum over all {cfg.n_stars} stars)"}
 
     if rank == 0:
-        irs = state["irs"].stats
+        irs = state["irs"]
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "warmup": max(args.warmup, 3), "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "rays_ipm": evals_ipm, "rays_irs": evals_irs,
                        "stars_seed": seed, "order_p": p, "border": "eq16",
                        "l2": "flushed between steps (512 MiB fill outside the per-step events)",
-                       "parallelism": f"{world} independent realisations" if world > 1 else "1 GPU"},
-            "phases_ms": {"ipm_map": st["ms_total"], "ipm_shoot_kernels": st["ms_shoot"], "ipm_drain_kernels": st["ms_drain"],
+                       "parallelism": (f"{world} GPUs: star-weighted row slabs of one map + all-reduce of the map "
+                                       f"(rank 0 rows {state['slab']})") if world > 1 else "1 GPU"},
+            "phases_ms": {"ipm_map": st["ms_total"], "ipm_shoot_kernels": st["ms_shoot"], "ipm_drain_and_walk_kernels": st["ms_drain"],
                           "irs_map": irs["ms_total"], "irs_shoot_kernels": irs["ms_shoot"],
                           "create_and_rest": sec * 1e3 - st["ms_total"] - irs["ms_total"]},
             "ipm_map_wall_ms": st["ms_total"],
             "evals_per_s_ipm_kernel": rays_k / (st["ms_shoot"] * 1e-3) if st["ms_shoot"] > 0 else None,
-            "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_small", "n_tri_queued", "n_queue_chunks",
-                                                  "n_queue_overflow", "n_rays_fallback")},
+            "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
+                                                  "n_queue_overflow", "n_px_clipped", "n_edge_steps", "n_rays_fallback")},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
             "roofline": roofline, "cpu_baseline": cpu,
         }))

@@ -136,23 +136,23 @@ typedef struct {
     int64_t n_rays;                /* lens-equation evaluations performed (incl. tile-border duplicates) */
     int64_t n_cells;
     int64_t n_tri_single;          /* triangles wholly inside one pixel */
-    int64_t n_tri_small;           /* triangles apportioned by the thread that mapped them */
-    int64_t n_tri_queued;          /* large triangles sent through the cooperative queue */
-    int64_t n_queue_chunks;        /* row chunks those were split into */
-    int64_t n_queue_overflow;      /* large triangles processed inline because the queue was full */
-    int64_t n_rays_fallback;       /* rays evaluated outside the tile's cached leaves */
+    int64_t n_tri_strip;           /* triangles over two adjacent pixels (closed-form split in the shooting kernel) */
+    int64_t n_tri_queued;          /* general triangles handed to the apportioning kernels through the global queue */
+    int64_t n_tri_walked;          /* ... of which walked edge by edge (large boxes), the rest clipped pixel by pixel */
+    int64_t n_queue_overflow;      /* general triangles apportioned by the shooting kernel itself: queue full */
+    int64_t n_rays_fallback;       /* rays evaluated through the tree instead of the tile's series */
     int32_t n_bands;               /* row bands the sub-range was processed in */
     int32_t gpu_launches;          /* kernels launched by this call */
     float ms_total;                /* device time of the call (CUDA events), only when sync = 1 */
     float ms_shoot;                /* summed device time of the fused evaluate+deposit launches (IPM or IRS) */
-    float ms_drain;                /* summed device time of the large-triangle drain launches (IPM) */
+    float ms_drain;                /* summed device time of the apportioning launches (drain + walk kernels, IPM) */
     float ms_finalise;             /* device time of the fixed-point -> double conversion */
     int32_t n_shoot_launches;      /* launches behind ms_shoot */
-    int64_t n_near_terms;          /* near-field star terms summed over all rays (eq 23 direct part) */
-    int64_t n_px_small;            /* (triangle, pixel) pairs clipped by the mapping thread itself */
-    int64_t n_px_interior;         /* ... covered by queued triangles as interior pixels (constant deposit) */
-    int64_t n_px_edge;             /* ... clipped exactly by the cooperative drain */
-    int64_t n_rows;                /* pixel rows of queued triangles */
+    int64_t n_near_terms;          /* near-field star terms summed directly over all rays (eq 23 direct part) */
+    int64_t n_px_strip;            /* pixel deposits of the strips */
+    int64_t n_px_clipped;          /* (triangle, pixel) pairs clipped exactly by the drain kernel */
+    int64_t n_edge_steps;          /* major-axis steps of the edge walk */
+    int64_t reserved_;
     int64_t n_tiles_full;          /* tile slots whose truncation bound failed (evaluated with the leaf's full series) */
     int32_t tile_order;            /* order of the per-tile series */
     int32_t pad_;

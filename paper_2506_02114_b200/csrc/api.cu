@@ -15,6 +15,19 @@ void set_error(const char *fmt, ...) {
     va_end(ap);
 }
 
+int pool_init() {
+    static std::atomic<int> done{0};
+    if (done.load()) return MLENS_OK;
+    int dev = 0;
+    ML_CUDA(cudaGetDevice(&dev));
+    cudaMemPool_t pool;
+    ML_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
+    unsigned long long keep = ~0ull;
+    ML_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+    done.store(1);
+    return MLENS_OK;
+}
+
 static int check_device() {
     int n = 0;
     cudaError_t e = cudaGetDeviceCount(&n);
@@ -29,12 +42,15 @@ static int check_device() {
 // staging of caller arrays: device pointers pass through, host pointers are copied
 struct Stage {
     std::vector<void *> owned;
-    ~Stage() { for (void *p : owned) cudaFree(p); }
+    cudaStream_t s_;
+    explicit Stage(cudaStream_t s) : s_(s) {}
+    ~Stage() { for (void *p : owned) cudaFreeAsync(p, s_); }       // stream-ordered: after the copies back
     template <typename T>
     int in(const T *src, size_t n, int kind, cudaStream_t s, const T **out) {
         if (kind == MLENS_PTR_DEVICE || n == 0) { *out = src; return MLENS_OK; }
         T *d = nullptr;
-        ML_CUDA(cudaMalloc(&d, n * sizeof(T)));
+        ML_TRY(pool_init());
+        ML_CUDA(cudaMallocAsync(&d, n * sizeof(T), s));
         owned.push_back(d);
         ML_CUDA(cudaMemcpyAsync(d, src, n * sizeof(T), cudaMemcpyHostToDevice, s));
         *out = d;
@@ -44,7 +60,8 @@ struct Stage {
     int out(T *dst, size_t n, int kind, T **dev) {
         if (kind == MLENS_PTR_DEVICE || n == 0 || dst == nullptr) { *dev = dst; return MLENS_OK; }
         T *d = nullptr;
-        ML_CUDA(cudaMalloc(&d, n * sizeof(T)));
+        ML_TRY(pool_init());
+        ML_CUDA(cudaMallocAsync(&d, n * sizeof(T), s_));
         owned.push_back(d);
         *dev = d;
         return MLENS_OK;
@@ -281,7 +298,7 @@ static int points_call(const mlens_field *f, int64_t n, const double *zx, const 
     if (!f || n < 0 || (n > 0 && (!zx || !zy || !ox || !oy))) { set_error("bad arguments"); return MLENS_EINVAL; }
     if (eval_mode != MLENS_EVAL_FMM && eval_mode != MLENS_EVAL_DIRECT) { set_error("bad eval mode"); return MLENS_EINVAL; }
     cudaStream_t s = (cudaStream_t)stream;
-    Stage st;
+    Stage st(s);
     const double *dzx, *dzy; double *dox, *doy;
     ML_TRY(st.in(zx, (size_t)n, ptr_kind, s, &dzx)); ML_TRY(st.in(zy, (size_t)n, ptr_kind, s, &dzy));
     ML_TRY(st.out(ox, (size_t)n, ptr_kind, &dox)); ML_TRY(st.out(oy, (size_t)n, ptr_kind, &doy));
@@ -313,7 +330,7 @@ int mlens_shoot(mlens_field *f, const mlens_shoot_desc *d, double *map, uint64_t
     ML_TRY(geometry(f, d, &g));
     cudaStream_t s = (cudaStream_t)stream;
     size_t npix = (size_t)d->npix1 * d->npix2;
-    Stage st;
+    Stage st(s);
     double *dmap = nullptr; unsigned long long *dcnt = nullptr;
     ML_TRY(st.out(map, npix, d->ptr_kind, &dmap));
     ML_TRY(st.out((unsigned long long *)counts, npix, d->ptr_kind, &dcnt));

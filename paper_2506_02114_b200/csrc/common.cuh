@@ -42,6 +42,10 @@ extern std::atomic<long long> g_launches;
         if (rc_ != MLENS_OK) return rc_; \
     } while (0)
 
+// Device memory comes from the stream-ordered pool of the device (cudaMallocAsync), with the pool told to keep
+// what is freed: creating and destroying fields in a loop then costs no driver allocation at all.
+int pool_init();
+
 // Growable device array that keeps its contents on reserve().
 template <typename T>
 struct DevBuf {
@@ -49,15 +53,17 @@ struct DevBuf {
     size_t cap = 0;
     int reserve(size_t n, cudaStream_t s, bool keep = true) {
         if (n <= cap) return MLENS_OK;
+        ML_TRY(pool_init());
         size_t ncap = n + n / 4 + 64;
         T *q = nullptr;
-        ML_CUDA(cudaMalloc(&q, ncap * sizeof(T)));
+        ML_CUDA(cudaMallocAsync(&q, ncap * sizeof(T), s));
         if (p && keep && cap) ML_CUDA(cudaMemcpyAsync(q, p, cap * sizeof(T), cudaMemcpyDeviceToDevice, s));
-        if (p) { ML_CUDA(cudaStreamSynchronize(s)); cudaFree(p); }
+        if (p) ML_CUDA(cudaFreeAsync(p, s));
         p = q; cap = ncap;
         return MLENS_OK;
     }
-    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+    // callers synchronise the streams that used the buffer before releasing it
+    void release() { if (p) cudaFreeAsync(p, 0); p = nullptr; cap = 0; }
 };
 
 struct Tree {

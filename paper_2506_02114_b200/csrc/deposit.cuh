@@ -25,8 +25,6 @@ static const unsigned long long FIX_ONE = 1ull << FIXBITS;
 static const int QENT = 6;                 // doubles per queue entry: the 3 vertices in pixel units
 static const int QCHUNK = 256;             // queue entries a warp reserves at a time
 
-enum { C_QUEUE = 0, C_TILE, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR,
-       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_BIG, C_WALK, C_NCOUNTERS };
 
 struct Win {                           // where a warp's deposits go (uniform registers)
     unsigned int *w32;                 // the warp's shared window viewed as 32-bit halves, or nullptr
@@ -325,19 +323,35 @@ __device__ __forceinline__ unsigned apportion_batch(const ShootDev &S, const Win
                 if (wc > 0 && hc > 0) {
                     big = WALK_BIG && (wc * hc > (long long)S.small_px);
                     if (!big) {
-                        npx = (int)((wc * hc < (1ll << 26)) ? wc * hc : (1ll << 26));   // (only a full queue can bring such boxes here)
-                        double *rc = rec[lane];
-                        rc[0] = 2.0 / A2;
-                        rc[1] = __hiloint2double(loy, lox);
-                        rc[2] = __hiloint2double((int)fby, (int)fbx);
-                        rc[3] = __hiloint2double(0, (int)wc);
                         const double dx0 = x1 - x0, dx1 = x2 - x1, dx2 = x0 - x2, dy0 = y1 - y0, dy1 = y2 - y1, dy2 = y0 - y2;
-                        rc[4] = (dx0 != 0.0) ? fast_rcp(fabs(dx0)) * (dx0 < 0.0 ? -1.0 : 1.0) : 0.0;
-                        rc[5] = (dx1 != 0.0) ? fast_rcp(fabs(dx1)) * (dx1 < 0.0 ? -1.0 : 1.0) : 0.0;
-                        rc[6] = (dx2 != 0.0) ? fast_rcp(fabs(dx2)) * (dx2 < 0.0 ? -1.0 : 1.0) : 0.0;
-                        rc[7] = (dy0 != 0.0) ? fast_rcp(fabs(dy0)) * (dy0 < 0.0 ? -1.0 : 1.0) : 0.0;
-                        rc[8] = (dy1 != 0.0) ? fast_rcp(fabs(dy1)) * (dy1 < 0.0 ? -1.0 : 1.0) : 0.0;
-                        rc[9] = (dy2 != 0.0) ? fast_rcp(fabs(dy2)) * (dy2 < 0.0 ? -1.0 : 1.0) : 0.0;
+                        const double idx[3] = {(dx0 != 0.0) ? fast_rcp(fabs(dx0)) * (dx0 < 0.0 ? -1.0 : 1.0) : 0.0,
+                                               (dx1 != 0.0) ? fast_rcp(fabs(dx1)) * (dx1 < 0.0 ? -1.0 : 1.0) : 0.0,
+                                               (dx2 != 0.0) ? fast_rcp(fabs(dx2)) * (dx2 < 0.0 ? -1.0 : 1.0) : 0.0};
+                        const double idy[3] = {(dy0 != 0.0) ? fast_rcp(fabs(dy0)) * (dy0 < 0.0 ? -1.0 : 1.0) : 0.0,
+                                               (dy1 != 0.0) ? fast_rcp(fabs(dy1)) * (dy1 < 0.0 ? -1.0 : 1.0) : 0.0,
+                                               (dy2 != 0.0) ? fast_rcp(fabs(dy2)) * (dy2 < 0.0 ? -1.0 : 1.0) : 0.0};
+                        if (wc == 2 && hc == 2 && mxx - fbx < 2.0 && mxy - fby < 2.0 && fbx >= 0.0 && fby >= 0.0) {
+                            // the commonest general triangle, four pixels around one grid corner: one clipped pixel
+                            // and the two line fractions give all four by inclusion-exclusion
+                            const double xs[3] = {x0, x1, x2}, ys[3] = {y0, y1, y2};
+                            const double f00 = tri_pixel_area(xs, ys, idx, idy, 0.0, 0.0) * (2.0 / A2);
+                            const double fl = frac_below(x0 - 1.0, x1 - 1.0, x2 - 1.0), fb = frac_below(y0 - 1.0, y1 - 1.0, y2 - 1.0);
+                            const unsigned long long a00 = to_fix(f00), a10 = to_fix(fb - f00), a01 = to_fix(fl - f00);
+                            const unsigned long long rest = a00 + a10 + a01;
+                            pix_add(S, W, lox, loy, a00);
+                            pix_add(S, W, lox + 1, loy, a10);
+                            pix_add(S, W, lox, loy + 1, a01);
+                            pix_add(S, W, lox + 1, loy + 1, rest < FIX_ONE ? FIX_ONE - rest : 0ull);
+                            done += 4;
+                        } else {
+                            npx = (int)((wc * hc < (1ll << 26)) ? wc * hc : (1ll << 26));   // (only a full queue can bring such boxes here)
+                            double *rc = rec[lane];
+                            rc[0] = 2.0 / A2;
+                            rc[1] = __hiloint2double(loy, lox);
+                            rc[2] = __hiloint2double((int)fby, (int)fbx);
+                            rc[3] = __hiloint2double(0, (int)wc);
+                            rc[4] = idx[0]; rc[5] = idx[1]; rc[6] = idx[2]; rc[7] = idy[0]; rc[8] = idy[1]; rc[9] = idy[2];
+                        }
                     }
                 }
             }
@@ -409,7 +423,7 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
 
 // The shooting kernel's own copy, for the triangles it could not hand to the global queue (queue full).
 // Out of line, cold.
-static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w32, int ax, int ay, WarpShared *Wsp, int head, int n) {
+static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w32, int ax, int ay, WarpSharedIpm *Wsp, int head, int n) {
     Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
     int done = 0;
     __syncwarp();

@@ -41,7 +41,7 @@ struct Pend {
 };
 
 // Runs the pending-work rings down to fewer than `keep` entries (keep = 32 inside a tile, 1 at the end).
-__device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, WarpShared &Ws, Pend &P, int keep, ThreadCounters &tc) {
+__device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, int keep, ThreadCounters &tc) {
     const int lane = threadIdx.x & 31;
     while (P.S2.count >= keep) {
         const int n = min(P.S2.count, 32);
@@ -60,7 +60,7 @@ __device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, War
 // General triangles go to the global queue, which drain_kernel apportions at full occupancy.  A warp reserves
 // QCHUNK entries at a time (one atomic per chunk); if the queue is full they stay in the warp's own ring and
 // are clipped by the (cold) in-kernel copy.
-__device__ __forceinline__ void queue_push(const ShootDev &S, WarpShared &Ws, Pend &P, bool pred, const double (&e)[6], ThreadCounters &tc) {
+__device__ __forceinline__ void queue_push(const ShootDev &S, WarpSharedIpm &Ws, Pend &P, bool pred, const double (&e)[6], ThreadCounters &tc) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const unsigned m = __ballot_sync(full, pred);
@@ -94,7 +94,7 @@ __device__ __forceinline__ void queue_push(const ShootDev &S, WarpShared &Ws, Pe
 //   a = (prev, lane), b = (prev, lane+1), c = (cur, lane+1), d = (cur, lane);  T1 = a, b, c;  T2 = a, c, d  (reading G9)
 // Triangles inside one pixel are run-length merged and added at once; two-pixel strips and general triangles
 // are pushed onto the warp's rings and apportioned 32 at a time.
-__device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpShared &Ws, Pend &P, int prev, int cur, bool cellv,
+__device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, int prev, int cur, bool cellv,
                                          ThreadCounters &tc) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31, l1 = min(lane + 1, 31);
@@ -144,15 +144,13 @@ __device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSh
             s4[3] = __hiloint2double((mny << 16) | (mnx & 0xffff), (ay ? 1 : 0) | (A2 == 0.0 ? 2 : 0));
             ring_push<4>(P.S2, Ws.ringS, strip, s4);
         }
-        if (S.dbg & 1) P.E.count = 0;
-        if (S.dbg & 2) P.S2.count = 0;
         run_batches(S, W, Ws, P, 32, tc);
     }
 }
 
 __global__ void __launch_bounds__(SHOOT_WARPS * 32) shoot_ipm_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    WarpShared &Ws = reinterpret_cast<WarpShared *>(smem_raw)[threadIdx.x >> 5];
+    WarpSharedIpm &Ws = reinterpret_cast<WarpSharedIpm *>(smem_raw)[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     ThreadCounters tc;
@@ -168,7 +166,7 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32) shoot_ipm_kernel(const __gri
         const int tx = (int)(tile % S.ntx);
         const long long ci0 = S.i0 + (long long)tx * (TCX - 1), cj0 = S.j0 + ty * (TCY - 1);
         const long long ci1 = min(ci0 + TCX - 1, S.i1), cj1 = min(cj0 + TCY - 1, S.j1);   // last corner of the tile
-        wtile_setup(S, Ws, C, ci0, cj0, ci1, cj1, 0.0, &S.counters[C_TILES_FULL]);
+        wtile_setup(S, Ws, C, ci0, cj0, ci1, cj1, 0.0);
 
         const long long ci = ci0 + lane;
         const bool colv = ci <= S.i1, cellv = (lane < TCX - 1) && (ci < S.i1);
@@ -317,7 +315,7 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32) shoot_irs_kernel(const __gri
         const int tx = (int)(tile % S.ntx);
         const long long ci0 = S.i0 + (long long)tx * TCX, cj0 = S.j0 + ty * TCY;
         const long long ci1 = min(ci0 + TCX, S.i1) - 1, cj1 = min(cj0 + TCY, S.j1) - 1;      // last cell of the tile
-        wtile_setup(S, Ws, C, ci0, cj0, ci1, cj1, 0.5, &S.counters[C_TILES_FULL]);
+        wtile_setup(S, Ws, C, ci0, cj0, ci1, cj1, 0.5);
         const long long ci = ci0 + lane;
         for (int g = 0; g < NGRP; ++g) {
             if (cj0 + g * RPT >= S.j1) break;
@@ -479,7 +477,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if (ipm) {
         ML_TRY(f->diff.reserve((size_t)npix, s, false));
         ML_CUDA(cudaMemsetAsync(f->diff.p, 0, (size_t)npix * 8, s));
-        long long qmb = env_ll("MLENS_QUEUE_MB", 1024);
+        long long qmb = env_ll("MLENS_QUEUE_MB", 2048);
         qcap = qmb * (1ll << 20) / (QCHUNK * QENT * 8);              // chunks
         ML_TRY(f->queue.reserve((size_t)qcap * QCHUNK * QENT, s, false));
         ML_TRY(f->qcount.reserve((size_t)qcap, s, false));
@@ -500,7 +498,6 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if (S.tq > TQMAX) S.tq = TQMAX;
     if (S.tq < 2) S.tq = 2;
     S.small_px = (int)env_ll("MLENS_SMALL_PX", 64);
-    S.dbg = (int)env_ll("MLENS_DBG", 0);
     // truncation budget of the tile series: 5 % of the deflection accuracy the field was built for
     S.eps_far = 0.02 * f->eps * f->theta;
     S.eps_star = 0.03 * f->eps * f->theta / (double)ML_NEAR;
@@ -511,7 +508,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 26);
+    long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 27);
     long long rows_per_band = band_cells / (ntx * stepx * stepy);
     if (rows_per_band < 1) rows_per_band = 1;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -525,16 +522,16 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         cudaEvent_t e; ML_CUDA(cudaEventCreate(&e)); ML_CUDA(cudaEventRecord(e, s)); ev.push_back(e);
         return MLENS_OK;
     };
-    const size_t smem = SHOOT_WARPS * sizeof(WarpShared);
+    const size_t smem_ipm = SHOOT_WARPS * sizeof(WarpSharedIpm), smem_irs = SHOOT_WARPS * sizeof(WarpShared);
     static bool attr_set = false;
     if (!attr_set) {
-        ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
+        ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_irs));
         attr_set = true;
     }
     int bps_ipm = 1, bps_irs = 1;
-    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_ipm, shoot_ipm_kernel, SHOOT_WARPS * 32, smem));
-    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_irs, shoot_irs_kernel, SHOOT_WARPS * 32, smem));
+    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_ipm, shoot_ipm_kernel, SHOOT_WARPS * 32, smem_ipm));
+    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_irs, shoot_irs_kernel, SHOOT_WARPS * 32, smem_irs));
     if (bps_ipm < 1 || bps_irs < 1) { set_error("shooting kernels do not fit on this device"); return MLENS_ECUDA; }
     for (long long r0 = 0; r0 < nty; r0 += rows_per_band, ++bands) {
         S.tile_row0 = r0;
@@ -547,14 +544,14 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         ML_CUDA(cudaMemsetAsync(f->counters.p + C_DRAIN, 0, 3 * 8, s));   // drain, big-list and walk counters
         ML_TRY(mark());
         if (ipm) {
-            ML_LAUNCH(shoot_ipm_kernel, grid, SHOOT_WARPS * 32, smem, s, S);
+            ML_LAUNCH(shoot_ipm_kernel, grid, SHOOT_WARPS * 32, smem_ipm, s, S);
             ML_TRY(mark());
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
             ML_LAUNCH(walk_kernel, nsm * 8, 256, 0, s, S);
             ML_TRY(mark());
             launches += 3;
         } else {
-            ML_LAUNCH(shoot_irs_kernel, grid, SHOOT_WARPS * 32, smem, s, S);
+            ML_LAUNCH(shoot_irs_kernel, grid, SHOOT_WARPS * 32, smem_irs, s, S);
             ML_TRY(mark());
             launches += 1;
         }
@@ -575,12 +572,12 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         memset(st, 0, sizeof(*st));
         st->n_rays = (int64_t)h[C_RAYS];
         st->n_cells = (i1 - i0) * (j1 - j0);
-        st->n_tri_single = (int64_t)h[C_SINGLE]; st->n_tri_small = (int64_t)h[C_SMALL];
-        st->n_tri_queued = (int64_t)h[C_QUEUED]; st->n_queue_chunks = (int64_t)h[C_QUEUED];
+        st->n_tri_single = (int64_t)h[C_SINGLE]; st->n_tri_strip = (int64_t)h[C_SMALL];
+        st->n_tri_queued = (int64_t)h[C_QUEUED]; st->n_tri_walked = (int64_t)h[C_BIG];
         st->n_queue_overflow = (int64_t)h[C_OVERFLOW]; st->n_rays_fallback = (int64_t)h[C_FALLBACK];
         st->n_near_terms = (int64_t)h[C_NEAR];
-        st->n_px_small = (int64_t)h[C_PX_SMALL]; st->n_px_interior = (int64_t)h[C_PX_INT];
-        st->n_px_edge = (int64_t)h[C_PX_EDGE]; st->n_rows = 0;
+        st->n_px_strip = (int64_t)h[C_PX_SMALL]; st->n_px_clipped = (int64_t)h[C_PX_INT];
+        st->n_edge_steps = (int64_t)h[C_PX_EDGE];
         st->n_tiles_full = (int64_t)h[C_TILES_FULL];
         st->tile_order = S.tq;
         st->n_bands = bands; st->gpu_launches = launches; st->n_shoot_launches = bands;

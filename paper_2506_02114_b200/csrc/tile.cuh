@@ -23,6 +23,10 @@ static const int WX = 32, WY = 16;    // per-warp shared-memory pixel window
 static const int FOLDJ = WX * WY * 8 / (32 * 16);   // series terms per pass of the star folding (scratch = the window)
 static const int BN = 2 * ML_P1MAX;   // stride of the Pascal triangle
 
+// slots of ShootDev::counters
+enum { C_QUEUE = 0, C_TILE, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR,
+       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_BIG, C_WALK, C_NCOUNTERS };
+
 // What a shooting kernel needs besides the lens: the ray grid, the map, the accumulators.
 struct ShootDev {
     LensDev L;
@@ -45,23 +49,26 @@ struct ShootDev {
     long long tile_row0, tile_rows;    // band of tile rows handled by this launch
     int tq;                            // order of the tile series
     double eps_far, eps_star;          // truncation budgets of the tile series (absolute, units of theta)
-    int dbg;
-    int small_px;                      // triangles whose bounding box has more pixels than this go to the global queue
+    int small_px;                      // queued triangles whose clipped bounding box has more pixels than this are walked, not clipped
 };
 
 __device__ __forceinline__ double corner_x(const ShootDev &S, long long i) { return __dadd_rn(S.x0_1, __dmul_rn((double)i, S.h1)); }
 __device__ __forceinline__ double corner_y(const ShootDev &S, long long j) { return __dadd_rn(S.x0_2, __dmul_rn((double)j, S.h2)); }
 
-// Per-warp shared memory.  `win` doubles as the scratch of the tile set-up (fold terms), which is why it
-// is zeroed at the end of the set-up and not by the flush.
+// Per-warp shared memory of the evaluator.  `win` doubles as the scratch of the tile set-up (fold terms), which
+// is why it is zeroed at the end of the set-up and not by the flush.
 struct WarpShared {
     unsigned long long win[WY * WX];                         // 4 KB
-    double2 t[NSLOT][TQMAX + 1];                                 // conj(alpha)(u) = sum_j t_j u^j, theta^2 included
+    double2 t[NSLOT][TQMAX + 1];                             // conj(alpha)(u) = sum_j t_j u^j, theta^2 included
     double sx[NSLOT][ML_NEAR], sy[NSLOT][ML_NEAR], sm[NSLOT][ML_NEAR];   // direct stars (absolute positions, m theta^2)
     double2 e[ML_P1MAX];                                     // the leaf's derivative series (set-up scratch)
     uint32_t bx0[NSLOT], bx1[NSLOT], by0[NSLOT], by1[NSLOT];
     int leaf[NSLOT], node[NSLOT], nd[NSLOT], mode[NSLOT];
-    double ringE[64][6];                                     // pending general triangles (3 vertices, pixel units)
+    double ctx[4];                                           // zt_x, zt_y, 1/rt, fast flag: what the set-up hands back
+};
+// ... plus what the IPM kernel needs for apportioning
+struct WarpSharedIpm : WarpShared {
+    double ringE[64][6];                                     // pending general triangles the global queue could not take
     double ringS[64][4];                                     // pending two-pixel strips
     double rec[32][10];                                      // per-triangle records of the batch being apportioned
     double stu[RPT + 1][32], stv[RPT + 1][32];               // mapped corners of the row group in pixel units (row 0 = last row of the previous group)
@@ -176,12 +183,21 @@ __device__ __forceinline__ void zero_window(WarpShared &W) {
 
 // Sets up the warp's tile: centre, radius, leaves of the four extreme rays, one slot per distinct leaf.
 // off = offset of the rays from the grid corners in cells (0 for IPM, 0.5 for IRS).  Leaves the window zeroed.
-__device__ __forceinline__ void wtile_setup(const ShootDev &S, WarpShared &W, TileCtx &C, long long ci0, long long cj0,
-                                            long long ci1, long long cj1, double off, unsigned long long *full_counter) {
+static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShared *Wp, long long ci0, long long cj0,
+                                                    long long ci1, long long cj1, double off) {
+    const ShootDev &S = *Sp;
+    WarpShared &W = *Wp;
+    TileCtx C;
+    unsigned long long *full_counter = &S.counters[C_TILES_FULL];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     C.inv_rt = 1.0; C.fast = false; C.zt_x = 0.0; C.zt_y = 0.0;
-    if (S.eval_mode != MLENS_EVAL_FMM) { zero_window(W); __syncwarp(); return; }
+    if (S.eval_mode != MLENS_EVAL_FMM) {
+        zero_window(W);
+        if (lane == 0) { W.ctx[0] = 0.0; W.ctx[1] = 0.0; W.ctx[2] = 1.0; W.ctx[3] = 0.0; }
+        __syncwarp();
+        return;
+    }
     const double rt = 0.5 * sqrt((double)((TCX - 1) * (TCX - 1)) * S.h1 * S.h1 + (double)((TCY - 1) * (TCY - 1)) * S.h2 * S.h2) * (1.0 + 1e-9);
     C.zt_x = corner_x(S, ci0) + (0.5 * (TCX - 1) + off) * S.h1;
     C.zt_y = corner_y(S, cj0) + (0.5 * (TCY - 1) + off) * S.h2;
@@ -222,8 +238,14 @@ __device__ __forceinline__ void wtile_setup(const ShootDev &S, WarpShared &W, Ti
         if (lane == 0 && W.mode[s] == 1 && full_counter) atomicAdd(full_counter, 1ull);
     }
     zero_window(W);
+    if (lane == 0) { W.ctx[0] = C.zt_x; W.ctx[1] = C.zt_y; W.ctx[2] = C.inv_rt; W.ctx[3] = (one_leaf && W.mode[0] == 0) ? 1.0 : 0.0; }
     __syncwarp();
-    C.fast = one_leaf && W.mode[0] == 0;
+}
+// Sets up the warp's tile (out of line: once per 1024 rays) and returns its context in registers.
+__device__ __forceinline__ void wtile_setup(const ShootDev &S, WarpShared &W, TileCtx &C, long long ci0, long long cj0,
+                                            long long ci1, long long cj1, double off) {
+    wtile_setup_ool(&S, &W, ci0, cj0, ci1, cj1, off);
+    C.zt_x = W.ctx[0]; C.zt_y = W.ctx[1]; C.inv_rt = W.ctx[2]; C.fast = W.ctx[3] != 0.0;
 }
 
 struct ThreadCounters { unsigned int single = 0, small_ = 0, queued = 0, chunks = 0, overflow = 0, fallback = 0, rays = 0, near_ = 0, px_small = 0; };
@@ -260,11 +282,34 @@ static __device__ __noinline__ double2 eval_one_ool(const ShootDev *Sp, const Wa
     return make_double2(sr, -si);
 }
 
+// The RPT rays of one lane when the fast path does not apply (tile straddling leaves, failed bound, partial
+// tile, DIRECT mode): one ray at a time, out of line.  Results go through a small local array.
+static __device__ __noinline__ void eval_group_ool(const ShootDev *Sp, const WarpShared *T, double x, double ux, double y0, double y1,
+                                                   double y2, double y3, double uy0, double duy, unsigned validmask,
+                                                   double *w /* [2 RPT] */, int *cnt /* rays, near, fallback */) {
+    const ShootDev &S = *Sp;
+    static_assert(RPT == 4, "four rows per group");
+#pragma unroll 1
+    for (int r = 0; r < RPT; ++r) {
+        w[2 * r] = 0.0; w[2 * r + 1] = 0.0;
+        if (!((validmask >> r) & 1u)) continue;
+        const double y = (r == 0) ? y0 : (r == 1) ? y1 : (r == 2) ? y2 : y3;
+        ++cnt[0];
+        double2 a;
+        if (S.eval_mode == MLENS_EVAL_DIRECT) a = direct_all_ool(&S.L, x, y);
+        else {
+            int kind;
+            a = eval_one_ool(Sp, T, x, y, ux, uy0 + duy * (double)r, &kind);
+            if (kind >= 0) cnt[1] += kind; else ++cnt[2];
+        }
+        lens_w(S.L, x, y, a.x, a.y, w[2 * r], w[2 * r + 1]);
+    }
+}
+
 // w(z) of eq 12 for the RPT rays of one lane (same column, consecutive rows).
 __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T, const TileCtx &C, const double (&x)[RPT],
                                           const double (&y)[RPT], const double (&ux)[RPT], const double (&uy)[RPT],
                                           const bool (&valid)[RPT], double (&wx)[RPT], double (&wy)[RPT], ThreadCounters &tc) {
-    double ax[RPT], ay[RPT];
     bool all = true;
 #pragma unroll
     for (int r = 0; r < RPT; ++r) all = all && valid[r];
@@ -300,27 +345,18 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
             }
         }
 #pragma unroll
-        for (int r = 0; r < RPT; ++r) { ax[r] = sr[r]; ay[r] = -si[r]; }
+        for (int r = 0; r < RPT; ++r) lens_w(S.L, x[r], y[r], sr[r], -si[r], wx[r], wy[r]);
     } else {
+        double w[2 * RPT];
+        int cnt[3] = {0, 0, 0};
+        unsigned vm = 0;
 #pragma unroll
-        for (int r = 0; r < RPT; ++r) {
-            ax[r] = ay[r] = 0.0;
-            if (!valid[r]) continue;
-            ++tc.rays;
-            double2 a;
-            if (S.eval_mode == MLENS_EVAL_DIRECT) a = direct_all_ool(&S.L, x[r], y[r]);
-            else {
-                int kind;
-                a = eval_one_ool(&S, &T, x[r], y[r], ux[r], uy[r], &kind);
-                if (kind >= 0) tc.near_ += (unsigned int)kind; else ++tc.fallback;
-            }
-            ax[r] = a.x; ay[r] = a.y;
-        }
+        for (int r = 0; r < RPT; ++r) vm |= valid[r] ? (1u << r) : 0u;
+        eval_group_ool(&S, &T, x[0], ux[0], y[0], y[1], y[2], y[3], uy[0], uy[1] - uy[0], vm, w, cnt);
+        tc.rays += cnt[0]; tc.near_ += cnt[1]; tc.fallback += cnt[2];
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) { wx[r] = w[2 * r]; wy[r] = w[2 * r + 1]; }
     }
-#pragma unroll
-    for (int r = 0; r < RPT; ++r)
-        if (valid[r]) lens_w(S.L, x[r], y[r], ax[r], ay[r], wx[r], wy[r]);
-        else { wx[r] = 0.0; wy[r] = 0.0; }
 }
 
 }  // namespace ml

@@ -70,12 +70,12 @@ class Grid(C.Structure):
 
 
 class Stats(C.Structure):
-    _fields_ = [("n_rays", C.c_int64), ("n_cells", C.c_int64), ("n_tri_single", C.c_int64), ("n_tri_small", C.c_int64),
-                ("n_tri_queued", C.c_int64), ("n_queue_chunks", C.c_int64), ("n_queue_overflow", C.c_int64),
+    _fields_ = [("n_rays", C.c_int64), ("n_cells", C.c_int64), ("n_tri_single", C.c_int64), ("n_tri_strip", C.c_int64),
+                ("n_tri_queued", C.c_int64), ("n_tri_walked", C.c_int64), ("n_queue_overflow", C.c_int64),
                 ("n_rays_fallback", C.c_int64), ("n_bands", C.c_int32), ("gpu_launches", C.c_int32),
                 ("ms_total", C.c_float), ("ms_shoot", C.c_float), ("ms_drain", C.c_float),
                 ("ms_finalise", C.c_float), ("n_shoot_launches", C.c_int32), ("n_near_terms", C.c_int64),
-                ("n_px_small", C.c_int64), ("n_px_interior", C.c_int64), ("n_px_edge", C.c_int64), ("n_rows", C.c_int64),
+                ("n_px_strip", C.c_int64), ("n_px_clipped", C.c_int64), ("n_edge_steps", C.c_int64), ("reserved_", C.c_int64),
                 ("n_tiles_full", C.c_int64), ("tile_order", C.c_int32), ("pad_", C.c_int32)]
 
     def as_dict(self):

@@ -219,7 +219,8 @@ def test_ipm_map_config0_whole(ml, orc):
     assert res.map.sum() == pytest.approx(ref.sum(), rel=1e-9)
     st = res.stats
     assert st["n_cells"] == g.n1 * g.n2
-    assert st["n_tri_single"] + st["n_tri_small"] + st["n_tri_queued"] + st["n_queue_overflow"] <= 2 * st["n_cells"]
+    assert st["n_tri_single"] + st["n_tri_strip"] + st["n_tri_queued"] + st["n_queue_overflow"] <= 2 * st["n_cells"]
+    assert st["n_queue_overflow"] == 0 and st["n_tri_walked"] <= st["n_tri_queued"]
     # the "no FMM" mode gives the same map
     res2 = gf.shoot(cfg.half_y, cfg.npix, cfg.rays_per_pixel_length, border_mode=cfg.border_mode,
                     border_param=cfg.border_param, eval_mode=ml.EVAL_DIRECT)
@@ -314,3 +315,103 @@ def test_errors(ml):
     # more than 32 coincident stars cannot be separated by the tree
     with pytest.raises(ml.MlensError):
         ml.Field.from_stars(0.5, 0.1, np.full(40, 0.3), np.full(40, 0.3), np.ones(40), kappa_star=0.1, R=2.0)
+
+
+# ----------------------------------------------------------------------------- apportioning paths
+def _with_env(**env):
+    """Context manager: environment knobs libmlens reads at every shoot call."""
+    import contextlib
+    import os
+
+    @contextlib.contextmanager
+    def cm():
+        old = {k: os.environ.get(k) for k in env}
+        os.environ.update({k: str(v) for k, v in env.items()})
+        try:
+            yield
+        finally:
+            for k, v in old.items():
+                if v is None:
+                    os.environ.pop(k, None)
+                else:
+                    os.environ[k] = v
+    return cm()
+
+
+def test_apportioning_paths_agree(ml, orc):
+    # The same map through (a) pixel clipping of every queued triangle, (b) the edge walk of every queued
+    # triangle, (c) a queue too small to take them (the shooting kernel's own fallback), (d) one-tile bands:
+    # four routes to the same area integrals.  All must match the oracle; (a)-(d) match each other far tighter.
+    cfg, gf, of, _ = _cfg_field(ml, orc, 0)
+    kw = dict(border_mode=cfg.border_mode, border_param=cfg.border_param)
+    g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, 96, 2.0, cfg.border_mode, cfg.border_param)
+    ref = orc.shoot(of, g, 0)
+    base = gf.shoot(cfg.half_y, 96, 2.0, **kw)
+    _map_check(base.map, ref, "default")
+    assert base.stats["n_tri_walked"] > 0 and base.stats["n_px_clipped"] > 0 and base.stats["n_queue_overflow"] == 0
+    with _with_env(MLENS_SMALL_PX=100000000):
+        clip = gf.shoot(cfg.half_y, 96, 2.0, **kw)
+    assert clip.stats["n_tri_walked"] == 0
+    with _with_env(MLENS_SMALL_PX=1):
+        walk = gf.shoot(cfg.half_y, 96, 2.0, **kw)
+    assert walk.stats["n_tri_walked"] > base.stats["n_tri_walked"]
+    with _with_env(MLENS_QUEUE_MB=1, MLENS_BAND_CELLS=1 << 30):
+        over = gf.shoot(cfg.half_y, 96, 2.0, **kw)
+    assert over.stats["n_queue_overflow"] > 0
+    with _with_env(MLENS_BAND_CELLS=1):
+        bands = gf.shoot(cfg.half_y, 96, 2.0, **kw)
+    assert bands.stats["n_bands"] > 10
+    for name, r in (("clip", clip), ("walk", walk), ("overflow", over), ("bands", bands)):
+        _map_check(r.map, ref, name)
+        assert np.max(np.abs(r.map - base.map)) <= 1e-9 * base.map.max(), name
+        assert r.map.sum() == pytest.approx(base.map.sum(), rel=1e-11)
+    assert np.array_equal(bands.map, base.map)          # same routes, other launch split: bit-identical (integer sums)
+
+
+def test_giant_triangles_conserve_flux(ml, orc):
+    # one star in the middle of the window: the cells around it map to triangles far larger than the map.
+    # Every route must put exactly the in-map part of them into the map.
+    f = ml.Field.from_stars(0.3, 0.1, np.array([0.013]), np.array([-0.007]), np.ones(1), kappa_star=0.0, R=1e9)
+    of = orc.Field.make(0.3, 0.0, 0.1, [0.013], [-0.007], [1.0], R=1e9)
+    g = orc.geometry(0.3, 0.0, 0.1, 1.0, 40, 3.0, 3, He=(2.2, 2.6))
+    ref = orc.shoot(of, g, 0)
+    res = f.shoot(1.0, 40, 3.0, border_mode=BORDER_EXPLICIT, He=(2.2, 2.6))
+    assert res.stats["n_tri_walked"] > 0
+    _map_check(res.map, ref, "one star")
+    assert res.map.sum() == pytest.approx(ref.sum(), rel=1e-9)
+
+
+def test_nonsquare_offcentre_map(ml, orc):
+    cfg, gf, of, _ = _cfg_field(ml, orc, 0)
+    half, npix, Y = (3.0, 2.0), (72, 40), (0.7, -0.4)
+    g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, half, npix, 2.0, 0, Y=Y)
+    res = gf.shoot(half, npix, 2.0, border_mode=ml.BORDER_EQ16, center=Y)
+    assert (res.grid.n1, res.grid.n2, res.grid.x0_1, res.grid.x0_2) == (g.n1, g.n2, g.x0_1, g.x0_2)
+    assert res.map.shape == (40, 72)
+    _map_check(res.map, orc.shoot(of, g, 0), "non-square, off-centre")
+    irs = gf.shoot(half, npix, 2.0, border_mode=ml.BORDER_EQ16, center=Y, map_mode=ml.MAP_IRS, dump=True, want_counts=True)
+    assert np.array_equal(irs.counts, orc.bin_irs(irs.dump[0], irs.dump[1], g))
+
+
+def test_rect_field_map(ml, orc):
+    # rectangular star region (P:165, eq B7) through the whole IPM path
+    n, c1, c2 = 300, 30.0, 12.0
+    ks = math.pi * n / (4 * c1 * c2)
+    xs, ys, ms = synth.rect_stars(n, c1, c2, 11)
+    gf = ml.Field.from_stars(0.5, 0.1, xs, ys, ms, kappa_star=ks, shape=ml.SHAPE_RECT, c1=c1, c2=c2)
+    of = orc.Field.make(0.5, ks, 0.1, xs, ys, ms, shape=1, c1=c1, c2=c2)
+    g = orc.geometry(0.5, ks, 0.1, 2.0, 48, 2.0, 2, 0.2)
+    res = gf.shoot(2.0, 48, 2.0, border_mode=ml.BORDER_MARGIN, border_param=0.2)
+    _map_check(res.map, orc.shoot(of, g, 0), "rectangle")
+
+
+def test_ipm_and_irs_agree_on_gpu(ml):
+    # P:288 "we do not find any differences": IRS at high density converges to the IPM map within Poisson error
+    cfg = synth.get_config(0)
+    f = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, 5, kappa_star=cfg.kappa_star)
+    kw = dict(border_mode=ml.BORDER_EQ16)
+    ipm = f.shoot(4.0, 32, 2.0, **kw).map
+    irs = f.shoot(4.0, 32, 24.0, map_mode=ml.MAP_IRS, **kw).map
+    sig = np.sqrt(np.maximum(irs, 1e-9) / 24.0 ** 2)
+    assert np.mean(np.abs(irs - ipm) / sig) < 1.5 and np.max(np.abs(irs - ipm) / sig) < 8.0
+    assert irs.mean() == pytest.approx(ipm.mean(), rel=5e-3)
