@@ -395,7 +395,10 @@ __device__ __forceinline__ unsigned apportion_batch(const ShootDev &S, const Win
 }
 
 // Warp-cooperative edge walk of one large triangle (v = its 3 vertices in pixel units, same in all lanes).
-__device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT]) {
+// Lanes 0-2 set up one edge each into `scratch` (3 x 16 doubles of the warp's shared memory); then the steps
+// of all three edges form one index space the lanes stride over, so a triangle of a few dozen steps still
+// fills the warp.
+__device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT], double *scratch) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
@@ -409,16 +412,32 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
     const double fbx = (double)bx, fby = (double)by;
     const double hgt = fmax(v[1], fmax(v[3], v[5])) - fby + 1.0;
     const double ry0 = fmax(0.0, -fby), ry1 = fmin(hgt, (double)S.npix2 - fby), cx1 = (double)S.npix1 - fbx;
-    unsigned long long n_pieces = 0;
-#pragma unroll 1
-    for (int ed = 0; ed < 3; ++ed) {
-        const int ia = 2 * ed, ib = (ed == 2) ? 0 : 2 * ed + 2;
+    int ne = 0;
+    __syncwarp();
+    if (lane < 3) {
+        const double xa = (lane == 0) ? v[0] : (lane == 1) ? v[2] : v[4], ya = (lane == 0) ? v[1] : (lane == 1) ? v[3] : v[5];
+        const double xb = (lane == 0) ? v[2] : (lane == 1) ? v[4] : v[0], yb = (lane == 0) ? v[3] : (lane == 1) ? v[5] : v[1];
         EdgeWalk E;
-        edge_setup(E, v[ia] - fbx, v[ia + 1] - fby, v[ib] - fbx, v[ib + 1] - fby, ry0, ry1, cx1);
-        for (int k = lane; k < E.n; k += 32) edge_step(S, E, k, cs, bx, by);
-        n_pieces += (unsigned long long)E.n;
+        edge_setup(E, xa - fbx, ya - fby, xb - fbx, yb - fby, ry0, ry1, cx1);
+        double *q = scratch + 16 * lane;
+        q[0] = E.x0; q[1] = E.y0; q[2] = E.x1; q[3] = E.y1; q[4] = E.dx; q[5] = E.dy; q[6] = E.idx; q[7] = E.idy;
+        q[8] = E.ta; q[9] = E.tb; q[10] = E.g0; q[11] = E.sg; q[12] = __hiloint2double(E.n, E.majorY);
+        ne = E.n;
     }
-    return n_pieces;
+    const int n0 = __shfl_sync(full, ne, 0), n1 = __shfl_sync(full, ne, 1), n2 = __shfl_sync(full, ne, 2);
+    const int total = n0 + n1 + n2;
+    __syncwarp();
+#pragma unroll 1
+    for (int k = lane; k < total; k += 32) {
+        const int e = (k >= n0 + n1) ? 2 : (k >= n0 ? 1 : 0);
+        const double *q = scratch + 16 * e;
+        EdgeWalk E;
+        E.x0 = q[0]; E.y0 = q[1]; E.x1 = q[2]; E.y1 = q[3]; E.dx = q[4]; E.dy = q[5]; E.idx = q[6]; E.idy = q[7];
+        E.ta = q[8]; E.tb = q[9]; E.g0 = q[10]; E.sg = q[11]; E.majorY = __double2loint(q[12]); E.n = __double2hiint(q[12]);
+        edge_step(S, E, k - (e == 2 ? n0 + n1 : (e == 1 ? n0 : 0)), cs, bx, by);
+    }
+    __syncwarp();
+    return (unsigned long long)total;
 }
 
 // The shooting kernel's own copy, for the triangles it could not hand to the global queue (queue full).
@@ -434,7 +453,7 @@ static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w
         double v[QENT];
 #pragma unroll
         for (int k = 0; k < QENT; ++k) v[k] = Wsp->ringE[(head + i) & 63][k];
-        walk_triangle(*Sp, v);
+        walk_triangle(*Sp, v, &Wsp->rec[0][0]);
     }
     return done;
 }

@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_co
                 double v[QENT];
 #pragma unroll
                 for (int k = 0; k < QENT; ++k) v[k] = base[(size_t)(b0 + i) * QENT + k];
-                n_pieces += walk_triangle(S, v);
+                n_pieces += walk_triangle(S, v, &rec[0][0]);
             }
         }
     }
@@ -277,6 +277,8 @@ __global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_co
 
 // Edge walk of the large triangles the drain set aside: one warp per triangle, handed out one at a time.
 __global__ void __launch_bounds__(256) walk_kernel(const __grid_constant__ ShootDev S) {
+    __shared__ double scratch_s[8][48];
+    double *scratch = scratch_s[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     long long nb = (long long)S.counters[C_BIG];
@@ -291,9 +293,10 @@ __global__ void __launch_bounds__(256) walk_kernel(const __grid_constant__ Shoot
         double v[QENT];
 #pragma unroll
         for (int k = 0; k < QENT; ++k) v[k] = __ldg(&e[k]);
-        n_pieces += walk_triangle(S, v);
+        n_pieces += walk_triangle(S, v, scratch);
     }
     if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&S.counters[C_CHUNKS], (unsigned long long)nb);   // walked, all bands
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -573,7 +576,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         st->n_rays = (int64_t)h[C_RAYS];
         st->n_cells = (i1 - i0) * (j1 - j0);
         st->n_tri_single = (int64_t)h[C_SINGLE]; st->n_tri_strip = (int64_t)h[C_SMALL];
-        st->n_tri_queued = (int64_t)h[C_QUEUED]; st->n_tri_walked = (int64_t)h[C_BIG];
+        st->n_tri_queued = (int64_t)h[C_QUEUED]; st->n_tri_walked = (int64_t)h[C_CHUNKS];
         st->n_queue_overflow = (int64_t)h[C_OVERFLOW]; st->n_rays_fallback = (int64_t)h[C_FALLBACK];
         st->n_near_terms = (int64_t)h[C_NEAR];
         st->n_px_strip = (int64_t)h[C_PX_SMALL]; st->n_px_clipped = (int64_t)h[C_PX_INT];
