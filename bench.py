@@ -48,8 +48,8 @@ UNIT = "evals/s"
 # by mlens_bench_dfma in the same run is reported beside it as `peak_measured_dfma`.
 FP64_LANES_PER_SM = 64
 # dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/r01_ncu_full_shoot_ipm.md); None until a capture exists for the current kernel.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# (profiles/r01b_ncu_full.md: dram read + write of shoot_ipm_kernel, mean of the two captured launches).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 515.0e6
 
 
 def parse():
