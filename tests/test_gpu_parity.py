@@ -160,7 +160,7 @@ def test_fmm_coefficients_against_definitions(ml, orc):
 
 
 # ----------------------------------------------------------------------------- deflection (the 1e-8 surface)
-@pytest.mark.parametrize("idx,npts", [(0, 100000), (1, 40000), (2, 6000)])
+@pytest.mark.parametrize("idx,npts", [(0, 100000), (1, 40000), (2, 6000), (3, 2400), (4, 800)])
 def test_deflection_parity(ml, orc, idx, npts):
     cfg, gf, of, (xs, ys, ms, R) = _cfg_field(ml, orc, idx)
     g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, cfg.npix, cfg.rays_per_pixel_length,
@@ -244,32 +244,41 @@ def test_irs_counts_exact_config0(ml, orc):
     assert np.sum(own != want) <= 4
 
 
-@pytest.mark.parametrize("idx", [1, 2])
-def test_ipm_patches_big_configs(ml, orc, idx):
-    cfg, gf, of, (xs, ys, ms, R) = _cfg_field(ml, orc, idx, n_override=20000 if idx == 2 else None)
-    k = cfg.rays_per_pixel_length
-    half, npix = (cfg.half_y, cfg.npix) if idx == 1 else (cfg.half_y * 0.2, cfg.npix // 5)
+@pytest.mark.parametrize("idx,P,npatch", [(1, 128, 8), (2, 64, 5), (3, 32, 4), (4, 24, 3)])
+def test_ipm_patches_big_configs(ml, orc, idx, P, npatch):
+    # configs too large for a whole oracle map: index-aligned patches of P x P cells shot by both sides into
+    # partial maps (one holding a star, the window corners, random ones), at the configs' full star counts
+    cfg, gf, of, (xs, ys, ms, R) = _cfg_field(ml, orc, idx)
+    k, half, npix = cfg.rays_per_pixel_length, cfg.half_y, cfg.npix
     g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, half, npix, k, cfg.border_mode, cfg.border_param,
                      m2_over_m=cfg.m2_over_m)
+    gg = gf.grid(half, npix, k, border_mode=cfg.border_mode, border_param=cfg.border_param)
+    assert (gg.n1, gg.n2, gg.x0_1, gg.x0_2, gg.h1, gg.h2) == (g.n1, g.n2, g.x0_1, g.x0_2, g.h1, g.h2)
     rng = np.random.default_rng(5)
     inside = np.where((np.abs(xs) < g.H1 * 0.9) & (np.abs(ys) < g.H2 * 0.9))[0]
     patches = []
     s = inside[0]                                     # a patch holding a star
-    patches.append((int((xs[s] - g.x0_1) / g.h1) - 64, int((ys[s] - g.x0_2) / g.h2) - 64))
+    patches.append((int((xs[s] - g.x0_1) / g.h1) - P // 2, int((ys[s] - g.x0_2) / g.h2) - P // 2))
     patches.append((0, 0))                            # window corner
-    patches.append((g.n1 - 128, g.n2 - 128))
-    for _ in range(5):
-        patches.append((int(rng.integers(0, g.n1 - 128)), int(rng.integers(0, g.n2 - 128))))
-    for (pi, pj) in patches:
-        pi, pj = max(0, min(pi, g.n1 - 128)), max(0, min(pj, g.n2 - 128))
-        sub = (pi, pi + 128, pj, pj + 128)
+    patches.append((g.n1 - P, g.n2 - P))
+    while len(patches) < npatch:
+        patches.append((int(rng.integers(0, g.n1 - P)), int(rng.integers(0, g.n2 - P))))
+    for (pi, pj) in patches[:npatch]:
+        pi, pj = max(0, min(pi, g.n1 - P)), max(0, min(pj, g.n2 - P))
+        sub = (pi, pi + P, pj, pj + P)
         res = gf.shoot(half, npix, k, border_mode=cfg.border_mode, border_param=cfg.border_param, sub=sub, dump=True)
         ref = orc.shoot(of, g, 0, sub=sub)
         ox, oy = orc.map_corners(of, g, *sub)
         assert np.max(np.hypot(res.dump[0] - ox, res.dump[1] - oy)) <= 1e-8
         tot = ref.sum()
-        assert np.max(np.abs(res.map - ref)) <= 1e-4 * max(ref.max(), 1e-300) + 1e-12, (pi, pj)
-        assert res.map.sum() == pytest.approx(tot, rel=1e-6, abs=1e-12)
+        # floor: the fixed-point quantum (2^-36 of a triangle's weight, DESIGN.md R-fix) times the triangles of the
+        # patch -- a triangle far larger than the map (config 3: 1e10 pixels) gives each pixel less than one quantum
+        quantum = 2.0 * P * P * g.weight * 2.0 ** -36
+        assert np.max(np.abs(res.map - ref)) <= 1e-4 * max(ref.max(), 1e-300) + quantum, (pi, pj)
+        # a walked triangle conserves its total exactly, but the part of it that falls inside the map is known
+        # to one quantum per map row and column it spans
+        assert res.map.sum() == pytest.approx(tot, rel=1e-6, abs=quantum * (npix + npix))
+        assert res.stats["n_queue_overflow"] == 0
 
 
 def test_closed_forms_on_gpu(ml, orc):
