@@ -17,7 +17,8 @@
  *     HOST pointers when MLENS_PTR_HOST (then the call copies host<->device itself and synchronises).
  *     Inputs are copied at create time, never aliased.
  *   - all work is enqueued on the cudaStream_t passed as `stream` (void*, NULL = default stream).
- *     Calls that return scalars to the host (create, grid_info, stats) synchronise that stream.
+ *     Calls that return scalars to the host (create, grid_info, stats) synchronise that stream; an IPM
+ *     shoot also waits on it between row bands (it sizes each band from the counters of the one before).
  *   - there is NO CPU fallback: without a CUDA device every compute call fails with MLENS_ECUDA.
  *   - maps are row-major double[npix2][npix1], row index = x2 (y2) ascending, i.e. map[iy*npix1+ix];
  *     a pixel owns its lower edges (floor rule).  IPM maps are in magnification units (an identity

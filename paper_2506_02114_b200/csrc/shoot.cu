@@ -536,7 +536,22 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_ipm, shoot_ipm_kernel, SHOOT_WARPS * 32, smem_ipm));
     ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_irs, shoot_irs_kernel, SHOOT_WARPS * 32, smem_irs));
     if (bps_ipm < 1 || bps_irs < 1) { set_error("shooting kernels do not fit on this device"); return MLENS_ECUDA; }
+    // IPM: the band height follows the rate at which the map's cells produce general triangles (they must fit the
+    // queue of one band): the first band assumes the worst case of two per cell, later ones use the measured
+    // rate of the bands before.  The host reads two counters after each band's shooting kernel, while the
+    // apportioning kernels of that band are already queued behind it.
+    const long long nwarps_res = (long long)nsm * (ipm ? bps_ipm : bps_irs) * SHOOT_WARPS;
+    const double cap_entries = ipm ? fmax(0.0, 0.8 * (double)qcap - (double)nwarps_res) * (double)QCHUNK * 0.85 : 0.0;
+    double rate = -1.0;                                            // general triangles per cell, measured
+    const bool adapt = env_ll("MLENS_BAND_FIXED", 0) == 0;          // MLENS_BAND_FIXED=1: always MLENS_BAND_CELLS (tests)
+    unsigned long long q_before = 0;
     for (long long r0 = 0; r0 < nty; r0 += rows_per_band, ++bands) {
+        if (ipm && adapt) {
+            double cells = (rate < 0.0) ? 0.5 * cap_entries : cap_entries / fmax(rate, 1e-3);
+            if (cells > (double)band_cells) cells = (double)band_cells;
+            rows_per_band = (long long)(cells / (double)(ntx * stepx * stepy));
+            if (rows_per_band < 1) rows_per_band = 1;
+        }
         S.tile_row0 = r0;
         S.tile_rows = (nty - r0 < rows_per_band) ? (nty - r0) : rows_per_band;
         long long nt = ntx * S.tile_rows;
@@ -549,6 +564,16 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         if (ipm) {
             ML_LAUNCH(shoot_ipm_kernel, grid, SHOOT_WARPS * 32, smem_ipm, s, S);
             ML_TRY(mark());
+            if (adapt && r0 + rows_per_band < nty) {             // feedback for the next band's height
+                unsigned long long h3[3] = {0, 0, 0};                 // queued, (walked), overflowed: cumulative
+                ML_CUDA(cudaMemcpyAsync(h3, f->counters.p + C_QUEUED, 24, cudaMemcpyDeviceToHost, s));
+                ML_CUDA(cudaStreamSynchronize(s));
+                const unsigned long long hq = h3[0] + h3[2];
+                const double cells_done = (double)S.tile_rows * (double)(ntx * stepx * stepy);
+                const double r_new = (double)(hq - q_before) / fmax(cells_done, 1.0);
+                q_before = hq;
+                rate = (rate < 0.0) ? 1.25 * r_new : fmax(1.25 * r_new, 0.7 * rate);   // head-room; forget slowly
+            }
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
             ML_LAUNCH(walk_kernel, nsm * 8, 256, 0, s, S);
             ML_TRY(mark());

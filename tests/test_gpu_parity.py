@@ -364,10 +364,10 @@ def test_apportioning_paths_agree(ml, orc):
     with _with_env(MLENS_SMALL_PX=1):
         walk = gf.shoot(cfg.half_y, 96, 2.0, **kw)
     assert walk.stats["n_tri_walked"] > base.stats["n_tri_walked"]
-    with _with_env(MLENS_QUEUE_MB=1, MLENS_BAND_CELLS=1 << 30):
+    with _with_env(MLENS_QUEUE_MB=1, MLENS_BAND_CELLS=1 << 30, MLENS_BAND_FIXED=1):
         over = gf.shoot(cfg.half_y, 96, 2.0, **kw)
     assert over.stats["n_queue_overflow"] > 0
-    with _with_env(MLENS_BAND_CELLS=1):
+    with _with_env(MLENS_BAND_CELLS=1, MLENS_BAND_FIXED=1):
         bands = gf.shoot(cfg.half_y, 96, 2.0, **kw)
     assert bands.stats["n_bands"] > 10
     for name, r in (("clip", clip), ("walk", walk), ("overflow", over), ("bands", bands)):
