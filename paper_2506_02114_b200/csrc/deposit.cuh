@@ -71,7 +71,8 @@ __device__ __forceinline__ int floor_to_int(double u) {
 }
 // pixel coordinates packed as two int16 (values beyond the map on one side collapse: such triangles are outside)
 __device__ __forceinline__ int pack_px(double u, double v) {
-    int a = (int)floor(fmin(fmax(u, -30000.0), 30000.0)), b = (int)floor(fmin(fmax(v, -30000.0), 30000.0));
+    // floor by the converting instruction itself (saturates for huge values, gives 0 for NaN), then clamp in integers
+    int a = max(min(__double2int_rd(u), 30000), -30000), b = max(min(__double2int_rd(v), 30000), -30000);
     if (u != u) a = -30000;
     if (v != v) b = -30000;
     return (b << 16) | (a & 0xffff);

@@ -148,7 +148,7 @@ __device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSh
     }
 }
 
-__global__ void __launch_bounds__(SHOOT_WARPS * 32) shoot_ipm_kernel(const __grid_constant__ ShootDev S) {
+__global__ void __launch_bounds__(SHOOT_WARPS * 32, 6) shoot_ipm_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpSharedIpm &Ws = reinterpret_cast<WarpSharedIpm *>(smem_raw)[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(256) walk_kernel(const __grid_constant__ Shoot
 
 // ------------------------------------------------------------------------------------------------
 // IRS: rays at cell centres (reading G10), floor of a true division (O5), counts.
-__global__ void __launch_bounds__(SHOOT_WARPS * 32) shoot_irs_kernel(const __grid_constant__ ShootDev S) {
+__global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpShared &Ws = reinterpret_cast<WarpShared *>(smem_raw)[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
