@@ -102,14 +102,15 @@ __device__ __forceinline__ double frac_below(double d0, double d1, double d2) {
     return lone_neg ? f : 1.0 - f;
 }
 
-// ---- warp ring buffers of pending work (entries of NW doubles, capacity 64, always < 32 pending before a push)
+// ---- warp ring buffers of pending work (entries of NW doubles, capacity MASK + 1; strips: always < 32 pending
+// before a push of at most 31; fallback triangles: always 0 pending before a push)
 struct Ring { int head = 0, count = 0; };
 
-template <int NW>
+template <int NW, int MASK>
 __device__ __forceinline__ void ring_push(Ring &R, double (*buf)[NW], bool pred, const double (&v)[NW]) {
     const unsigned m = __ballot_sync(0xffffffffu, pred);
     if (pred) {
-        int pos = (R.head + R.count + __popc(m & ((1u << (threadIdx.x & 31)) - 1u))) & 63;
+        int pos = (R.head + R.count + __popc(m & ((1u << (threadIdx.x & 31)) - 1u))) & MASK;
 #pragma unroll
         for (int k = 0; k < NW; ++k) buf[pos][k] = v[k];
     }
@@ -447,13 +448,13 @@ static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w
     Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
     int done = 0;
     __syncwarp();
-    unsigned big = apportion_batch<true>(*Sp, W, Wsp->rec, &Wsp->ringE[0][0], head, 63, n, done);
+    unsigned big = apportion_batch<true>(*Sp, W, Wsp->rec, &Wsp->ringE[0][0], head, 31, n, done);
     while (big) {
         const int i = __ffs(big) - 1;
         big &= big - 1;
         double v[QENT];
 #pragma unroll
-        for (int k = 0; k < QENT; ++k) v[k] = Wsp->ringE[(head + i) & 63][k];
+        for (int k = 0; k < QENT; ++k) v[k] = Wsp->ringE[(head + i) & 31][k];
         walk_triangle(*Sp, v, &Wsp->rec[0][0]);
     }
     return done;

@@ -49,11 +49,11 @@ __device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, War
         if (lane < n) { ++tc.small_; tc.px_small += 2; }
         P.S2.head = (P.S2.head + n) & 63; P.S2.count -= n;
     }
-    while (P.E.count >= keep) {
-        const int n = min(P.E.count, 32);
+    while (P.E.count > 0) {                                     // only when the global queue is full: cleared at once, 8 at a time
+        const int n = min(P.E.count, 8);
         tc.px_small += tri_batch(&S, W.w32, W.ax, W.ay, &Ws, P.E.head, n);
         if (lane < n) ++tc.small_;
-        P.E.head = (P.E.head + n) & 63; P.E.count -= n;
+        P.E.head = (P.E.head + n) & 31; P.E.count -= n;
     }
 }
 
@@ -78,7 +78,7 @@ __device__ __forceinline__ void queue_push(const ShootDev &S, WarpSharedIpm &Ws,
     }
     if (P.chunk < 0) {                                          // queue full
         if (pred) ++tc.overflow;
-        ring_push<6>(P.E, Ws.ringE, pred, e);
+        ring_push<6, 31>(P.E, Ws.ringE, pred, e);
         return;
     }
     if (pred) {
@@ -142,13 +142,13 @@ __device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSh
             double s4[4];
             s4[0] = (ay ? e[1] : e[0]) - line; s4[1] = (ay ? e[3] : e[2]) - line; s4[2] = (ay ? e[5] : e[4]) - line;
             s4[3] = __hiloint2double((mny << 16) | (mnx & 0xffff), (ay ? 1 : 0) | (A2 == 0.0 ? 2 : 0));
-            ring_push<4>(P.S2, Ws.ringS, strip, s4);
+            ring_push<4, 63>(P.S2, Ws.ringS, strip, s4);
         }
         run_batches(S, W, Ws, P, 32, tc);
     }
 }
 
-__global__ void __launch_bounds__(SHOOT_WARPS * 32, 6) shoot_ipm_kernel(const __grid_constant__ ShootDev S) {
+__global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpSharedIpm &Ws = reinterpret_cast<WarpSharedIpm *>(smem_raw)[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;

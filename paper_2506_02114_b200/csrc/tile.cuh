@@ -19,7 +19,7 @@ static const int RPT = 4;             // rays a lane evaluates together (indepen
 static const int NGRP = TCY / RPT;
 static const int TQMAX = 15;          // highest order of the tile series
 static const int NSLOT = 2;           // leaves a tile keeps a series for (rays in further leaves go through the tree)
-static const int WX = 32, WY = 16;    // per-warp shared-memory pixel window
+static const int WX = 32, WY = 8;     // per-warp shared-memory pixel window
 static const int FOLDJ = WX * WY * 8 / (32 * 16);   // series terms per pass of the star folding (scratch = the window)
 static const int BN = 2 * ML_P1MAX;   // stride of the Pascal triangle
 
@@ -68,9 +68,9 @@ struct WarpShared {
 };
 // ... plus what the IPM kernel needs for apportioning
 struct WarpSharedIpm : WarpShared {
-    double ringE[64][6];                                     // pending general triangles the global queue could not take
+    double ringE[32][6];                                     // general triangles the global queue could not take (cleared at once)
     double ringS[64][4];                                     // pending two-pixel strips
-    double rec[32][10];                                      // per-triangle records of the batch being apportioned
+    double rec[8][10];                                       // per-triangle records of the (cold) in-kernel apportioning, 8 at a time
     double stu[RPT + 1][32], stv[RPT + 1][32];               // mapped corners of the row group in pixel units (row 0 = last row of the previous group)
     int stp[RPT + 1][32];                                    // their packed pixels
 };
