@@ -61,6 +61,7 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--maps", default="", help="also time whole maps of these configs, e.g. 0,2,3,4 (create, IPM, IRS wall ms)")
     return ap.parse_args()
 
 
@@ -327,6 +328,35 @@ def run_ours(args):
                 "launch_ms": dur * 1e3, "launches_per_map": n_l,
                 "share_of_step": st["ms_shoot"] * 1e-3 / sec}
 
+    maps = None
+    if args.maps and world == 1:
+        # BASELINE.json's second metric, map wall-time, on the other configurations (one warm-up, one timed run each)
+        maps = {}
+        for ci in [int(c) for c in args.maps.split(",") if c != ""]:
+            c2 = synth.get_config(ci)
+            kw2 = dict(border_mode=c2.border_mode, border_param=c2.border_param)
+            out2 = torch.zeros((c2.npix, c2.npix), dtype=torch.float64, device=dev)
+            rec = {}
+            for rep in range(2):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                f2 = ml.Field.seeded(c2.kappa_tot, c2.gamma, c2.n_stars, c2.seed, kappa_star=c2.kappa_star,
+                                     mass_law=c2.mass_law, mass_a=c2.mass_a, mass_lo=c2.mass_lo, mass_hi=c2.mass_hi)
+                e1.record(stream); e1.synchronize()
+                rec["create_ms"] = e0.elapsed_time(e1)
+                for name, mode in (("ipm", ml.MAP_IPM), ("irs", ml.MAP_IRS)):
+                    r = f2.shoot(c2.half_y, c2.npix, c2.rays_per_pixel_length, out=out2, map_mode=mode, **kw2)
+                    rec[name + "_map_ms"] = r.stats["ms_total"]
+                    rec[name + "_rays"] = r.stats["n_rays"]
+                    rec[name + "_evals_per_s"] = r.stats["n_rays"] / (r.stats["ms_total"] * 1e-3)
+                    if mode == ml.MAP_IPM:
+                        rec["queue_overflow"] = r.stats["n_queue_overflow"]
+                        rec["mean_mu"] = float(out2.mean())
+                rec["order_p"] = f2.info()["order"]
+                f2.close()
+            maps[workload_name(c2)] = rec
+            del out2
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         e, t, thr, sub = oracle_sample(cfg, (384, 384))
@@ -353,7 +383,7 @@ def run_ours(args):
             "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
                                                   "n_queue_overflow", "n_px_clipped", "n_edge_steps", "n_rays_fallback")},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline, "cpu_baseline": cpu,
+            "roofline": roofline, "cpu_baseline": cpu, "maps": maps,
         }))
     if world > 1:
         dist.destroy_process_group()

@@ -36,25 +36,29 @@ __global__ void deflect_fmm_kernel(LensDev L, long long n, const double *zx, con
     else { ox[i] = ax; oy[i] = ay; }
 }
 
-// Direct sum over all stars (eq 13): warp-tiled P2P -- every thread owns DP_R points, the block
-// streams the stars through shared memory in tiles and each star value is reused by all threads.
+// Direct sum over all stars (eq 13): warp-tiled P2P -- every thread owns one point, the block streams its
+// share of the stars through shared memory in tiles and each star value is reused by all threads.  The stars
+// are split over gridDim.y blocks (few points against many stars must still fill the GPU); each block adds its
+// Kahan-compensated partial sum to the accumulators, direct_finish_kernel turns them into the result.
 static const int DP_T = 128, DP_TILE = 256;
-__global__ void deflect_direct_kernel(LensDev L, long long n, const double *zx, const double *zy,
-                                      double *ox, double *oy, int full_lens) {
+__global__ void deflect_direct_kernel(LensDev L, long long n, const double *zx, const double *zy, long long stars_per_block,
+                                      double *accx, double *accy) {
     __shared__ double tx[DP_TILE], ty[DP_TILE], tm[DP_TILE];
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     bool act = i < n;
     double x = act ? zx[i] : 0.0, y = act ? zy[i] : 0.0;
     double sx = 0.0, sy = 0.0, cx = 0.0, cy = 0.0;         // Kahan-compensated sums
-    for (long long base = 0; base < L.n_stars; base += DP_TILE) {
+    const long long s0 = blockIdx.y * stars_per_block;
+    const long long s1 = (s0 + stars_per_block < L.n_stars) ? s0 + stars_per_block : L.n_stars;
+    for (long long base = s0; base < s1; base += DP_TILE) {
         __syncthreads();
         for (int e = threadIdx.x; e < DP_TILE; e += DP_T) {
             long long j = base + e;
-            bool v = j < L.n_stars;
+            bool v = j < s1;
             tx[e] = v ? L.sx[j] : 0.0; ty[e] = v ? L.sy[j] : 0.0; tm[e] = v ? L.sm[j] : 0.0;
         }
         __syncthreads();
-        int cnt = (int)((L.n_stars - base < DP_TILE) ? (L.n_stars - base) : DP_TILE);
+        int cnt = (int)((s1 - base < DP_TILE) ? (s1 - base) : DP_TILE);
 #pragma unroll 4
         for (int e = 0; e < cnt; ++e) {
             double dx = x - tx[e], dy = y - ty[e];
@@ -67,8 +71,14 @@ __global__ void deflect_direct_kernel(LensDev L, long long n, const double *zx, 
         }
     }
     if (!act) return;
-    double ax = L.theta2 * sx, ay = L.theta2 * sy;
-    if (full_lens) { double wx, wy; lens_w(L, x, y, ax, ay, wx, wy); ox[i] = wx; oy[i] = wy; }
+    if (gridDim.y == 1) { accx[i] = sx; accy[i] = sy; }
+    else { atomicAdd(&accx[i], sx); atomicAdd(&accy[i], sy); }
+}
+__global__ void direct_finish_kernel(LensDev L, long long n, const double *zx, const double *zy, double *ox, double *oy, int full_lens) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double ax = L.theta2 * ox[i], ay = L.theta2 * oy[i];
+    if (full_lens) { double wx, wy; lens_w(L, zx[i], zy[i], ax, ay, wx, wy); ox[i] = wx; oy[i] = wy; }
     else { ox[i] = ax; oy[i] = ay; }
 }
 
@@ -80,8 +90,27 @@ int deflect_points(const mlens_field *f, int64_t n, const double *zx, const doub
         long long blocks = (n + 127) / 128;
         ML_LAUNCH(deflect_fmm_kernel, (unsigned)blocks, 128, 0, s, L, n, zx, zy, ox_, oy_, full_lens);
     } else {
-        long long blocks = (n + DP_T - 1) / DP_T;
-        ML_LAUNCH(deflect_direct_kernel, (unsigned)blocks, DP_T, 0, s, L, n, zx, zy, ox_, oy_, full_lens);
+        long long bx = (n + DP_T - 1) / DP_T;
+        int dev = 0, nsm = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        // enough blocks for 8 per SM; a block's share of the stars is whole tiles
+        long long by = (8ll * nsm + bx - 1) / bx;
+        long long max_by = (L.n_stars + 4 * DP_TILE - 1) / (4 * DP_TILE);
+        if (by > max_by) by = max_by;
+        if (by < 1) by = 1;
+        if (by > 65535) by = 65535;
+        long long per = (L.n_stars + by - 1) / by;
+        per = (per + DP_TILE - 1) / DP_TILE * DP_TILE;
+        if (per < DP_TILE) per = DP_TILE;
+        by = (L.n_stars + per - 1) / per;
+        if (by < 1) by = 1;
+        if (by > 1) {
+            ML_CUDA(cudaMemsetAsync(ox_, 0, (size_t)n * 8, s));
+            ML_CUDA(cudaMemsetAsync(oy_, 0, (size_t)n * 8, s));
+        }
+        ML_LAUNCH(deflect_direct_kernel, dim3((unsigned)bx, (unsigned)by), DP_T, 0, s, L, n, zx, zy, per, ox_, oy_);
+        ML_LAUNCH(direct_finish_kernel, (unsigned)((n + 255) / 256), 256, 0, s, L, n, zx, zy, ox_, oy_, full_lens);
     }
     ML_CUDA(cudaGetLastError());
     return MLENS_OK;
