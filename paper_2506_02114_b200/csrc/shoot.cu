@@ -23,6 +23,7 @@ __device__ __forceinline__ void flush_counters(const ShootDev &S, ThreadCounters
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
         unsigned int x = v[k];
+#pragma unroll 1
         for (int o = 16; o; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
         if ((threadIdx.x & 31) == 0 && x) atomicAdd(&S.counters[C_SINGLE + k], (unsigned long long)x);
     }
@@ -88,6 +89,14 @@ __device__ __forceinline__ void queue_push(const ShootDev &S, WarpSharedIpm &Ws,
         ++tc.queued;
     }
     P.used += n;
+}
+
+// Optional copy of the mapped rays to the caller (tests); out of line: never part of a production run.
+static __device__ __noinline__ void dump_rays(const ShootDev *Sp, size_t d0, size_t stride, unsigned validmask, double w0x, double w0y,
+                                              double w1x, double w1y, double w2x, double w2y, double w3x, double w3y) {
+    const double wx[4] = {w0x, w1x, w2x, w3x}, wy[4] = {w0y, w1y, w2y, w3y};
+    for (int r = 0; r < 4; ++r)
+        if ((validmask >> r) & 1u) { Sp->dump1[d0 + (size_t)r * stride] = wx[r]; Sp->dump2[d0 + (size_t)r * stride] = wy[r]; }
 }
 
 // The cell row between corner rows `prev` and `cur` of the staged group: lane = cell column.
@@ -186,12 +195,15 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
                 uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.h2 * C.inv_rt;
             }
             eval_rays(S, Ws, C, x, y, ux, uy, valid, wx, wy, tc);
+            if (S.dump1) {
+                unsigned vm = 0;
+#pragma unroll
+                for (int r = 0; r < RPT; ++r) vm |= valid[r] ? (1u << r) : 0u;
+                dump_rays(&S, (size_t)(cj0 + g * RPT - S.j0) * ncx + (size_t)(ci - S.i0), (size_t)ncx, vm,
+                          wx[0], wy[0], wx[1], wy[1], wx[2], wy[2], wx[3], wy[3]);
+            }
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
-                if (valid[r] && S.dump1) {
-                    size_t d = (size_t)(cj0 + g * RPT + r - S.j0) * ncx + (size_t)(ci - S.i0);
-                    S.dump1[d] = wx[r]; S.dump2[d] = wy[r];
-                }
                 const double u = (wx[r] - S.ylo1) * S.inv_p1, v = (wy[r] - S.ylo2) * S.inv_p2;
                 Ws.stu[r + 1][lane] = u; Ws.stv[r + 1][lane] = v; Ws.stp[r + 1][lane] = pack_px(u, v);
                 if (g == 0 && r == 1) {
@@ -299,6 +311,17 @@ __global__ void __launch_bounds__(256) walk_kernel(const __grid_constant__ Shoot
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&S.counters[C_CHUNKS], (unsigned long long)nb);   // walked, all bands
 }
 
+// floor(d / p), the pixel rule of O5, exactly: the product with the rounded reciprocal is within a few ulps of
+// the quotient, so its floor is the quotient's floor unless it lies next to an integer -- only then divide
+// (out of line: an inlined IEEE division is ~30 instructions, eight of them per row group).
+static __device__ __noinline__ double floor_div_exact(double d, double p) { return floor(d / p); }
+__device__ __forceinline__ double floor_div(double d, double p, double inv_p) {
+    const double q = d * inv_p, fq = floor(q);
+    const double r = q - fq;
+    const double tol = 1.0e-9 * fmax(1.0, fabs(q));
+    return (r > tol && r < 1.0 - tol) ? fq : floor_div_exact(d, p);
+}
+
 // ------------------------------------------------------------------------------------------------
 // IRS: rays at cell centres (reading G10), floor of a true division (O5), counts.
 __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __grid_constant__ ShootDev S) {
@@ -335,13 +358,16 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __
             }
             eval_rays(S, Ws, C, x, y, ux, uy, valid, wx, wy, tc);
             double fx[RPT], fy[RPT];
+            if (S.dump1) {
+                unsigned vm = 0;
+#pragma unroll
+                for (int r = 0; r < RPT; ++r) vm |= valid[r] ? (1u << r) : 0u;
+                dump_rays(&S, (size_t)(cj0 + g * RPT - S.j0) * nrx + (size_t)(ci - S.i0), (size_t)nrx, vm,
+                          wx[0], wy[0], wx[1], wy[1], wx[2], wy[2], wx[3], wy[3]);
+            }
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
-                if (valid[r] && S.dump1) {
-                    size_t d = (size_t)(cj0 + g * RPT + r - S.j0) * nrx + (size_t)(ci - S.i0);
-                    S.dump1[d] = wx[r]; S.dump2[d] = wy[r];
-                }
-                fx[r] = floor((wx[r] - S.ylo1) / S.p1); fy[r] = floor((wy[r] - S.ylo2) / S.p2);
+                fx[r] = floor_div(wx[r] - S.ylo1, S.p1, S.inv_p1); fy[r] = floor_div(wy[r] - S.ylo2, S.p2, S.inv_p2);
             }
             if (g == 0) {
                 double cu = __shfl_sync(full, fx[0] + 0.5 * (TCY - 1) * (fx[1] - fx[0]), TCX / 2);
@@ -502,6 +528,8 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if (S.tq < 2) S.tq = 2;
     S.small_px = (int)env_ll("MLENS_SMALL_PX", 64);
     // truncation budget of the tile series: 5 % of the deflection accuracy the field was built for
+    S.rt = 0.5 * sqrt((double)((TCX - 1) * (TCX - 1)) * g->h1 * g->h1 + (double)((TCY - 1) * (TCY - 1)) * g->h2 * g->h2) * (1.0 + 1e-9);
+    S.inv_rt = 1.0 / S.rt;
     S.eps_far = 0.02 * f->eps * f->theta;
     S.eps_star = 0.03 * f->eps * f->theta / (double)ML_NEAR;
     const int stepx = ipm ? TCX - 1 : TCX, stepy = ipm ? TCY - 1 : TCY;

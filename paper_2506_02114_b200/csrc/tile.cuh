@@ -49,6 +49,7 @@ struct ShootDev {
     long long tile_row0, tile_rows;    // band of tile rows handled by this launch
     int tq;                            // order of the tile series
     double eps_far, eps_star;          // truncation budgets of the tile series (absolute, units of theta)
+    double rt, inv_rt;                 // radius of a ray tile (half its diagonal) and its reciprocal
     int small_px;                      // queued triangles whose clipped bounding box has more pixels than this are walked, not clipped
 };
 
@@ -101,11 +102,13 @@ __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &
     for (int j = lane; j < p; j += 32) W.e[j] = S.L.ecoef[(size_t)leaf * S.L.p1 + j];
     __syncwarp();
     // ---- shift of the derivative series to the tile centre: T_j = rho^j sum_m e_{j+m} C(j+m, j) zeta_t^m   (eq C7)
-    const double rho = rt / half;
-    const double zr = (C.zt_x - cx) / half, zi = (C.zt_y - cy) / half;
+    const double ih = fast_rcp(half);
+    const double rho = rt * ih;
+    const double zr = (C.zt_x - cx) * ih, zi = (C.zt_y - cy) * ih;
     double tail = 0.0;
     for (int j = lane; j < p; j += 32) {
         double ar = 0.0, ai = 0.0;
+#pragma unroll 2
         for (int m = p - 1 - j; m >= 0; --m) {
             double bc = __ldg(&S.binom[(size_t)(j + m) * BN + j]);
             double2 c = W.e[j + m];
@@ -114,6 +117,7 @@ __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &
             ar = tr; ai = ti;
         }
         double sc = 1.0;
+#pragma unroll 1
         for (int k = 0; k < j; ++k) sc *= rho;
         ar *= sc; ai *= sc;
         if (j <= Q) W.t[s][j] = make_double2(ar, ai);
@@ -133,16 +137,18 @@ __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &
             x = S.L.near_x[o]; y = S.L.near_y[o]; m = S.L.near_m[o] * S.L.theta2;
             double dx = x - C.zt_x, dy = y - C.zt_y;
             double d2 = dx * dx + dy * dy, d = sqrt(d2);
-            double r = (d > 0.0) ? rt / d : 2.0;
+            const double id = (d > 0.0) ? fast_rcp(d) : 0.0;
+            double r = (d > 0.0) ? rt * id : 2.0;
             direct = true;
             if (r < 0.5) {
                 double rq = r;
+#pragma unroll 1
                 for (int k2 = 0; k2 < Q; ++k2) rq *= r;                  // r^(Q+1)
-                double bound = (m / d) * rq / (1.0 - r);
+                double bound = (m * id) * rq * fast_rcp(1.0 - r);
                 if (bound <= S.eps_star) {
                     direct = false;
                     // conj(alpha_i) = m/(eta - d) = -(m/d) sum_j (eta/d)^j ; with eta = rt u: term_j = -(m/d)(rt/d)^j
-                    double id2 = 1.0 / d2;
+                    double id2 = id * id;
                     term = make_double2(-m * dx * id2, m * dy * id2);     // -m/d = -m conj(d)/|d|^2
                     w = make_double2(rt * dx * id2, -rt * dy * id2);      // rt/d
                 }
@@ -164,7 +170,7 @@ __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &
                 __syncwarp();
                 if (lane < FOLDJ && j0 + lane <= Q) {
                     double2 a = W.t[s][j0 + lane];
-#pragma unroll 8
+#pragma unroll 4
                     for (int kk = 0; kk < 32; ++kk) { double2 f = fold[lane * 32 + kk]; a.x += f.x; a.y += f.y; }
                     W.t[s][j0 + lane] = a;
                 }
@@ -198,10 +204,10 @@ static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShar
         __syncwarp();
         return;
     }
-    const double rt = 0.5 * sqrt((double)((TCX - 1) * (TCX - 1)) * S.h1 * S.h1 + (double)((TCY - 1) * (TCY - 1)) * S.h2 * S.h2) * (1.0 + 1e-9);
+    const double rt = S.rt;
     C.zt_x = corner_x(S, ci0) + (0.5 * (TCX - 1) + off) * S.h1;
     C.zt_y = corner_y(S, cj0) + (0.5 * (TCY - 1) + off) * S.h2;
-    C.inv_rt = 1.0 / rt;
+    C.inv_rt = S.inv_rt;
     int leaf = -1, node = -1;
     uint32_t b0x = 0, b1x = 0, b0y = 0, b1y = 0;
     if (lane < 4) {
@@ -321,6 +327,7 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
         double2 c = t[Q];
 #pragma unroll
         for (int r = 0; r < RPT; ++r) { sr[r] = c.x; si[r] = c.y; }
+#pragma unroll 1
         for (int j = Q - 1; j >= 0; --j) {
             c = t[j];
 #pragma unroll
@@ -333,6 +340,7 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
         const int nd = T.nd[0];
         tc.rays += RPT;
         tc.near_ += (unsigned int)(nd * RPT);
+#pragma unroll 1
         for (int k = 0; k < nd; ++k) {
             double X = T.sx[0][k], Y = T.sy[0][k], M = T.sm[0][k];
 #pragma unroll
