@@ -12,6 +12,7 @@
 #include "deposit.cuh"
 #include <math.h>
 #include <stdlib.h>
+#include <limits.h>
 
 namespace ml {
 
@@ -179,22 +180,22 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
 
         const long long ci = ci0 + lane;
         const bool colv = ci <= S.i1, cellv = (lane < TCX - 1) && (ci < S.i1);
+        const double x = corner_x(S, ci), ux = ((double)lane - 0.5 * (TCX - 1)) * S.dux;
 #pragma unroll 1
         for (int g = 0; g < NGRP; ++g) {
             if (cj0 + g * RPT > S.j1) break;                             // warp-uniform
             // ---- hot loop A: map RPT corner rows (eq 12)
-            double x[RPT], y[RPT], ux[RPT], uy[RPT], wx[RPT], wy[RPT];
+            double y[RPT], uy[RPT], wx[RPT], wy[RPT];
             bool valid[RPT];
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 const int row = g * RPT + r;
                 const long long cj = cj0 + row;
                 valid[r] = colv && (cj <= S.j1);
-                x[r] = corner_x(S, ci); y[r] = corner_y(S, cj);
-                ux[r] = ((double)lane - 0.5 * (TCX - 1)) * S.h1 * C.inv_rt;
-                uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.h2 * C.inv_rt;
+                y[r] = corner_y(S, cj);
+                uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.duy;
             }
-            eval_rays(S, Ws, C, x, y, ux, uy, valid, wx, wy, tc);
+            eval_rays(S, Ws, C, x, ux, y, uy, valid, wx, wy, tc);
             if (S.dump1) {
                 unsigned vm = 0;
 #pragma unroll
@@ -311,15 +312,20 @@ __global__ void __launch_bounds__(256) walk_kernel(const __grid_constant__ Shoot
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&S.counters[C_CHUNKS], (unsigned long long)nb);   // walked, all bands
 }
 
-// floor(d / p), the pixel rule of O5, exactly: the product with the rounded reciprocal is within a few ulps of
-// the quotient, so its floor is the quotient's floor unless it lies next to an integer -- only then divide
-// (out of line: an inlined IEEE division is ~30 instructions, eight of them per row group).
-static __device__ __noinline__ double floor_div_exact(double d, double p) { return floor(d / p); }
-__device__ __forceinline__ double floor_div(double d, double p, double inv_p) {
-    const double q = d * inv_p, fq = floor(q);
-    const double r = q - fq;
-    const double tol = 1.0e-9 * fmax(1.0, fabs(q));
-    return (r > tol && r < 1.0 - tol) ? fq : floor_div_exact(d, p);
+// floor(d / p), the pixel rule of O5, exactly, as an integer (saturated; NaN -> INT_MIN, outside every map): the
+// product with the rounded reciprocal is within a few ulps of the quotient, so its floor is the quotient's floor
+// unless it lies within `tol` of an integer -- only then divide (out of line: an inlined IEEE division is ~30
+// instructions, eight of them per row group).  The floor itself is the rounding mode of the conversion.
+static __device__ __noinline__ int floor_div_exact(double d, double p) {
+    const double f = floor(d / p);
+    if (!(f == f)) return INT_MIN;
+    return (f >= 2.0e9) ? INT_MAX : (f <= -2.0e9) ? INT_MIN : (int)f;
+}
+__device__ __forceinline__ int floor_div(double d, double p, double inv_p, double tol) {
+    const double q = d * inv_p;
+    const int n = __double2int_rd(q);
+    const double r = q - (double)n;                       // in [0, 1) unless the conversion saturated (or NaN)
+    return (fabs(r - 0.5) < 0.5 - tol) ? n : floor_div_exact(d, p);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -343,21 +349,22 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __
         const long long ci1 = min(ci0 + TCX, S.i1) - 1, cj1 = min(cj0 + TCY, S.j1) - 1;      // last cell of the tile
         wtile_setup(S, Ws, C, ci0, cj0, ci1, cj1, 0.5);
         const long long ci = ci0 + lane;
+        const double x = corner_x(S, ci) + 0.5 * S.h1, ux = ((double)lane - 0.5 * (TCX - 1)) * S.dux;
+#pragma unroll 1
         for (int g = 0; g < NGRP; ++g) {
             if (cj0 + g * RPT >= S.j1) break;
-            double x[RPT], y[RPT], ux[RPT], uy[RPT], wx[RPT], wy[RPT];
+            double y[RPT], uy[RPT], wx[RPT], wy[RPT];
             bool valid[RPT];
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 const int row = g * RPT + r;
                 const long long cj = cj0 + row;
                 valid[r] = (ci < S.i1) && (cj < S.j1);
-                x[r] = corner_x(S, ci) + 0.5 * S.h1; y[r] = corner_y(S, cj) + 0.5 * S.h2;
-                ux[r] = ((double)lane - 0.5 * (TCX - 1)) * S.h1 * C.inv_rt;
-                uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.h2 * C.inv_rt;
+                y[r] = corner_y(S, cj) + 0.5 * S.h2;
+                uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.duy;
             }
-            eval_rays(S, Ws, C, x, y, ux, uy, valid, wx, wy, tc);
-            double fx[RPT], fy[RPT];
+            eval_rays(S, Ws, C, x, ux, y, uy, valid, wx, wy, tc);
+            int fx[RPT], fy[RPT];
             if (S.dump1) {
                 unsigned vm = 0;
 #pragma unroll
@@ -367,18 +374,21 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __
             }
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
-                fx[r] = floor_div(wx[r] - S.ylo1, S.p1, S.inv_p1); fy[r] = floor_div(wy[r] - S.ylo2, S.p2, S.inv_p2);
+                fx[r] = floor_div(wx[r] - S.ylo1, S.p1, S.inv_p1, S.fd_tol); fy[r] = floor_div(wy[r] - S.ylo2, S.p2, S.inv_p2, S.fd_tol);
             }
             if (g == 0) {
-                double cu = __shfl_sync(full, fx[0] + 0.5 * (TCY - 1) * (fx[1] - fx[0]), TCX / 2);
-                double cv = __shfl_sync(full, fy[0] + 0.5 * (TCY - 1) * (fy[1] - fy[0]), TCX / 2);
-                W.ax = floor_to_int(cu) - WX / 2; W.ay = floor_to_int(cv) - WY / 2;
+                // window anchor: the tile centre extrapolated from its first two rows (any anchor is correct)
+                const int ax0 = max(min(fx[0], 40000), -40000), ax1 = max(min(fx[1], 40000), -40000);
+                const int ay0 = max(min(fy[0], 40000), -40000), ay1 = max(min(fy[1], 40000), -40000);
+                const int cu = __shfl_sync(full, ax0 + ((TCY - 1) * (ax1 - ax0)) / 2, TCX / 2);
+                const int cv = __shfl_sync(full, ay0 + ((TCY - 1) * (ay1 - ay0)) / 2, TCX / 2);
+                W.ax = cu - WX / 2; W.ay = cv - WY / 2;
             }
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 int key = -1;
-                if (valid[r] && fx[r] >= 0.0 && fx[r] < (double)S.npix1 && fy[r] >= 0.0 && fy[r] < (double)S.npix2) {
-                    key = ((int)fy[r] << 16) | (int)fx[r];
+                if (valid[r] && (unsigned)fx[r] < (unsigned)S.npix1 && (unsigned)fy[r] < (unsigned)S.npix2) {
+                    key = (fy[r] << 16) | fx[r];
                     ++tc.single;
                 }
                 // runs of equal pixels among consecutive lanes become one add
@@ -527,9 +537,12 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if (S.tq > TQMAX) S.tq = TQMAX;
     if (S.tq < 2) S.tq = 2;
     S.small_px = (int)env_ll("MLENS_SMALL_PX", 64);
+    S.fd_tol = 1.0e-9 * (double)((d->npix1 > d->npix2) ? d->npix1 : d->npix2);
     // truncation budget of the tile series: 5 % of the deflection accuracy the field was built for
     S.rt = 0.5 * sqrt((double)((TCX - 1) * (TCX - 1)) * g->h1 * g->h1 + (double)((TCY - 1) * (TCY - 1)) * g->h2 * g->h2) * (1.0 + 1e-9);
     S.inv_rt = 1.0 / S.rt;
+    S.dux = g->h1 * S.inv_rt; S.duy = g->h2 * S.inv_rt;
+    S.a1_lin = S.L.one_minus_kappa + S.L.gamma + S.L.kappa_star; S.a2_lin = S.L.one_minus_kappa - S.L.gamma + S.L.kappa_star;
     S.eps_far = 0.02 * f->eps * f->theta;
     S.eps_star = 0.03 * f->eps * f->theta / (double)ML_NEAR;
     const int stepx = ipm ? TCX - 1 : TCX, stepy = ipm ? TCY - 1 : TCY;

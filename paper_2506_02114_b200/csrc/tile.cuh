@@ -50,6 +50,9 @@ struct ShootDev {
     int tq;                            // order of the tile series
     double eps_far, eps_star;          // truncation budgets of the tile series (absolute, units of theta)
     double rt, inv_rt;                 // radius of a ray tile (half its diagonal) and its reciprocal
+    double a1_lin, a2_lin;             // inside the star disc w = (a1 x - Re alpha_star, a2 y - Im alpha_star): a = 1 - kappa +- gamma + kappa_star
+    double dux, duy;                   // cell size over tile radius: step of the tile series' argument per ray
+    double fd_tol;                     // IRS: quotients closer than this to an integer are divided exactly
     int small_px;                      // queued triangles whose clipped bounding box has more pixels than this are walked, not clipped
 };
 
@@ -80,6 +83,7 @@ static_assert(FOLDJ >= 4 && ML_NEAR == 32, "fold scratch must fit the window");
 struct TileCtx {                       // warp-uniform registers
     double zt_x, zt_y, inv_rt;
     bool fast;                         // the whole tile sits in one leaf whose tile series passed its bound
+    bool lin;                          // the whole tile lies inside the star disc: the sheet term of eq 19 is -kappa_star z
 };
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -244,14 +248,21 @@ static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShar
         if (lane == 0 && W.mode[s] == 1 && full_counter) atomicAdd(full_counter, 1ull);
     }
     zero_window(W);
-    if (lane == 0) { W.ctx[0] = C.zt_x; W.ctx[1] = C.zt_y; W.ctx[2] = C.inv_rt; W.ctx[3] = (one_leaf && W.mode[0] == 0) ? 1.0 : 0.0; }
+    // eq 19 inside the disc is linear in z: the farthest ray of the tile decides (the disc is convex)
+    const double rmax = sqrt(C.zt_x * C.zt_x + C.zt_y * C.zt_y) + rt;
+    const bool lin = S.L.shape == MLENS_SHAPE_DISC && rmax * rmax <= S.L.R2;
+    if (lane == 0) {
+        W.ctx[0] = C.zt_x; W.ctx[1] = C.zt_y; W.ctx[2] = C.inv_rt;
+        W.ctx[3] = ((one_leaf && W.mode[0] == 0) ? 1.0 : 0.0) + (lin ? 2.0 : 0.0);
+    }
     __syncwarp();
 }
 // Sets up the warp's tile (out of line: once per 1024 rays) and returns its context in registers.
 __device__ __forceinline__ void wtile_setup(const ShootDev &S, WarpShared &W, TileCtx &C, long long ci0, long long cj0,
                                             long long ci1, long long cj1, double off) {
     wtile_setup_ool(&S, &W, ci0, cj0, ci1, cj1, off);
-    C.zt_x = W.ctx[0]; C.zt_y = W.ctx[1]; C.inv_rt = W.ctx[2]; C.fast = W.ctx[3] != 0.0;
+    const int flags = (int)W.ctx[3];
+    C.zt_x = W.ctx[0]; C.zt_y = W.ctx[1]; C.inv_rt = W.ctx[2]; C.fast = (flags & 1) != 0; C.lin = (flags & 2) != 0;
 }
 
 struct ThreadCounters { unsigned int single = 0, small_ = 0, queued = 0, chunks = 0, overflow = 0, fallback = 0, rays = 0, near_ = 0, px_small = 0; };
@@ -312,9 +323,16 @@ static __device__ __noinline__ void eval_group_ool(const ShootDev *Sp, const War
     }
 }
 
-// w(z) of eq 12 for the RPT rays of one lane (same column, consecutive rows).
-__device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T, const TileCtx &C, const double (&x)[RPT],
-                                          const double (&y)[RPT], const double (&ux)[RPT], const double (&uy)[RPT],
+// The full eq 12 from alpha_star where the sheet term is not linear (outside the disc, rectangle): out of line.
+static __device__ __noinline__ double2 lens_w_ool(const LensDev *L, double x, double y, double ax, double ay) {
+    double wx, wy;
+    lens_w(*L, x, y, ax, ay, wx, wy);
+    return make_double2(wx, wy);
+}
+
+// w(z) of eq 12 for the RPT rays of one lane (same column x, consecutive rows).
+__device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T, const TileCtx &C, double x, double ux,
+                                          const double (&y)[RPT], const double (&uy)[RPT],
                                           const bool (&valid)[RPT], double (&wx)[RPT], double (&wy)[RPT], ThreadCounters &tc) {
     bool all = true;
 #pragma unroll
@@ -327,13 +345,25 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
         double2 c = t[Q];
 #pragma unroll
         for (int r = 0; r < RPT; ++r) { sr[r] = c.x; si[r] = c.y; }
+        int j = Q - 1;
+        // two terms per trip: the chains ping-pong between two register sets, no copies
 #pragma unroll 1
-        for (int j = Q - 1; j >= 0; --j) {
-            c = t[j];
+        for (; j >= 1; j -= 2) {
+            const double2 c1 = t[j], c0 = t[j - 1];
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
-                double tr = fma(sr[r], ux[r], fma(-si[r], uy[r], c.x));
-                double ti = fma(sr[r], uy[r], fma(si[r], ux[r], c.y));
+                const double tr = fma(sr[r], ux, fma(-si[r], uy[r], c1.x));
+                const double ti = fma(sr[r], uy[r], fma(si[r], ux, c1.y));
+                sr[r] = fma(tr, ux, fma(-ti, uy[r], c0.x));
+                si[r] = fma(tr, uy[r], fma(ti, ux, c0.y));
+            }
+        }
+        if (j == 0) {
+            c = t[0];
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                const double tr = fma(sr[r], ux, fma(-si[r], uy[r], c.x));
+                const double ti = fma(sr[r], uy[r], fma(si[r], ux, c.y));
                 sr[r] = tr; si[r] = ti;
             }
         }
@@ -343,24 +373,33 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
 #pragma unroll 1
         for (int k = 0; k < nd; ++k) {
             double X = T.sx[0][k], Y = T.sy[0][k], M = T.sm[0][k];
+            const double dx = x - X;
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
-                double dx = x[r] - X, dy = y[r] - Y;
+                double dy = y[r] - Y;
                 double r2 = fma(dx, dx, dy * dy);
                 double q = (__double2hiint(r2) >= 0x00100000) ? M * fast_rcp(r2) : 0.0;   // reading G11: skip r = 0
                 sr[r] = fma(q, dx, sr[r]);
                 si[r] = fma(-q, dy, si[r]);
             }
         }
+        if (C.lin) {
 #pragma unroll
-        for (int r = 0; r < RPT; ++r) lens_w(S.L, x[r], y[r], sr[r], -si[r], wx[r], wy[r]);
+            for (int r = 0; r < RPT; ++r) { wx[r] = fma(S.a1_lin, x, -sr[r]); wy[r] = fma(S.a2_lin, y[r], si[r]); }
+        } else {
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                const double2 w = lens_w_ool(&S.L, x, y[r], sr[r], -si[r]);
+                wx[r] = w.x; wy[r] = w.y;
+            }
+        }
     } else {
         double w[2 * RPT];
         int cnt[3] = {0, 0, 0};
         unsigned vm = 0;
 #pragma unroll
         for (int r = 0; r < RPT; ++r) vm |= valid[r] ? (1u << r) : 0u;
-        eval_group_ool(&S, &T, x[0], ux[0], y[0], y[1], y[2], y[3], uy[0], uy[1] - uy[0], vm, w, cnt);
+        eval_group_ool(&S, &T, x, ux, y[0], y[1], y[2], y[3], uy[0], uy[1] - uy[0], vm, w, cnt);
         tc.rays += cnt[0]; tc.near_ += cnt[1]; tc.fallback += cnt[2];
 #pragma unroll
         for (int r = 0; r < RPT; ++r) { wx[r] = w[2 * r]; wy[r] = w[2 * r + 1]; }
