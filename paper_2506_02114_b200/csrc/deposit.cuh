@@ -216,14 +216,19 @@ __device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, 
     // at most one grid line of the other axis lies strictly between os and oe
     const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
     const bool cross = (od != 0.0) && ((oe > os) ? (gl < oe) : (gl > oe)) && (oe != os);
+    double mg = me, og = oe;                                   // where the first piece ends
     if (cross) {
         const double tg = fmin(fmax((gl - oc0) * oid, ts), te);
-        const double mg = fma(tg, d, c0);
-        if (E.majorY) { piece_deposit(S, os, ms, gl, mg, cs, bx, by); piece_deposit(S, gl, mg, oe, me, cs, bx, by); }
-        else { piece_deposit(S, ms, os, mg, gl, cs, bx, by); piece_deposit(S, mg, gl, me, oe, cs, bx, by); }
-    } else {
-        if (E.majorY) piece_deposit(S, os, ms, oe, me, cs, bx, by);
-        else piece_deposit(S, ms, os, me, oe, cs, bx, by);
+        mg = fma(tg, d, c0); og = gl;
+    }
+    // one copy of the deposit for all lanes, whatever their axis: first piece, then the second of those that cross
+    const bool my = E.majorY != 0;
+    double xs = my ? os : ms, ys = my ? ms : os, xe = my ? og : mg, ye = my ? mg : og;
+#pragma unroll 1
+    for (int pc = 0; pc < 2; ++pc) {
+        piece_deposit(S, xs, ys, xe, ye, cs, bx, by);
+        if (!cross) break;
+        xs = xe; ys = ye; xe = my ? oe : me; ye = my ? me : oe;
     }
 }
 
