@@ -77,6 +77,12 @@ __device__ __forceinline__ int pack_px(double u, double v) {
     if (v != v) b = -30000;
     return (b << 16) | (a & 0xffff);
 }
+// ... and the sides of the map the pixel lies beyond (Cohen-Sutherland code): a triangle whose three codes share a
+// bit cannot touch the map
+__device__ __forceinline__ int out_code(int pk, int npix1, int npix2) {
+    const int a = (int)(short)(pk & 0xffff), b = pk >> 16;
+    return (a < 0 ? 1 : 0) | (a >= npix1 ? 2 : 0) | (b < 0 ? 4 : 0) | (b >= npix2 ? 8 : 0);
+}
 __device__ __forceinline__ int px_of(int pk) { return (int)(short)(pk & 0xffff); }
 __device__ __forceinline__ int py_of(int pk) { return pk >> 16; }
 
@@ -115,26 +121,6 @@ __device__ __forceinline__ void ring_push(Ring &R, double (*buf)[NW], bool pred,
         for (int k = 0; k < NW; ++k) buf[pos][k] = v[k];
     }
     R.count += __popc(m);
-}
-
-// ---- two-pixel strips: entry = signed distances of the vertices from the pixel line, pixel, axis.
-// Out of line (one copy in the instruction cache); lanes [0, n) take one pending entry each.
-static __device__ __noinline__ void strip2_batch(const ShootDev *Sp, unsigned int *w32, int ax, int ay, const double (*ring)[4], int head, int n) {
-    const ShootDev &S = *Sp;
-    const int lane = threadIdx.x & 31;
-    Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
-    __syncwarp();
-    if (lane < n) {
-        const double *q = ring[(head + lane) & 63];
-        const double d0 = q[0], d1 = q[1], d2 = q[2];
-        const int code = __double2loint(q[3]), pk = __double2hiint(q[3]);     // code: bit 0 = axis (1: pixels stacked in y), bit 1 = degenerate
-        const int px = px_of(pk), py = py_of(pk);
-        const unsigned long long a = (code & 2) ? ((d0 < 0.0) ? FIX_ONE : 0ull) : to_fix(frac_below(d0, d1, d2));
-#pragma unroll 1
-        for (int k = 0; k < 2; ++k)                             // rolled: one copy of the add in the instruction stream
-            pix_add(S, W, px + ((code & 1) ? 0 : k), py + ((code & 1) ? k : 0), k ? FIX_ONE - a : a);
-    }
-    __syncwarp();
 }
 
 // ---- the edge walk ------------------------------------------------------------------------------------------

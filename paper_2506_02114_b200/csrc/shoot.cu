@@ -37,21 +37,15 @@ __device__ __forceinline__ long long fetch_tile(const ShootDev &S) {
 }
 
 struct Pend {
-    Ring E, S2;                        // E: only what the global queue could not take
+    Ring E;                            // only what the global queue could not take
     long long chunk = -1;              // queue chunk this warp is filling
     int used = 0;
 };
 
-// Runs the pending-work rings down to fewer than `keep` entries (keep = 32 inside a tile, 1 at the end).
-__device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, int keep, ThreadCounters &tc) {
+// Clears the fallback ring (only ever filled when the global queue is full), 8 triangles at a time.
+__device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, ThreadCounters &tc) {
     const int lane = threadIdx.x & 31;
-    while (P.S2.count >= keep) {
-        const int n = min(P.S2.count, 32);
-        strip2_batch(&S, W.w32, W.ax, W.ay, Ws.ringS, P.S2.head, n);
-        if (lane < n) { ++tc.small_; tc.px_small += 2; }
-        P.S2.head = (P.S2.head + n) & 63; P.S2.count -= n;
-    }
-    while (P.E.count > 0) {                                     // only when the global queue is full: cleared at once, 8 at a time
+    while (P.E.count > 0) {
         const int n = min(P.E.count, 8);
         tc.px_small += tri_batch(&S, W.w32, W.ax, W.ay, &Ws, P.E.head, n);
         if (lane < n) ++tc.small_;
@@ -100,23 +94,23 @@ static __device__ __noinline__ void dump_rays(const ShootDev *Sp, size_t d0, siz
         if ((validmask >> r) & 1u) { Sp->dump1[d0 + (size_t)r * stride] = wx[r]; Sp->dump2[d0 + (size_t)r * stride] = wy[r]; }
 }
 
-// The cell row between corner rows `prev` and `cur` of the staged group: lane = cell column.
-//   a = (prev, lane), b = (prev, lane+1), c = (cur, lane+1), d = (cur, lane);  T1 = a, b, c;  T2 = a, c, d  (reading G9)
-// Triangles inside one pixel are run-length merged and added at once; two-pixel strips and general triangles
-// are pushed onto the warp's rings and apportioned 32 at a time.
-__device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, int prev, int cur, bool cellv,
+// The cell row between corner rows `prev` and `prev + 1` of the staged group: lane = cell column.
+//   a = (prev, lane), b = (prev, lane+1), c = (prev+1, lane+1), d = (prev+1, lane);  T1 = a, b, c;  T2 = a, c, d  (reading G9)
+// Triangles inside one pixel are run-length merged and added at once.  All others that can touch the map only
+// leave their name (row, column, which) in the warp's list: process_pending apportions them 32 at a time at the
+// end of the row group, every lane busy, from the corners still staged in shared memory.
+__device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, int &npend, int prev, bool cellv,
                                          ThreadCounters &tc) {
     const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31, l1 = min(lane + 1, 31);
+    const int lane = threadIdx.x & 31, l1 = min(lane + 1, 31), cur = prev + 1;
     const int pa = Ws.stp[prev][lane], pb = Ws.stp[prev][l1], pc = Ws.stp[cur][l1], pd = Ws.stp[cur][lane];
+    const int oa = Ws.sto[prev][lane], ob = Ws.sto[prev][l1], oc = Ws.sto[cur][l1], od = Ws.sto[cur][lane];
     const bool t1 = (pa == pb) && (pa == pc), t2 = (pa == pc) && (pa == pd);
     {
         // single-pixel triangles: equal pixels in consecutive lanes become one deposit
-        const int xa = px_of(pa), ya = py_of(pa);
-        const bool inmap = (unsigned)xa < (unsigned)S.npix1 && (unsigned)ya < (unsigned)S.npix2;
         const int ns = cellv ? (int)t1 + (int)t2 : 0;
         tc.single += ns;
-        const int key = (ns > 0 && inmap) ? pa : -1;
+        const int key = (ns > 0 && oa == 0) ? pa : -1;
         const int kprev = __shfl_up_sync(full, key, 1);
         const bool head = (lane == 0) || (key != kprev);
         const unsigned heads = __ballot_sync(full, head);
@@ -126,36 +120,54 @@ __device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSh
             const int next = above ? (__ffs(above) - 1) : 32;
             const unsigned run = ((next == 32) ? 0xffffffffu : ((1u << next) - 1u)) & ~((1u << lane) - 1u);
             const unsigned long long n = 2ull * __popc(two & run) + __popc(one & run);
-            pix_add(S, W, xa, ya, n << FIXBITS);
+            pix_add(S, W, px_of(pa), py_of(pa), n << FIXBITS);
         }
     }
+    const bool act1 = cellv && !t1 && !(oa & ob & oc), act2 = cellv && !t2 && !(oa & oc & od);
+    const unsigned b1 = __ballot_sync(full, act1), b2 = __ballot_sync(full, act2);
+    const unsigned lt = (1u << lane) - 1u;
+    const int n1 = __popc(b1), idb = (prev << 6) | (lane << 1);
+    if (act1) Ws.ids[npend + __popc(b1 & lt)] = idb;
+    if (act2) Ws.ids[npend + n1 + __popc(b2 & lt)] = idb | 1;
+    npend += n1 + __popc(b2);
+}
+
+// Apportions the `count` listed triangles of the row group, 32 at a time.  A triangle over two adjacent pixels is
+// split in closed form (the fraction of its area beyond the pixel line is the product of two edge ratios); any
+// other goes to the global queue.
+__device__ __forceinline__ void process_pending(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, int count, ThreadCounters &tc) {
+    const int lane = threadIdx.x & 31;
+    __syncwarp();
 #pragma unroll 1
-    for (int tt = 0; tt < 2; ++tt) {
-        const int p2 = tt ? pc : pb, p3 = tt ? pd : pc;
+    for (int h0 = 0; h0 < count; h0 += 32) {
+        const bool have = h0 + lane < count;
+        const int id = have ? Ws.ids[h0 + lane] : 0;
+        const int tt = id & 1, c = (id >> 1) & 31, r = id >> 6, c1 = min(c + 1, 31);
+        const int r2 = tt ? r + 1 : r, c3 = tt ? c : c1;                 // vertices (r, c), (r2, c1), (r + 1, c3)
+        const int pa = Ws.stp[r][c], p2 = Ws.stp[r2][c1], p3 = Ws.stp[r + 1][c3];
+        double e[6];
+        e[0] = Ws.stu[r][c]; e[1] = Ws.stv[r][c];
+        e[2] = Ws.stu[r2][c1]; e[3] = Ws.stv[r2][c1];
+        e[4] = Ws.stu[r + 1][c3]; e[5] = Ws.stv[r + 1][c3];
         const int x1 = px_of(pa), x2 = px_of(p2), x3 = px_of(p3), y1 = py_of(pa), y2 = py_of(p2), y3 = py_of(p3);
         const int mnx = min(x1, min(x2, x3)), mxx = max(x1, max(x2, x3)), mny = min(y1, min(y2, y3)), mxy = max(y1, max(y2, y3));
-        const bool act = cellv && !(tt ? t2 : t1) && !(mxx < 0 || mxy < 0 || mnx >= S.npix1 || mny >= S.npix2);
         const int w = mxx - mnx, h = mxy - mny;
-        const bool strip = act && (w + h == 1);
-        double e[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-        if (act) {
-            const int r2 = tt ? cur : prev, c2 = l1, r3 = cur, c3 = tt ? lane : l1;
-            e[0] = Ws.stu[prev][lane]; e[1] = Ws.stv[prev][lane];
-            e[2] = Ws.stu[r2][c2]; e[3] = Ws.stv[r2][c2];
-            e[4] = Ws.stu[r3][c3]; e[5] = Ws.stv[r3][c3];
-        }
-        queue_push(S, Ws, P, act && !strip, e, tc);
-        {
+        const bool strip = have && (w + h == 1);
+        queue_push(S, Ws, P, have && !strip, e, tc);
+        if (strip) {
             const bool ay = (h == 1);                                        // pixels stacked in y
             const double line = ay ? (double)(mny + 1) : (double)(mnx + 1);
             const double A2 = (e[2] - e[0]) * (e[5] - e[1]) - (e[4] - e[0]) * (e[3] - e[1]);
-            double s4[4];
-            s4[0] = (ay ? e[1] : e[0]) - line; s4[1] = (ay ? e[3] : e[2]) - line; s4[2] = (ay ? e[5] : e[4]) - line;
-            s4[3] = __hiloint2double((mny << 16) | (mnx & 0xffff), (ay ? 1 : 0) | (A2 == 0.0 ? 2 : 0));
-            ring_push<4, 63>(P.S2, Ws.ringS, strip, s4);
+            const double d0 = (ay ? e[1] : e[0]) - line, d1 = (ay ? e[3] : e[2]) - line, d2 = (ay ? e[5] : e[4]) - line;
+            const unsigned long long a = (A2 == 0.0) ? ((d0 < 0.0) ? FIX_ONE : 0ull) : to_fix(frac_below(d0, d1, d2));
+#pragma unroll 1
+            for (int k = 0; k < 2; ++k)                             // rolled: one copy of the add in the instruction stream
+                pix_add(S, W, mnx + (ay ? 0 : k), mny + (ay ? k : 0), k ? FIX_ONE - a : a);
+            ++tc.small_; tc.px_small += 2;
         }
-        run_batches(S, W, Ws, P, 32, tc);
+        run_batches(S, W, Ws, P, tc);
     }
+    __syncwarp();
 }
 
 __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __grid_constant__ ShootDev S) {
@@ -169,6 +181,7 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
     Win W; W.w32 = reinterpret_cast<unsigned int *>(Ws.win); W.ax = 0; W.ay = 0;
     const long long ntiles = (long long)S.ntx * S.tile_rows;
     const long long ncx = S.i1 - S.i0 + 1;               // corners per dump row
+    int npend = 0;
 
     for (long long tile = fetch_tile(S); tile < ntiles;) {
         const long long tile_next = fetch_tile(S);       // the hand-out latency hides behind this tile's work
@@ -206,7 +219,8 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 const double u = (wx[r] - S.ylo1) * S.inv_p1, v = (wy[r] - S.ylo2) * S.inv_p2;
-                Ws.stu[r + 1][lane] = u; Ws.stv[r + 1][lane] = v; Ws.stp[r + 1][lane] = pack_px(u, v);
+                const int pk = pack_px(u, v);
+                Ws.stu[r + 1][lane] = u; Ws.stv[r + 1][lane] = v; Ws.stp[r + 1][lane] = pk; Ws.sto[r + 1][lane] = out_code(pk, S.npix1, S.npix2);
                 if (g == 0 && r == 1) {
                     // window anchor: the tile centre extrapolated from its first two rows (any anchor is correct)
                     const double u0 = Ws.stu[1][lane], v0 = Ws.stv[1][lane];
@@ -220,19 +234,18 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
 #pragma unroll 1
             for (int r = (g == 0) ? 1 : 0; r < RPT; ++r) {
                 if (cj0 + g * RPT + r > S.j1) break;                     // warp-uniform
-                cell_row(S, W, Ws, P, r, r + 1, cellv, tc);
+                cell_row(S, W, Ws, npend, r, cellv, tc);
             }
-            __syncwarp();
+            process_pending(S, W, Ws, P, npend, tc);
+            npend = 0;
             Ws.stu[0][lane] = Ws.stu[RPT][lane]; Ws.stv[0][lane] = Ws.stv[RPT][lane]; Ws.stp[0][lane] = Ws.stp[RPT][lane];
+            Ws.sto[0][lane] = Ws.sto[RPT][lane];
             __syncwarp();
         }
         flush_window(S, Ws, W);
         __syncwarp();
         tile = tile_next;
     }
-    // pending work of the last tiles goes straight to the map
-    W.w32 = nullptr;
-    run_batches(S, W, Ws, P, 1, tc);
     if (lane == 0 && P.chunk >= 0) S.qcount[P.chunk] = P.used;
     flush_counters(S, tc);
 }

@@ -73,10 +73,11 @@ struct WarpShared {
 // ... plus what the IPM kernel needs for apportioning
 struct WarpSharedIpm : WarpShared {
     double ringE[32][6];                                     // general triangles the global queue could not take (cleared at once)
-    double ringS[64][4];                                     // pending two-pixel strips
+    int ids[256];                                            // triangles of the row group that are not singles: (corner row, column, which of the two)
     double rec[8][10];                                       // per-triangle records of the (cold) in-kernel apportioning, 8 at a time
     double stu[RPT + 1][32], stv[RPT + 1][32];               // mapped corners of the row group in pixel units (row 0 = last row of the previous group)
     int stp[RPT + 1][32];                                    // their packed pixels
+    int sto[RPT + 1][32];                                    // and on which sides of the map they lie (0: inside)
 };
 static_assert(FOLDJ >= 4 && ML_NEAR == 32, "fold scratch must fit the window");
 
