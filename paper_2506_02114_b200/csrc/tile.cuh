@@ -324,6 +324,19 @@ static __device__ __noinline__ void eval_group_ool(const ShootDev *Sp, const War
     }
 }
 
+// Slot of the tile that holds both (x, ya) and (x, yb) -- hence every ray of the column between them, a leaf being
+// a box -- with a tile series that passed its bound; -1 if there is none.  Only tiles that straddle leaves ask.
+static __device__ __noinline__ int slot_of_column(const ShootDev *Sp, const WarpShared *T, double x, double ya, double yb) {
+    uint32_t qx, qa, qb, qx2;
+    if (!quantise(Sp->L, x, ya, qx, qa) || !quantise(Sp->L, x, yb, qx2, qb)) return -1;
+    int s = -1;
+#pragma unroll 1
+    for (int k = 0; k < NSLOT; ++k)
+        if (T->leaf[k] >= 0 && T->mode[k] == 0 && qx >= T->bx0[k] && qx < T->bx1[k] && qa >= T->by0[k] && qa < T->by1[k] &&
+            qb >= T->by0[k] && qb < T->by1[k]) s = k;
+    return s;
+}
+
 // The full eq 12 from alpha_star where the sheet term is not linear (outside the disc, rectangle): out of line.
 static __device__ __noinline__ double2 lens_w_ool(const LensDev *L, double x, double y, double ax, double ay) {
     double wx, wy;
@@ -338,10 +351,18 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
     bool all = true;
 #pragma unroll
     for (int r = 0; r < RPT; ++r) all = all && valid[r];
-    if (C.fast && all) {
-        // the common case: the whole tile in one leaf, RPT independent Horner chains share every coefficient load
+    int s = 0;
+    bool fastlane = C.fast && all;
+    if (!C.fast && all && S.eval_mode == MLENS_EVAL_FMM) {
+        // a tile over two leaves: the lanes whose four rays share a leaf still take the fast path, each with its slot
+        s = slot_of_column(&S, &T, x, y[0], y[RPT - 1]);
+        fastlane = s >= 0;
+        s = max(s, 0);
+    }
+    if (fastlane) {
+        // the common case: the four rays in one leaf, RPT independent Horner chains share every coefficient load
         const int Q = S.tq;
-        const double2 *t = T.t[0];
+        const double2 *t = T.t[s];
         double sr[RPT], si[RPT];
         double2 c = t[Q];
 #pragma unroll
@@ -368,12 +389,12 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
                 sr[r] = tr; si[r] = ti;
             }
         }
-        const int nd = T.nd[0];
+        const int nd = T.nd[s];
         tc.rays += RPT;
         tc.near_ += (unsigned int)(nd * RPT);
 #pragma unroll 1
         for (int k = 0; k < nd; ++k) {
-            double X = T.sx[0][k], Y = T.sy[0][k], M = T.sm[0][k];
+            double X = T.sx[s][k], Y = T.sy[s][k], M = T.sm[s][k];
             const double dx = x - X;
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
