@@ -301,25 +301,108 @@ __global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_co
     if (lane == 0 && n_clipped) atomicAdd(&S.counters[C_PX_INT], (unsigned long long)n_clipped);
 }
 
-// Edge walk of the large triangles the drain set aside: one warp per triangle, handed out one at a time.
-__global__ void __launch_bounds__(256) walk_kernel(const __grid_constant__ ShootDev S) {
-    __shared__ double scratch_s[8][48];
-    double *scratch = scratch_s[threadIdx.x >> 5];
+// Edge walk of the large triangles the drain set aside.  A warp takes WB triangles at a time: lane = triangle
+// for the local frame, lane = edge for the clipped edges (records in shared memory); then the steps of all the
+// edges form one index space the lanes stride over, so the set-up is shared by a whole batch and a triangle
+// of a few dozen steps costs a few dozen lane-steps.  The next batch is fetched while this one is walked.
+static const int WALK_WARPS = 8;
+static const int WB = 16;              // triangles per batch
+static const int EREC = 10;            // doubles per edge record
+__global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_constant__ ShootDev S) {
+    __shared__ double er_s[WALK_WARPS][3 * WB][EREC];
+    __shared__ double tr_s[WALK_WARPS][WB][8];           // local vertices, cs, (bx, by)
+    double (*er)[EREC] = er_s[threadIdx.x >> 5];
+    double (*tr)[8] = tr_s[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     long long nb = (long long)S.counters[C_BIG];
     if (nb > S.big_cap) nb = S.big_cap;
+    const long long nbatch = (nb + WB - 1) / WB;
+    Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
     unsigned long long n_pieces = 0;
-    while (true) {
-        long long i = 0;
-        if (lane == 0) i = (long long)atomicAdd(&S.counters[C_WALK], 1ull);
-        i = __shfl_sync(full, i, 0);
-        if (i >= nb) break;
-        const double *e = S.queue + (size_t)S.biglist[i] * QENT;
-        double v[QENT];
+    long long b = 0;
+    if (lane == 0) b = (long long)atomicAdd(&S.counters[C_WALK], 1ull);
+    b = __shfl_sync(full, b, 0);
+    while (b < nbatch) {
+        long long bnext = 0;
+        if (lane == 0) bnext = (long long)atomicAdd(&S.counters[C_WALK], 1ull);
+        // ---- lane = triangle: local frame
+        const long long it = b + (long long)lane * nbatch;      // strided: the giant triangles of one star's tiles sit next to each other in the list
+        int status = 0;
+        double ry0 = 0.0, ry1 = 0.0, cx1 = 0.0;
+        if (lane < WB && it < nb) {
+            const double *e = S.queue + (size_t)S.biglist[it] * QENT;
+            double v[QENT];
 #pragma unroll
-        for (int k = 0; k < QENT; ++k) v[k] = __ldg(&e[k]);
-        n_pieces += walk_triangle(S, v, scratch);
+            for (int k = 0; k < QENT; ++k) v[k] = __ldg(&e[k]);
+            TriSetup T;
+            tri_setup(S, W, v, T);                                  // a degenerate triangle deposits here (reading G12)
+            status = T.status;
+            if (status == 1) {
+                double *q = tr[lane];
+                q[0] = T.x[0]; q[1] = T.y[0]; q[2] = T.x[1]; q[3] = T.y[1]; q[4] = T.x[2]; q[5] = T.y[2];
+                q[6] = T.cs; q[7] = __hiloint2double(T.by, T.bx);
+                ry0 = T.ry0; ry1 = T.ry1; cx1 = T.cx1;
+            }
+        }
+        __syncwarp();
+        // ---- lane = edge (3 WB of them, two passes)
+#pragma unroll
+        for (int ps = 0; ps < 2; ++ps) {
+            const int ed = ps * 32 + lane, ti = ed / 3, e = ed - 3 * ti, tis = min(ti, WB - 1);
+            const int st = __shfl_sync(full, status, tis);
+            const double r0 = __shfl_sync(full, ry0, tis), r1 = __shfl_sync(full, ry1, tis), c1 = __shfl_sync(full, cx1, tis);
+            if (ed < 3 * WB) {
+                EdgeWalk E;
+                E.n = 0; E.majorY = 1; E.sg = 1.0;
+                double *q = er[ed];
+                if (st == 1) {
+                    const int e1 = (e == 2) ? 0 : e + 1;
+                    const double *t = tr[ti];
+                    edge_setup(E, t[2 * e], t[2 * e + 1], t[2 * e1], t[2 * e1 + 1], r0, r1, c1);
+                    q[0] = E.x0; q[1] = E.y0; q[2] = E.x1; q[3] = E.y1; q[4] = E.idx; q[5] = E.idy; q[6] = E.ta; q[7] = E.tb; q[8] = E.g0;
+                }
+                q[9] = __hiloint2double(E.n, E.majorY | (E.sg < 0.0 ? 2 : 0));
+
+            }
+        }
+        __syncwarp();
+        // steps per triangle (lane < WB) and their inclusive prefix
+        int ntot = 0;
+        if (lane < WB) ntot = __double2hiint(er[3 * lane][9]) + __double2hiint(er[3 * lane + 1][9]) + __double2hiint(er[3 * lane + 2][9]);
+        int inc = ntot;
+#pragma unroll
+        for (int o = 1; o < WB; o <<= 1) { int t = __shfl_up_sync(full, inc, o); if (lane >= o) inc += t; }
+        const int total = __shfl_sync(full, inc, WB - 1);
+#pragma unroll 1
+        for (int k0 = 0; k0 < total; k0 += 32) {
+            const int k = k0 + lane;
+            int i = 0;                                              // first triangle whose inclusive prefix exceeds k
+#pragma unroll
+            for (int step = WB / 2; step; step >>= 1) {
+                int v = __shfl_sync(full, inc, i + step - 1);
+                if (v <= k) i += step;
+            }
+            i = min(i, WB - 1);
+            const int incl = __shfl_sync(full, inc, i), cnt = __shfl_sync(full, ntot, i);
+            if (k < total) {
+                int m = k - (incl - cnt);
+                const int n0 = __double2hiint(er[3 * i][9]), n1 = __double2hiint(er[3 * i + 1][9]);
+                const int e = (m >= n0 + n1) ? 2 : (m >= n0 ? 1 : 0);
+                m -= (e == 2) ? n0 + n1 : (e == 1 ? n0 : 0);
+                const double *q = er[3 * i + e];
+                EdgeWalk E;
+                E.x0 = q[0]; E.y0 = q[1]; E.x1 = q[2]; E.y1 = q[3]; E.dx = E.x1 - E.x0; E.dy = E.y1 - E.y0;
+                E.idx = q[4]; E.idy = q[5]; E.ta = q[6]; E.tb = q[7]; E.g0 = q[8];
+                const int fl = __double2loint(q[9]);
+                E.majorY = fl & 1; E.sg = (fl & 2) ? -1.0 : 1.0; E.n = __double2hiint(q[9]);
+                const double pk = tr[i][7];
+                edge_step(S, E, m, tr[i][6], __double2loint(pk), __double2hiint(pk));
+            }
+        }
+        __syncwarp();
+        n_pieces += (unsigned long long)total;
+        b = __shfl_sync(full, bnext, 0);
     }
     if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&S.counters[C_CHUNKS], (unsigned long long)nb);   // walked, all bands
@@ -629,7 +712,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
                 rate = (rate < 0.0) ? 1.25 * r_new : fmax(1.25 * r_new, 0.7 * rate);   // head-room; forget slowly
             }
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
-            ML_LAUNCH(walk_kernel, nsm * 8, 256, 0, s, S);
+            ML_LAUNCH(walk_kernel, nsm * 4, WALK_WARPS * 32, 0, s, S);
             ML_TRY(mark());
             launches += 3;
         } else {
