@@ -612,11 +612,27 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if (ipm) {
         ML_TRY(f->diff.reserve((size_t)npix, s, false));
         ML_CUDA(cudaMemsetAsync(f->diff.p, 0, (size_t)npix * 8, s));
-        long long qmb = env_ll("MLENS_QUEUE_MB", 2048);
-        qcap = qmb * (1ll << 20) / (QCHUNK * QENT * 8);              // chunks
-        ML_TRY(f->queue.reserve((size_t)qcap * QCHUNK * QENT, s, false));
-        ML_TRY(f->qcount.reserve((size_t)qcap, s, false));
-        ML_TRY(f->biglist.reserve((size_t)qcap * QCHUNK / 4, s, false));
+        // Queue of general triangles: every band ends with the tails of three kernels, so bands should be few and
+        // the queue large -- 8 GiB unless the device is small, never more than the worst case of this map (two
+        // triangles per cell); halved until it can be had.  MLENS_QUEUE_MB overrides.
+        size_t mem_free = 0, mem_total = 0;
+        cudaMemGetInfo(&mem_free, &mem_total);
+        long long qmb = 8192;
+        if (mem_total > 0 && (long long)(mem_total >> 24) < qmb) qmb = (long long)(mem_total >> 24);   // <= 1/16 of the device
+        const double need_mb = 3.2 * (double)(i1 - i0) * (double)(j1 - j0) * (QENT * 8) / 1048576.0 + 64.0;
+        if ((double)qmb > need_mb) qmb = (long long)need_mb;
+        const long long qmb_env = env_ll("MLENS_QUEUE_MB", 0);
+        if (qmb_env > 0) qmb = qmb_env;
+        for (;;) {
+            qcap = qmb * (1ll << 20) / (QCHUNK * QENT * 8);          // chunks
+            int rc = f->queue.reserve((size_t)qcap * QCHUNK * QENT, s, false);
+            if (rc == MLENS_OK) rc = f->qcount.reserve((size_t)qcap, s, false);
+            if (rc == MLENS_OK) rc = f->biglist.reserve((size_t)qcap * QCHUNK / 4, s, false);
+            if (rc == MLENS_OK) break;
+            if (rc != MLENS_ENOMEM || qmb_env > 0 || qmb <= 256) return rc;
+            cudaGetLastError();
+            qmb /= 2;
+        }
     }
     ShootDev S;
     S.L = make_lens_dev(f);
@@ -648,7 +664,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 27);
+    long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 30);
     long long rows_per_band = band_cells / (ntx * stepx * stepy);
     if (rows_per_band < 1) rows_per_band = 1;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
