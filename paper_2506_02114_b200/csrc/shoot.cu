@@ -667,6 +667,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 30);
     long long rows_per_band = band_cells / (ntx * stepx * stepy);
     if (rows_per_band < 1) rows_per_band = 1;
+    if (!ipm && env_ll("MLENS_BAND_FIXED", 0) == 0) rows_per_band = nty;      // IRS has no queue to bound: one launch
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     const bool timed = st && (d->sync || d->ptr_kind == MLENS_PTR_HOST);
     if (timed) { ML_CUDA(cudaEventCreate(&e0)); ML_CUDA(cudaEventCreate(&e1)); ML_CUDA(cudaEventRecord(e0, s)); }

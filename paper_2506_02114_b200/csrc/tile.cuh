@@ -167,17 +167,22 @@ __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &
         }
         if (k == 0) { W.nd[s] = __popc(dm); W.mode[s] = (tail <= S.eps_far) ? 0 : 1; }
         if (fm) {
-            // FOLDJ series terms per pass: lane = star writes its terms, lane = term sums over the stars
+            // FOLDJ series terms per pass: lane = star writes its terms, then the warp sums them over the stars
             for (int j0 = 0; j0 <= Q; j0 += FOLDJ) {
                 __syncwarp();
 #pragma unroll
                 for (int j = 0; j < FOLDJ; ++j) { fold[j * 32 + k] = term; term = cmul(term, w); }
                 __syncwarp();
-                if (lane < FOLDJ && j0 + lane <= Q) {
-                    double2 a = W.t[s][j0 + lane];
-#pragma unroll 4
-                    for (int kk = 0; kk < 32; ++kk) { double2 f = fold[lane * 32 + kk]; a.x += f.x; a.y += f.y; }
-                    W.t[s][j0 + lane] = a;
+                {
+                    // lane = (term jj, eighth q): four stars each, then the eighths are summed by shuffles
+                    static_assert(FOLDJ == 4, "32 lanes = 4 terms x 8");
+                    const int jj = lane >> 3, q = lane & 7;
+                    double2 a = fold[jj * 32 + q];
+#pragma unroll
+                    for (int kk = 1; kk < 4; ++kk) { double2 f = fold[jj * 32 + kk * 8 + q]; a.x += f.x; a.y += f.y; }
+#pragma unroll
+                    for (int o = 1; o < 8; o <<= 1) { a.x += __shfl_xor_sync(full, a.x, o); a.y += __shfl_xor_sync(full, a.y, o); }
+                    if (q == 0 && j0 + jj <= Q) { double2 t0 = W.t[s][j0 + jj]; W.t[s][j0 + jj] = make_double2(t0.x + a.x, t0.y + a.y); }
                 }
             }
         }
