@@ -48,8 +48,8 @@ UNIT = "evals/s"
 # by mlens_bench_dfma in the same run is reported beside it as `peak_measured_dfma`.
 FP64_LANES_PER_SM = 64
 # dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/r01b_ncu_full.md: dram read + write of shoot_ipm_kernel, mean of the two captured launches).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 515.0e6
+# (profiles/r01c_ncu_full.md: dram read + write of shoot_ipm_kernel, mean of the two launches of a map).
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.43e9
 
 
 def parse():
@@ -266,11 +266,13 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item()) * 1e-3
 
-    for _ in range(max(args.warmup, 3)):
-        step_device()
+    # the sampler starts before the warm-up: nvidia-smi takes ~0.5 s to come up, and its start-up inside the timed
+    # region (a few hundred ms in all) stalls the host round trips of create; it keeps sampling through the timed steps
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        step_device()
     l0 = ml.launch_count()
     sec = timed(step_device, args.steps)
     launches = (ml.launch_count() - l0) // args.steps

@@ -124,6 +124,11 @@ int deflect_points(const mlens_field *f, int64_t n, const double *zx, const doub
 int generate_stars(uint64_t seed, int64_t n, int shape, double a1, double a2, int mass_law, double a,
                    double lo, double hi, double *x, double *y, double *m, cudaStream_t s);
 // shoot.cu
+// The general-triangle queue is gigabytes of scratch that belongs to no field in particular: a destroyed field
+// parks it here (after the device has been synchronised) and the next field that shoots on that device takes it,
+// so that creating and destroying fields in a loop never allocates it again.
+void scratch_park(mlens_field *f);
+void scratch_take(mlens_field *f);
 int geometry(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid *g);
 int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double *map,
           unsigned long long *counts, mlens_stats *st, cudaStream_t s);

@@ -13,6 +13,7 @@
 #include <math.h>
 #include <stdlib.h>
 #include <limits.h>
+#include <mutex>
 
 namespace ml {
 
@@ -590,6 +591,27 @@ int geometry(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid *g) {
 }
 
 
+namespace {
+struct ParkedScratch { DevBuf<double> queue; DevBuf<int> qcount; DevBuf<unsigned int> biglist; int device = -1; };
+ParkedScratch g_parked;
+std::mutex g_parked_mutex;
+}  // namespace
+
+void scratch_park(mlens_field *f) {
+    std::lock_guard<std::mutex> lock(g_parked_mutex);
+    if (!f->queue.p || f->queue.cap <= g_parked.queue.cap) return;              // the larger one is kept
+    g_parked.queue.release(); g_parked.qcount.release(); g_parked.biglist.release();
+    g_parked.queue = f->queue; g_parked.qcount = f->qcount; g_parked.biglist = f->biglist; g_parked.device = f->device;
+    f->queue = DevBuf<double>(); f->qcount = DevBuf<int>(); f->biglist = DevBuf<unsigned int>();
+}
+
+void scratch_take(mlens_field *f) {
+    std::lock_guard<std::mutex> lock(g_parked_mutex);
+    if (f->queue.p || !g_parked.queue.p || g_parked.device != f->device) return;
+    f->queue = g_parked.queue; f->qcount = g_parked.qcount; f->biglist = g_parked.biglist;
+    g_parked.queue = DevBuf<double>(); g_parked.qcount = DevBuf<int>(); g_parked.biglist = DevBuf<unsigned int>();
+}
+
 static long long env_ll(const char *name, long long dflt) {
     const char *v = getenv(name);
     if (!v || !*v) return dflt;
@@ -623,6 +645,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         if ((double)qmb > need_mb) qmb = (long long)need_mb;
         const long long qmb_env = env_ll("MLENS_QUEUE_MB", 0);
         if (qmb_env > 0) qmb = qmb_env;
+        scratch_take(f);
         for (;;) {
             qcap = qmb * (1ll << 20) / (QCHUNK * QENT * 8);          // chunks
             int rc = f->queue.reserve((size_t)qcap * QCHUNK * QENT, s, false);
@@ -648,7 +671,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     S.tq = (int)env_ll("MLENS_TILE_ORDER", 12);
     if (S.tq > TQMAX) S.tq = TQMAX;
     if (S.tq < 2) S.tq = 2;
-    S.small_px = (int)env_ll("MLENS_SMALL_PX", 64);
+    S.small_px = (int)env_ll("MLENS_SMALL_PX", 24);
     S.fd_tol = 1.0e-9 * (double)((d->npix1 > d->npix2) ? d->npix1 : d->npix2);
     // truncation budget of the tile series: 5 % of the deflection accuracy the field was built for
     S.rt = 0.5 * sqrt((double)((TCX - 1) * (TCX - 1)) * g->h1 * g->h1 + (double)((TCY - 1) * (TCY - 1)) * g->h2 * g->h2) * (1.0 + 1e-9);
