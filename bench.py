@@ -351,7 +351,12 @@ def run_ours(args):
                     rec[name + "_map_ms"] = r.stats["ms_total"]
                     rec[name + "_rays"] = r.stats["n_rays"]
                     rec[name + "_evals_per_s"] = r.stats["n_rays"] / (r.stats["ms_total"] * 1e-3)
+                    rec[name + "_shoot_ms"] = r.stats["ms_shoot"]
                     if mode == ml.MAP_IPM:
+                        rec["ipm_drain_walk_ms"] = r.stats["ms_drain"]
+                        rec["ipm_bands"] = r.stats["n_bands"]
+                        rec["tri"] = {k: r.stats[k] for k in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
+                                                              "n_px_clipped", "n_edge_steps")}
                         rec["queue_overflow"] = r.stats["n_queue_overflow"]
                         rec["mean_mu"] = float(out2.mean())
                 rec["order_p"] = f2.info()["order"]

@@ -123,6 +123,11 @@ __device__ __forceinline__ void ring_push(Ring &R, double (*buf)[NW], bool pred,
     R.count += __popc(m);
 }
 
+// min / max by one compare and one select (fmin / fmax also order NaNs: a dozen instructions each on FP64)
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }     // operands are never NaN here
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
+__device__ __forceinline__ double clamp01(double v) { return dmin(dmax(v, 0.0), 1.0); }
+
 // ---- the edge walk ------------------------------------------------------------------------------------------
 // An edge is walked along its MAJOR axis: between two consecutive grid lines of that axis it stays inside one
 // row (or column) of pixels and, its slope being <= 1, crosses at most one grid line of the other axis -- so a
@@ -175,7 +180,7 @@ __device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, doub
     long long r = tcov;                                        // left of the map: the whole cover enters at column 0
     int c0 = 0;
     if (ic >= 0) {
-        const double m = fmin(fmax(xm - fi, 0.0), 1.0);
+        const double m = clamp01(xm - fi);
         r = __double2ll_rn((double)tcov * m);
         c0 = ic + 1;
         diff_add(S, ic, jr, (unsigned long long)(tcov - r));
@@ -192,30 +197,26 @@ __device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, 
     // start and end in (major, other) coordinates
     double ms, os, me, oe, ts, te;
     if (k == 0) { ts = E.ta; ms = (ts == 0.0) ? c0 : fma(ts, d, c0); os = (ts == 0.0) ? oc0 : fma(ts, od, oc0); }
-    else { ms = E.g0 + E.sg * (double)(k - 1); ts = fmin(fmax((ms - c0) * id, E.ta), E.tb); os = fma(ts, od, oc0); }
+    else { ms = E.g0 + E.sg * (double)(k - 1); ts = dmin(dmax((ms - c0) * id, E.ta), E.tb); os = fma(ts, od, oc0); }
     if (k == E.n - 1) {
         te = E.tb;
         const bool vtx = (te == 1.0);
         me = vtx ? (E.majorY ? E.y1 : E.x1) : fma(te, d, c0);
         oe = vtx ? (E.majorY ? E.x1 : E.y1) : fma(te, od, oc0);
-    } else { me = E.g0 + E.sg * (double)k; te = fmin(fmax((me - c0) * id, E.ta), E.tb); oe = fma(te, od, oc0); }
+    } else { me = E.g0 + E.sg * (double)k; te = dmin(dmax((me - c0) * id, E.ta), E.tb); oe = fma(te, od, oc0); }
     // at most one grid line of the other axis lies strictly between os and oe
     const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
     const bool cross = (od != 0.0) && ((oe > os) ? (gl < oe) : (gl > oe)) && (oe != os);
     double mg = me, og = oe;                                   // where the first piece ends
     if (cross) {
-        const double tg = fmin(fmax((gl - oc0) * oid, ts), te);
+        const double tg = dmin(dmax((gl - oc0) * oid, ts), te);
         mg = fma(tg, d, c0); og = gl;
     }
-    // one copy of the deposit for all lanes, whatever their axis: first piece, then the second of those that cross
+    // the axes are swapped back before the deposit, so that one copy of it serves all lanes: the first piece,
+    // then the second of those that cross
     const bool my = E.majorY != 0;
-    double xs = my ? os : ms, ys = my ? ms : os, xe = my ? og : mg, ye = my ? mg : og;
-#pragma unroll 1
-    for (int pc = 0; pc < 2; ++pc) {
-        piece_deposit(S, xs, ys, xe, ye, cs, bx, by);
-        if (!cross) break;
-        xs = xe; ys = ye; xe = my ? oe : me; ye = my ? me : oe;
-    }
+    piece_deposit(S, my ? os : ms, my ? ms : os, my ? og : mg, my ? mg : og, cs, bx, by);
+    if (cross) piece_deposit(S, my ? og : mg, my ? mg : og, my ? oe : me, my ? me : oe, cs, bx, by);
 }
 
 struct TriSetup {
@@ -230,9 +231,11 @@ struct TriSetup {
 __device__ __forceinline__ void tri_setup(const ShootDev &S, const Win &W, const double *v, TriSetup &T) {
     T.status = 0;
     const double u0 = v[0], v0 = v[1], u1 = v[2], v1 = v[3], u2 = v[4], v2 = v[5];
-    const double mnx = fmin(u0, fmin(u1, u2)), mxx = fmax(u0, fmax(u1, u2));
-    const double mny = fmin(v0, fmin(v1, v2)), mxy = fmax(v0, fmax(v1, v2));
-    if (!(mxx >= 0.0) || !(mxy >= 0.0) || !(mnx < (double)S.npix1) || !(mny < (double)S.npix2)) return;   // also NaN
+    const double nan_probe = (u0 + u1 + u2) + (v0 + v1 + v2);                    // NaN if any is (or if infinities cancel)
+    if (!(nan_probe == nan_probe)) return;
+    const double mnx = dmin(u0, dmin(u1, u2)), mxx = dmax(u0, dmax(u1, u2));
+    const double mny = dmin(v0, dmin(v1, v2)), mxy = dmax(v0, dmax(v1, v2));
+    if (!(mxx >= 0.0) || !(mxy >= 0.0) || !(mnx < (double)S.npix1) || !(mny < (double)S.npix2)) return;
     if (!(mnx > -1.0e9) || !(mny > -1.0e9) || !(mxx < 1.0e9) || !(mxy < 1.0e9)) return;                     // inf / absurd
     const double fbx = floor(mnx), fby = floor(mny);
     T.bx = (int)fbx; T.by = (int)fby;
@@ -254,9 +257,6 @@ __device__ __forceinline__ void tri_setup(const ShootDev &S, const Win &W, const
 // Sutherland-Hodgman clipping + shoelace up to rounding; no polygon arrays, no data-dependent vertex
 // counts.  Signed like the triangle.  (x, y)[3] = vertices, (idx, idy)[3] = reciprocal edge vectors (0 if the
 // component is 0), edge k runs from vertex k to vertex k+1.
-__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }     // operands are never NaN here
-__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
-__device__ __forceinline__ double clamp01(double v) { return dmin(dmax(v, 0.0), 1.0); }
 __device__ __forceinline__ double tri_pixel_area(const double (&x)[3], const double (&y)[3], const double (&idx)[3], const double (&idy)[3],
                                                  double qx, double qy) {
     double s = 0.0;
@@ -299,9 +299,10 @@ __device__ __forceinline__ unsigned apportion_batch(const ShootDev &S, const Win
     if (lane < n) {
         const double *v = ent + (size_t)((head + lane) & mask) * QENT;
         const double u0 = v[0], v0 = v[1], u1 = v[2], v1 = v[3], u2 = v[4], v2 = v[5];
-        const double mnx = fmin(u0, fmin(u1, u2)), mxx = fmax(u0, fmax(u1, u2));
-        const double mny = fmin(v0, fmin(v1, v2)), mxy = fmax(v0, fmax(v1, v2));
-        const bool sane = (mxx >= 0.0) && (mxy >= 0.0) && (mnx < (double)S.npix1) && (mny < (double)S.npix2) &&
+        const double nan_probe = (u0 + u1 + u2) + (v0 + v1 + v2);                // NaN if any is (or if infinities cancel)
+        const double mnx = dmin(u0, dmin(u1, u2)), mxx = dmax(u0, dmax(u1, u2));
+        const double mny = dmin(v0, dmin(v1, v2)), mxy = dmax(v0, dmax(v1, v2));
+        const bool sane = (nan_probe == nan_probe) && (mxx >= 0.0) && (mxy >= 0.0) && (mnx < (double)S.npix1) && (mny < (double)S.npix2) &&
                           (mnx > -1.0e9) && (mny > -1.0e9) && (mxx < 1.0e9) && (mxy < 1.0e9);      // false for NaN too
         if (sane) {
             const double fbx = floor(mnx), fby = floor(mny);
