@@ -260,6 +260,8 @@ def run_ours(args):
             e1.record(stream)
             e1.synchronize()
             total_ms += e0.elapsed_time(e1)
+            if os.environ.get("MLENS_BENCH_VERBOSE"):
+                print(f"step {fn.__name__}: {e0.elapsed_time(e1):.2f} ms", file=sys.stderr)
         barrier()
         t = torch.tensor([total_ms / steps], dtype=torch.float64, device=dev)
         if world > 1:
