@@ -332,6 +332,27 @@ def run_ours(args):
                 "launch_ms": dur * 1e3, "launches_per_map": n_l,
                 "share_of_step": st["ms_shoot"] * 1e-3 / sec}
 
+    # the single-precision evaluator on the same workload, beside the float64 numbers
+    f32 = None
+    if world == 1:
+        ff = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, seed, kappa_star=cfg.kappa_star,
+                             mass_law=cfg.mass_law, mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
+        out32 = torch.zeros((npix, npix), dtype=torch.float64, device=dev)
+        f32 = {}
+        for name, mode in (("ipm", ml.MAP_IPM), ("irs", ml.MAP_IRS)):
+            for _ in range(2):
+                r32 = ff.shoot(half, npix, k, out=out32, map_mode=mode, eval_mode=ml.EVAL_FMM_F32, **kw)
+            f32[name + "_map_ms"] = r32.stats["ms_total"]
+            f32[name + "_shoot_ms"] = r32.stats["ms_shoot"]
+            ref64 = map_ipm if mode == ml.MAP_IPM else map_irs
+            sel = ref64 >= 0.1
+            rel = ((out32 - ref64).abs()[sel] / ref64[sel])
+            f32[name + "_pixels_beyond_1e-3_of_f64"] = float((rel > 1e-3).double().mean())
+            f32[name + "_median_rel_dev_of_f64"] = float(rel.median())
+        f32["f64_ipm_shoot_ms"] = state["ipm"]["ms_shoot"]; f32["f64_irs_shoot_ms"] = state["irs"]["ms_shoot"]
+        ff.close()
+        del out32
+
     maps = None
     if args.maps and world == 1:
         # BASELINE.json's second metric, map wall-time, on the other configurations (one warm-up, one timed run each)
@@ -392,7 +413,7 @@ def run_ours(args):
             "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
                                                   "n_queue_overflow", "n_px_clipped", "n_edge_steps", "n_rays_fallback")},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline, "cpu_baseline": cpu, "maps": maps,
+            "roofline": roofline, "cpu_baseline": cpu, "f32_mode": f32, "maps": maps,
         }))
     if world > 1:
         dist.destroy_process_group()

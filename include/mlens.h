@@ -42,7 +42,11 @@ enum { MLENS_OK = 0, MLENS_EINVAL = -1, MLENS_ENOMEM = -2, MLENS_ECUDA = -3,
 enum { MLENS_PTR_DEVICE = 0, MLENS_PTR_HOST = 1 };
 enum { MLENS_SHAPE_DISC = 0, MLENS_SHAPE_RECT = 1 };          /* star-region shape */
 enum { MLENS_MASS_EQUAL = 0, MLENS_MASS_POWER = 1 };          /* dN/dm ~ m^-a on [lo,hi] / theoretical mean */
-enum { MLENS_EVAL_FMM = 0, MLENS_EVAL_DIRECT = 1 };           /* DIRECT = the paper's "no FMM" mode (Table 1) */
+enum { MLENS_EVAL_FMM = 0, MLENS_EVAL_DIRECT = 1,             /* DIRECT = the paper's "no FMM" mode (Table 1) */
+       MLENS_EVAL_FMM_F32 = 2 };  /* mlens_shoot only: the paper's single-precision mode: far-field series and
+                                     near-field stars of a ray tile in float32, relative to the tile centre; macro
+                                     terms, pixel arithmetic and accumulation stay float64.  Deflections are then
+                                     good to ~1e-7 of their magnitude (not to eps_deflection). */
 enum { MLENS_MAP_IPM = 0, MLENS_MAP_IRS = 1 };
 enum { MLENS_BORDER_EQ16 = 0,      /* dY + 10 theta sqrt(kappa_star)                      (eq 16) */
        MLENS_BORDER_A6 = 1,        /* dY + theta sqrt(kappa_star <m^2>/(f <m>)), param=f (eq A6) */
@@ -110,7 +114,7 @@ typedef struct {
     int32_t npix1, npix2;
     double rays_per_pixel_length;  /* k: cell = pixel / k (Table 1 caption) */
     int32_t map_mode;              /* MLENS_MAP_IPM / MLENS_MAP_IRS */
-    int32_t eval_mode;             /* MLENS_EVAL_FMM / MLENS_EVAL_DIRECT */
+    int32_t eval_mode;             /* MLENS_EVAL_FMM / MLENS_EVAL_DIRECT / MLENS_EVAL_FMM_F32 */
     int32_t border_mode;           /* MLENS_BORDER_* */
     int32_t accumulate;            /* 0: overwrite map/counts, 1: add to their current contents */
     double border_param, He1, He2;

@@ -326,7 +326,7 @@ int mlens_grid_info(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid 
 int mlens_shoot(mlens_field *f, const mlens_shoot_desc *d, double *map, uint64_t *counts, mlens_stats *stats, void *stream) {
     if (!f || !d) { set_error("null argument"); return MLENS_EINVAL; }
     if (d->map_mode != MLENS_MAP_IPM && d->map_mode != MLENS_MAP_IRS) { set_error("bad map mode"); return MLENS_EINVAL; }
-    if (d->eval_mode != MLENS_EVAL_FMM && d->eval_mode != MLENS_EVAL_DIRECT) { set_error("bad eval mode"); return MLENS_EINVAL; }
+    if (d->eval_mode != MLENS_EVAL_FMM && d->eval_mode != MLENS_EVAL_DIRECT && d->eval_mode != MLENS_EVAL_FMM_F32) { set_error("bad eval mode"); return MLENS_EINVAL; }
     mlens_grid g;
     ML_TRY(geometry(f, d, &g));
     cudaStream_t s = (cudaStream_t)stream;

@@ -171,6 +171,7 @@ __device__ __forceinline__ void process_pending(const ShootDev &S, const Win &W,
     __syncwarp();
 }
 
+template <bool F32>
 __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpSharedIpm &Ws = reinterpret_cast<WarpSharedIpm *>(smem_raw)[threadIdx.x >> 5];
@@ -209,7 +210,7 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
                 y[r] = corner_y(S, cj);
                 uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.duy;
             }
-            eval_rays(S, Ws, C, x, ux, y, uy, valid, wx, wy, tc);
+            eval_rays<F32>(S, Ws, C, x, ux, y, uy, valid, wx, wy, tc);
             if (S.dump1) {
                 unsigned vm = 0;
 #pragma unroll
@@ -427,6 +428,7 @@ __device__ __forceinline__ int floor_div(double d, double p, double inv_p, doubl
 
 // ------------------------------------------------------------------------------------------------
 // IRS: rays at cell centres (reading G10), floor of a true division (O5), counts.
+template <bool F32>
 __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpShared &Ws = reinterpret_cast<WarpShared *>(smem_raw)[threadIdx.x >> 5];
@@ -460,7 +462,7 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __
                 y[r] = corner_y(S, cj) + 0.5 * S.h2;
                 uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.duy;
             }
-            eval_rays(S, Ws, C, x, ux, y, uy, valid, wx, wy, tc);
+            eval_rays<F32>(S, Ws, C, x, ux, y, uy, valid, wx, wy, tc);
             int fx[RPT], fy[RPT];
             if (S.dump1) {
                 unsigned vm = 0;
@@ -667,7 +669,8 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     S.dump1 = d->dump_w1; S.dump2 = d->dump_w2;
     S.binom = f->binom.p;
     if ((S.dump1 == nullptr) != (S.dump2 == nullptr)) { set_error("dump_w1 and dump_w2 go together"); return MLENS_EINVAL; }
-    S.eval_mode = d->eval_mode;
+    const bool f32 = d->eval_mode == MLENS_EVAL_FMM_F32;       // same tiles and slow paths as FMM; only the fast path differs
+    S.eval_mode = f32 ? MLENS_EVAL_FMM : d->eval_mode;
     S.tq = (int)env_ll("MLENS_TILE_ORDER", 12);
     if (S.tq > TQMAX) S.tq = TQMAX;
     if (S.tq < 2) S.tq = 2;
@@ -705,13 +708,15 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     const size_t smem_ipm = SHOOT_WARPS * sizeof(WarpSharedIpm), smem_irs = SHOOT_WARPS * sizeof(WarpShared);
     static bool attr_set = false;
     if (!attr_set) {
-        ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
-        ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_irs));
+        ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
+        ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_irs));
+        ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
+        ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_irs));
         attr_set = true;
     }
     int bps_ipm = 1, bps_irs = 1;
-    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_ipm, shoot_ipm_kernel, SHOOT_WARPS * 32, smem_ipm));
-    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_irs, shoot_irs_kernel, SHOOT_WARPS * 32, smem_irs));
+    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_ipm, shoot_ipm_kernel<false>, SHOOT_WARPS * 32, smem_ipm));
+    ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_irs, shoot_irs_kernel<false>, SHOOT_WARPS * 32, smem_irs));
     if (bps_ipm < 1 || bps_irs < 1) { set_error("shooting kernels do not fit on this device"); return MLENS_ECUDA; }
     // IPM: the band height follows the rate at which the map's cells produce general triangles (they must fit the
     // queue of one band): the first band assumes the worst case of two per cell, later ones use the measured
@@ -739,7 +744,8 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         ML_CUDA(cudaMemsetAsync(f->counters.p + C_DRAIN, 0, 3 * 8, s));   // drain, big-list and walk counters
         ML_TRY(mark());
         if (ipm) {
-            ML_LAUNCH(shoot_ipm_kernel, grid, SHOOT_WARPS * 32, smem_ipm, s, S);
+            if (f32) ML_LAUNCH(shoot_ipm_kernel<true>, grid, SHOOT_WARPS * 32, smem_ipm, s, S);
+            else ML_LAUNCH(shoot_ipm_kernel<false>, grid, SHOOT_WARPS * 32, smem_ipm, s, S);
             ML_TRY(mark());
             if (adapt && r0 + rows_per_band < nty) {             // feedback for the next band's height
                 unsigned long long h3[3] = {0, 0, 0};                 // queued, (walked), overflowed: cumulative
@@ -756,7 +762,8 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             ML_TRY(mark());
             launches += 3;
         } else {
-            ML_LAUNCH(shoot_irs_kernel, grid, SHOOT_WARPS * 32, smem_irs, s, S);
+            if (f32) ML_LAUNCH(shoot_irs_kernel<true>, grid, SHOOT_WARPS * 32, smem_irs, s, S);
+            else ML_LAUNCH(shoot_irs_kernel<false>, grid, SHOOT_WARPS * 32, smem_irs, s, S);
             ML_TRY(mark());
             launches += 1;
         }

@@ -350,6 +350,25 @@ static __device__ __noinline__ double2 lens_w_ool(const LensDev *L, double x, do
 }
 
 // w(z) of eq 12 for the RPT rays of one lane (same column x, consecutive rows).
+// float pairs for the packed single-precision FMA of sm_100 (FFMA2)
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float lo2(unsigned long long v) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return lo; }
+__device__ __forceinline__ float hi2(unsigned long long v) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return hi; }
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+// F32 (the paper's single-precision mode; MLENS_EVAL_FMM_F32): the tile series and the tile's direct stars
+// are evaluated in float32 -- the series in the tile's own argument u, the separations from the stars taken in
+// float64 and then rounded, so that only the deflection, never a position, is rounded to 24 bits -- and the
+// macro terms in float64.
+template <bool F32>
 __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T, const TileCtx &C, double x, double ux,
                                           const double (&y)[RPT], const double (&uy)[RPT],
                                           const bool (&valid)[RPT], double (&wx)[RPT], double (&wy)[RPT], ThreadCounters &tc) {
@@ -364,7 +383,71 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
         fastlane = s >= 0;
         s = max(s, 0);
     }
-    if (fastlane) {
+    if (fastlane && F32) {
+        const int Q = S.tq;
+        const double2 *t = T.t[s];
+        const float uxf = (float)ux;
+        float uyf[RPT], sr[RPT], si[RPT];
+#pragma unroll
+        for (int r = 0; r < RPT; ++r) uyf[r] = (float)uy[r];
+        // Blackwell's packed FFMA2 (fma.rn.f32x2) does two rays per instruction: the chains of rows (0, 1) and (2, 3)
+        // travel as float pairs, eight instructions per two terms and pair instead of sixteen
+        static_assert(RPT == 4, "two ray pairs");
+        const unsigned long long UX = pack2(uxf, uxf);
+        const unsigned long long UYa = pack2(uyf[0], uyf[1]), UYb = pack2(uyf[2], uyf[3]);
+        const unsigned long long NUYa = pack2(-uyf[0], -uyf[1]), NUYb = pack2(-uyf[2], -uyf[3]);
+        double2 cd = t[Q];
+        unsigned long long sra = pack2((float)cd.x, (float)cd.x), sia = pack2((float)cd.y, (float)cd.y), srb = sra, sib = sia;
+        int j = Q - 1;
+#pragma unroll 1
+        for (; j >= 1; j -= 2) {
+            const double2 d1 = t[j], d0 = t[j - 1];
+            const float c1x = (float)d1.x, c1y = (float)d1.y, c0x = (float)d0.x, c0y = (float)d0.y;
+            const unsigned long long C1X = pack2(c1x, c1x), C1Y = pack2(c1y, c1y), C0X = pack2(c0x, c0x), C0Y = pack2(c0y, c0y);
+            const unsigned long long tra = fma2(sra, UX, fma2(sia, NUYa, C1X)), tia = fma2(sra, UYa, fma2(sia, UX, C1Y));
+            const unsigned long long trb = fma2(srb, UX, fma2(sib, NUYb, C1X)), tib = fma2(srb, UYb, fma2(sib, UX, C1Y));
+            sra = fma2(tra, UX, fma2(tia, NUYa, C0X)); sia = fma2(tra, UYa, fma2(tia, UX, C0Y));
+            srb = fma2(trb, UX, fma2(tib, NUYb, C0X)); sib = fma2(trb, UYb, fma2(tib, UX, C0Y));
+        }
+        if (j == 0) {
+            cd = t[0];
+            const float c0x = (float)cd.x, c0y = (float)cd.y;
+            const unsigned long long C0X = pack2(c0x, c0x), C0Y = pack2(c0y, c0y);
+            const unsigned long long tra = fma2(sra, UX, fma2(sia, NUYa, C0X)), tia = fma2(sra, UYa, fma2(sia, UX, C0Y));
+            const unsigned long long trb = fma2(srb, UX, fma2(sib, NUYb, C0X)), tib = fma2(srb, UYb, fma2(sib, UX, C0Y));
+            sra = tra; sia = tia; srb = trb; sib = tib;
+        }
+        sr[0] = lo2(sra); sr[1] = hi2(sra); sr[2] = lo2(srb); sr[3] = hi2(srb);
+        si[0] = lo2(sia); si[1] = hi2(sia); si[2] = lo2(sib); si[3] = hi2(sib);
+        const int nd = T.nd[s];
+        tc.rays += RPT;
+        tc.near_ += (unsigned int)(nd * RPT);
+#pragma unroll 1
+        for (int k = 0; k < nd; ++k) {
+            // the separation is taken in float64 and then rounded: a ray next to a star keeps its relative accuracy
+            const double Yd = T.sy[s][k];
+            const float M = (float)T.sm[s][k];
+            const float dx = (float)(x - T.sx[s][k]);
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                const float dy = (float)(y[r] - Yd);
+                const float r2 = fmaf(dx, dx, dy * dy);
+                const float q = (r2 > 0.0f) ? __fdividef(M, r2) : 0.0f;                   // reading G11: skip r = 0
+                sr[r] = fmaf(q, dx, sr[r]);
+                si[r] = fmaf(-q, dy, si[r]);
+            }
+        }
+        if (C.lin) {
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) { wx[r] = fma(S.a1_lin, x, -(double)sr[r]); wy[r] = fma(S.a2_lin, y[r], (double)si[r]); }
+        } else {
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                const double2 w = lens_w_ool(&S.L, x, y[r], (double)sr[r], -(double)si[r]);
+                wx[r] = w.x; wy[r] = w.y;
+            }
+        }
+    } else if (fastlane) {
         // the common case: the four rays in one leaf, RPT independent Horner chains share every coefficient load
         const int Q = S.tq;
         const double2 *t = T.t[s];

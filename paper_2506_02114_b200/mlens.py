@@ -14,7 +14,7 @@ _lib = None
 
 SHAPE_DISC, SHAPE_RECT = 0, 1
 MASS_EQUAL, MASS_POWER = 0, 1
-EVAL_FMM, EVAL_DIRECT = 0, 1
+EVAL_FMM, EVAL_DIRECT, EVAL_FMM_F32 = 0, 1, 2
 MAP_IPM, MAP_IRS = 0, 1
 BORDER_EQ16, BORDER_A6, BORDER_MARGIN, BORDER_EXPLICIT = 0, 1, 2, 3
 PTR_DEVICE, PTR_HOST = 0, 1
