@@ -429,7 +429,7 @@ __device__ __forceinline__ int floor_div(double d, double p, double inv_p, doubl
 // ------------------------------------------------------------------------------------------------
 // IRS: rays at cell centres (reading G10), floor of a true division (O5), counts.
 template <bool F32>
-__global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_irs_kernel(const __grid_constant__ ShootDev S) {
+__global__ void __launch_bounds__(SHOOT_WARPS * 32, 12) shoot_irs_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     WarpShared &Ws = reinterpret_cast<WarpShared *>(smem_raw)[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
