@@ -440,14 +440,14 @@ static __device__ __noinline__ int tri_batch(const ShootDev *Sp, unsigned int *w
     Win W; W.w32 = w32; W.ax = ax; W.ay = ay;
     int done = 0;
     __syncwarp();
-    unsigned big = apportion_batch<true>(*Sp, W, Wsp->rec, &Wsp->ringE[0][0], head, 31, n, done);
+    unsigned big = apportion_batch<true>(*Sp, W, Wsp->rec(), &Wsp->ringE[0][0], head, 7, n, done);
     while (big) {
         const int i = __ffs(big) - 1;
         big &= big - 1;
         double v[QENT];
 #pragma unroll
-        for (int k = 0; k < QENT; ++k) v[k] = Wsp->ringE[(head + i) & 31][k];
-        walk_triangle(*Sp, v, &Wsp->rec[0][0]);
+        for (int k = 0; k < QENT; ++k) v[k] = Wsp->ringE[(head + i) & 7][k];
+        walk_triangle(*Sp, v, &Wsp->rec()[0][0]);
     }
     return done;
 }

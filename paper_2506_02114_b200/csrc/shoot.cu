@@ -38,26 +38,14 @@ __device__ __forceinline__ long long fetch_tile(const ShootDev &S) {
 }
 
 struct Pend {
-    Ring E;                            // only what the global queue could not take
     long long chunk = -1;              // queue chunk this warp is filling
     int used = 0;
 };
 
-// Clears the fallback ring (only ever filled when the global queue is full), 8 triangles at a time.
-__device__ __forceinline__ void run_batches(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, ThreadCounters &tc) {
-    const int lane = threadIdx.x & 31;
-    while (P.E.count > 0) {
-        const int n = min(P.E.count, 8);
-        tc.px_small += tri_batch(&S, W.w32, W.ax, W.ay, &Ws, P.E.head, n);
-        if (lane < n) ++tc.small_;
-        P.E.head = (P.E.head + n) & 31; P.E.count -= n;
-    }
-}
-
 // General triangles go to the global queue, which drain_kernel apportions at full occupancy.  A warp reserves
 // QCHUNK entries at a time (one atomic per chunk); if the queue is full they stay in the warp's own ring and
 // are clipped by the (cold) in-kernel copy.
-__device__ __forceinline__ void queue_push(const ShootDev &S, WarpSharedIpm &Ws, Pend &P, bool pred, const double (&e)[6], ThreadCounters &tc) {
+__device__ __forceinline__ void queue_push(const ShootDev &S, const Win &W, WarpSharedIpm &Ws, Pend &P, bool pred, const double (&e)[6], ThreadCounters &tc) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const unsigned m = __ballot_sync(full, pred);
@@ -73,9 +61,24 @@ __device__ __forceinline__ void queue_push(const ShootDev &S, WarpSharedIpm &Ws,
         P.chunk = (c < S.queue_cap) ? c : -1;
         P.used = 0;
     }
-    if (P.chunk < 0) {                                          // queue full
+    if (P.chunk < 0) {                                          // queue full: apportioned here, 8 at a time (cold)
         if (pred) ++tc.overflow;
-        ring_push<6, 31>(P.E, Ws.ringE, pred, e);
+        unsigned rem = m;
+        while (rem) {
+            unsigned take = 0, t = rem;
+#pragma unroll 1
+            for (int k = 0; k < 8 && t; ++k) { take |= t & (0u - t); t &= t - 1; }
+            const int n8 = __popc(take);
+            __syncwarp();
+            if (pred && ((take >> lane) & 1u)) {
+                double *q = Ws.ringE[__popc(take & ((1u << lane) - 1u))];
+#pragma unroll
+                for (int k = 0; k < QENT; ++k) q[k] = e[k];
+            }
+            tc.px_small += tri_batch(&S, W.w32, W.ax, W.ay, &Ws, 0, n8);
+            if (lane < n8) ++tc.small_;
+            rem &= ~take;
+        }
         return;
     }
     if (pred) {
@@ -154,7 +157,7 @@ __device__ __forceinline__ void process_pending(const ShootDev &S, const Win &W,
         const int mnx = min(x1, min(x2, x3)), mxx = max(x1, max(x2, x3)), mny = min(y1, min(y2, y3)), mxy = max(y1, max(y2, y3));
         const int w = mxx - mnx, h = mxy - mny;
         const bool strip = have && (w + h == 1);
-        queue_push(S, Ws, P, have && !strip, e, tc);
+        queue_push(S, W, Ws, P, have && !strip, e, tc);
         if (strip) {
             const bool ay = (h == 1);                                        // pixels stacked in y
             const double line = ay ? (double)(mny + 1) : (double)(mnx + 1);
@@ -166,7 +169,6 @@ __device__ __forceinline__ void process_pending(const ShootDev &S, const Win &W,
                 pix_add(S, W, mnx + (ay ? 0 : k), mny + (ay ? k : 0), k ? FIX_ONE - a : a);
             ++tc.small_; tc.px_small += 2;
         }
-        run_batches(S, W, Ws, P, tc);
     }
     __syncwarp();
 }

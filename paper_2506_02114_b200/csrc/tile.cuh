@@ -72,13 +72,15 @@ struct WarpShared {
 };
 // ... plus what the IPM kernel needs for apportioning
 struct WarpSharedIpm : WarpShared {
-    double ringE[32][6];                                     // general triangles the global queue could not take (cleared at once)
-    int ids[256];                                            // triangles of the row group that are not singles: (corner row, column, which of the two)
-    double rec[8][10];                                       // per-triangle records of the (cold) in-kernel apportioning, 8 at a time
+    double ringE[8][6];                                      // general triangles the global queue could not take, 8 at a time (cold)
+    unsigned char ids[256];                                  // triangles of the row group that are not singles: (corner row, column, which of the two)
     double stu[RPT + 1][32], stv[RPT + 1][32];               // mapped corners of the row group in pixel units (row 0 = last row of the previous group)
     int stp[RPT + 1][32];                                    // their packed pixels
     int sto[RPT + 1][32];                                    // and on which sides of the map they lie (0: inside)
+    // the per-triangle records of the (cold) in-kernel apportioning live in `e`, which only the tile set-up uses
+    __device__ double (*rec())[10] { return reinterpret_cast<double (*)[10]>(e); }
 };
+static_assert(sizeof(double2) * ML_P1MAX >= 8 * 10 * sizeof(double), "records must fit the set-up scratch");
 static_assert(FOLDJ >= 4 && ML_NEAR == 32, "fold scratch must fit the window");
 
 struct TileCtx {                       // warp-uniform registers
@@ -356,8 +358,8 @@ __device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
     return r;
 }
-__device__ __forceinline__ float lo2(unsigned long long v) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return lo; }
-__device__ __forceinline__ float hi2(unsigned long long v) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return hi; }
+__device__ __forceinline__ float lo2(unsigned long long v) { float lo, hi; (void)hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return lo; }
+__device__ __forceinline__ float hi2(unsigned long long v) { float lo, hi; (void)lo; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return hi; }
 __device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
     unsigned long long r;
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
