@@ -189,6 +189,107 @@ __global__ void downward_kernel(FmmDev F, int a, int b) {
     if (act) F.loc[(size_t)node * F.p1 + l] = (l >= 1) ? acc : make_double2(0.0, 0.0);
 }
 
+// The downward pass for orders p <= 31: one WARP per node, lane = coefficient l, no block barriers.  M2L is a
+// real p x p binomial matrix (the same for every pair, eq C5) times the complex source vectors scaled by powers of
+// -1/z0: the matrix sits transposed in shared memory (lane-contiguous, conflict free), DW_NP source vectors are
+// staged per pass so that one matrix element feeds 2 DW_NP FMAs, and the inner loop is bound by the FP64 pipe.
+static const int DW_WARPS = 8, DW_NP = 4, DW_PMAX = 31;
+__global__ void __launch_bounds__(DW_WARPS * 32) downward_warp_kernel(FmmDev F, int a, int b) {
+    __shared__ double Bt[DW_PMAX * 32];                         // Bt[(k-1) 32 + l] = C(l+k-1, k-1)
+    __shared__ double2 src_s[DW_WARPS][DW_NP][32];
+    const unsigned full = 0xffffffffu;
+    const int p = F.p, l = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < p * 32; i += blockDim.x) {
+        const int k = i / 32 + 1, ll = i % 32;
+        Bt[i] = (ll >= 1 && ll <= p) ? F.binom[(size_t)(ll + k - 1) * BN + (k - 1)] : 0.0;
+    }
+    __syncthreads();
+    double2 (*src)[32] = src_s[warp];
+    const bool act = (l <= p), row = act && (l >= 1);
+    const double inv_l = (l >= 1) ? 1.0 / (double)l : 0.0;
+    for (int node = a + blockIdx.x * DW_WARPS + warp; node < b; node += gridDim.x * DW_WARPS) {
+        const int P = F.parent[node], ix = F.ix[node], iy = F.iy[node], lev = F.level[node];
+        double2 acc = make_double2(0.0, 0.0);
+        // ---- L2L (eq C7, reading G3)
+        __syncwarp(full);
+        if (act) src[0][l] = F.loc[(size_t)P * F.p1 + l];
+        __syncwarp(full);
+        if (row) {
+            const int q = (ix & 1) + 2 * (iy & 1);
+            const double2 *zp = F.tab + (size_t)(TAB_L2L + q) * ML_P1MAX;
+            double2 t = make_double2(0.0, 0.0);
+            for (int k = l; k <= p; ++k) {
+                const double bc = F.binom[(size_t)k * BN + l];
+                const double2 u = cmul(src[0][k], zp[k - l]);
+                t.x = fma(bc, u.x, t.x); t.y = fma(bc, u.y, t.y);
+            }
+            acc = cscale(t, scalbn(1.0, -l));
+        }
+        // ---- M2L (eq C5), DW_NP pairs per pass
+        const int nm = F.m2l_cnt[node];
+        for (int e0 = 0; e0 < nm; e0 += DW_NP) {
+            const double2 *wp[DW_NP];
+            __syncwarp(full);
+#pragma unroll
+            for (int q = 0; q < DW_NP; ++q) {
+                double2 v = make_double2(0.0, 0.0);
+                wp[q] = F.tab + (size_t)(TAB_M2L + 3 * 7 + 3) * ML_P1MAX;       // offset (0, 0): all zeros beyond n = 0
+                if (e0 + q < nm) {
+                    const int S = F.m2l_list[(size_t)node * 27 + e0 + q];
+                    const int dx = F.ix[S] - ix, dy = F.iy[S] - iy;
+                    wp[q] = F.tab + (size_t)(TAB_M2L + (dy + 3) * 7 + dx + 3) * ML_P1MAX;   // (-1/z0)^n
+                    if (act) v = cmul(F.mp[(size_t)S * F.p1 + l], wp[q][l]);
+                }
+                src[q][l] = v;
+            }
+            __syncwarp(full);
+            double2 t[DW_NP];
+#pragma unroll
+            for (int q = 0; q < DW_NP; ++q) t[q] = make_double2(-src[q][0].x * inv_l, 0.0);
+#pragma unroll 2
+            for (int k = 1; k <= p; ++k) {
+                const double bc = Bt[(k - 1) * 32 + l];
+#pragma unroll
+                for (int q = 0; q < DW_NP; ++q) {
+                    const double2 sv = src[q][k];
+                    t[q].x = fma(bc, sv.x, t[q].x); t[q].y = fma(bc, sv.y, t[q].y);
+                }
+            }
+            if (row) {
+#pragma unroll
+                for (int q = 0; q < DW_NP; ++q) {
+                    if (e0 + q < nm) {
+                        double2 zi = wp[q][l];                        // (1/z0)^l = (-1)^l (-1/z0)^l
+                        if (l & 1) { zi.x = -zi.x; zi.y = -zi.y; }
+                        const double2 u = cmul(t[q], zi);
+                        acc.x += u.x; acc.y += u.y;
+                    }
+                }
+            }
+        }
+        // ---- P2L (eq C6): stars of coarser childless nodes outside this node's 3x3 block
+        const int np = F.p2l_cnt[node];
+        if (np > 0 && row) {
+            double cx, cy, half;
+            node_geom(F, node, cx, cy, half);
+            const int sh = ML_QBITS - lev;
+            for (int e = 0; e < np; ++e) {
+                const int Q = F.p2l_list[(size_t)node * 8 + e];
+                const int lo = F.lo[Q], n = F.n[Q];
+                for (int i = lo; i < lo + n; ++i) {
+                    const int cxq = (int)(F.sqx[i] >> sh), cyq = (int)(F.sqy[i] >> sh);
+                    if (abs(cxq - ix) <= 1 && abs(cyq - iy) <= 1) continue;
+                    const double2 zeta = make_double2((F.sx[i] - cx) / half, (F.sy[i] - cy) / half);
+                    const double2 w = cpowi(cinv(zeta), l);
+                    const double f = -F.sm[i] * inv_l;
+                    acc.x = fma(f, w.x, acc.x); acc.y = fma(f, w.y, acc.y);
+                }
+            }
+        }
+        if (act) F.loc[(size_t)node * F.p1 + l] = row ? acc : make_double2(0.0, 0.0);
+    }
+}
+
 // e_l = (l+1) c_{l+1} theta^2 / L for l < p: the derivative series of eq C4 the evaluator sums (eq 24)
 __global__ void leaf_coef_kernel(FmmDev F, int n_leaves) {
     int leaf = blockIdx.x, l = threadIdx.x;
@@ -221,7 +322,14 @@ int fmm_passes(mlens_field *f, cudaStream_t s) {
     }
     for (int lev = 2; lev < t.n_levels; ++lev) {
         int a = t.level_off[lev], b = t.level_off[lev + 1];
-        ML_LAUNCH(downward_kernel, b - a, T, 0, s, F, a, b);
+        if (p <= DW_PMAX) {
+            int nsm = 148;
+            cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, f->device);
+            const int want = (b - a + DW_WARPS - 1) / DW_WARPS, cap = nsm * 6;
+            ML_LAUNCH(downward_warp_kernel, (want < cap) ? want : cap, DW_WARPS * 32, 0, s, F, a, b);
+        } else {
+            ML_LAUNCH(downward_kernel, b - a, T, 0, s, F, a, b);
+        }
     }
     ML_LAUNCH(leaf_coef_kernel, (unsigned)nl, T, 0, s, F, (int)nl);
     ML_CUDA(cudaGetLastError());
