@@ -259,7 +259,7 @@ int mlens_field_destroy(mlens_field *f) {
     f->ox.release(); f->oy.release(); f->om.release(); f->sx.release(); f->sy.release(); f->sm.release();
     f->sqx.release(); f->sqy.release(); f->binom.release(); f->tab.release(); f->acc.release(); f->diff.release();
     scratch_park(f);
-    f->queue.release(); f->qcount.release(); f->biglist.release(); f->counters.release();
+    f->queue.release(); f->qcount.release(); f->biglist.release(); f->giant.release(); f->counters.release();
     f->tree.release();
     delete f;
     return MLENS_OK;

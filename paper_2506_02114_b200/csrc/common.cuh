@@ -107,6 +107,7 @@ struct mlens_field {
     ml::DevBuf<double> queue;            // general-triangle queue
     ml::DevBuf<int> qcount;              // entries per queue chunk
     ml::DevBuf<unsigned int> biglist;    // queue entries to be walked edge by edge
+    ml::DevBuf<unsigned long long> giant; // chunks of the giant triangles among them
     ml::DevBuf<unsigned long long> counters;
     int device = 0;
 };

@@ -392,7 +392,10 @@ __device__ __forceinline__ unsigned apportion_batch(const ShootDev &S, const Win
 // Lanes 0-2 set up one edge each into `scratch` (3 x 16 doubles of the warp's shared memory); then the steps
 // of all three edges form one index space the lanes stride over, so a triangle of a few dozen steps still
 // fills the warp.
-__device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT], double *scratch) {
+// Only the steps [k_lo, k_hi) of the triangle's step index space are walked (a giant triangle is shared out in
+// chunks; every chunk sets the same edges up, so the chunks' end points still agree bit for bit).
+__device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT], double *scratch,
+                                                            int k_lo = 0, int k_hi = 0x7fffffff) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
@@ -421,8 +424,9 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
     const int n0 = __shfl_sync(full, ne, 0), n1 = __shfl_sync(full, ne, 1), n2 = __shfl_sync(full, ne, 2);
     const int total = n0 + n1 + n2;
     __syncwarp();
+    const int k_end = min(total, k_hi);
 #pragma unroll 1
-    for (int k = lane; k < total; k += 32) {
+    for (int k = k_lo + lane; k < k_end; k += 32) {
         const int e = (k >= n0 + n1) ? 2 : (k >= n0 ? 1 : 0);
         const double *q = scratch + 16 * e;
         EdgeWalk E;
@@ -431,7 +435,7 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
         edge_step(S, E, k - (e == 2 ? n0 + n1 : (e == 1 ? n0 : 0)), cs, bx, by);
     }
     __syncwarp();
-    return (unsigned long long)total;
+    return (unsigned long long)max(k_end - k_lo, 0);
 }
 
 // The shooting kernel's own copy, for the triangles it could not hand to the global queue (queue full).

@@ -312,6 +312,8 @@ __global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_co
 static const int WALK_WARPS = 8;
 static const int WB = 16;              // triangles per batch
 static const int EREC = 10;            // doubles per edge record
+static const int GIANT_STEPS = 1024;   // a triangle with more steps than this is not walked by one warp alone
+static const int GIANT_CHUNK = 512;    // but in chunks of this many steps, one warp each
 __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_constant__ ShootDev S) {
     __shared__ double er_s[WALK_WARPS][3 * WB][EREC];
     __shared__ double tr_s[WALK_WARPS][WB][8];           // local vertices, cs, (bx, by)
@@ -374,6 +376,15 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
         // steps per triangle (lane < WB) and their inclusive prefix
         int ntot = 0;
         if (lane < WB) ntot = __double2hiint(er[3 * lane][9]) + __double2hiint(er[3 * lane + 1][9]) + __double2hiint(er[3 * lane + 2][9]);
+        if (ntot > GIANT_STEPS) {
+            // too many steps for one warp (the faint images of the whole map): shared out in chunks to walk_giant_kernel
+            const int nch = (ntot + GIANT_CHUNK - 1) / GIANT_CHUNK;
+            const unsigned long long at = atomicAdd(&S.counters[C_GIANT], (unsigned long long)nch);
+            if ((long long)(at + nch) <= S.giant_cap) {           // (else it stays here; the skipped slots keep their sentinel)
+                for (int c = 0; c < nch; ++c) S.giant[at + c] = ((unsigned long long)it << 20) | (unsigned long long)c;
+                ntot = 0;
+            }
+        }
         int inc = ntot;
 #pragma unroll
         for (int o = 1; o < WB; o <<= 1) { int t = __shfl_up_sync(full, inc, o); if (lane >= o) inc += t; }
@@ -410,6 +421,32 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
     }
     if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&S.counters[C_CHUNKS], (unsigned long long)nb);   // walked, all bands
+}
+
+// The giant triangles walk_kernel set aside: one warp per chunk of GIANT_CHUNK steps.
+__global__ void __launch_bounds__(256) walk_giant_kernel(const __grid_constant__ ShootDev S) {
+    __shared__ double scratch_s[8][48];
+    double *scratch = scratch_s[threadIdx.x >> 5];
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    long long n = (long long)S.counters[C_GIANT];
+    if (n > S.giant_cap) n = S.giant_cap;
+    unsigned long long n_pieces = 0;
+    while (true) {
+        long long i = 0;
+        if (lane == 0) i = (long long)atomicAdd(&S.counters[C_GWALK], 1ull);
+        i = __shfl_sync(full, i, 0);
+        if (i >= n) break;
+        const unsigned long long ent = S.giant[i];
+        if (ent == ~0ull) continue;                                 // a slot whose triangle stayed with walk_kernel
+        const int c = (int)(ent & 0xfffffull);
+        const double *e = S.queue + (size_t)S.biglist[ent >> 20] * QENT;
+        double v[QENT];
+#pragma unroll
+        for (int k = 0; k < QENT; ++k) v[k] = __ldg(&e[k]);
+        n_pieces += walk_triangle(S, v, scratch, c * GIANT_CHUNK, (c + 1) * GIANT_CHUNK);
+    }
+    if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
 }
 
 // floor(d / p), the pixel rule of O5, exactly, as an integer (saturated; NaN -> INT_MIN, outside every map): the
@@ -616,6 +653,8 @@ void scratch_take(mlens_field *f) {
     g_parked.queue = DevBuf<double>(); g_parked.qcount = DevBuf<int>(); g_parked.biglist = DevBuf<unsigned int>();
 }
 
+static const long long GIANT_CAP = 1ll << 20;       // chunk slots per band (8 MB)
+
 static long long env_ll(const char *name, long long dflt) {
     const char *v = getenv(name);
     if (!v || !*v) return dflt;
@@ -655,6 +694,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             int rc = f->queue.reserve((size_t)qcap * QCHUNK * QENT, s, false);
             if (rc == MLENS_OK) rc = f->qcount.reserve((size_t)qcap, s, false);
             if (rc == MLENS_OK) rc = f->biglist.reserve((size_t)qcap * QCHUNK / 4, s, false);
+            if (rc == MLENS_OK) rc = f->giant.reserve((size_t)GIANT_CAP, s, false);
             if (rc == MLENS_OK) break;
             if (rc != MLENS_ENOMEM || qmb_env > 0 || qmb <= 256) return rc;
             cudaGetLastError();
@@ -667,7 +707,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     S.i0 = i0; S.i1 = i1; S.j0 = j0; S.j1 = j1;
     S.ylo1 = g->ylo1; S.ylo2 = g->ylo2; S.p1 = g->p1; S.p2 = g->p2; S.inv_p1 = 1.0 / g->p1; S.inv_p2 = 1.0 / g->p2;
     S.npix1 = d->npix1; S.npix2 = d->npix2;
-    S.acc = f->acc.p; S.diff = f->diff.p; S.queue = f->queue.p; S.qcount = f->qcount.p; S.biglist = f->biglist.p; S.big_cap = qcap * QCHUNK / 4; S.counters = f->counters.p; S.queue_cap = qcap;
+    S.acc = f->acc.p; S.diff = f->diff.p; S.queue = f->queue.p; S.qcount = f->qcount.p; S.biglist = f->biglist.p; S.big_cap = qcap * QCHUNK / 4; S.giant = f->giant.p; S.giant_cap = ipm ? GIANT_CAP : 0; S.counters = f->counters.p; S.queue_cap = qcap;
     S.dump1 = d->dump_w1; S.dump2 = d->dump_w2;
     S.binom = f->binom.p;
     if ((S.dump1 == nullptr) != (S.dump2 == nullptr)) { set_error("dump_w1 and dump_w2 go together"); return MLENS_EINVAL; }
@@ -743,7 +783,8 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         const long long want = (nt + SHOOT_WARPS - 1) / SHOOT_WARPS;
         int grid = (int)((want < resident) ? want : resident);
         ML_CUDA(cudaMemsetAsync(f->counters.p, 0, 16, s));         // queue fill count and tile counter
-        ML_CUDA(cudaMemsetAsync(f->counters.p + C_DRAIN, 0, 3 * 8, s));   // drain, big-list and walk counters
+        ML_CUDA(cudaMemsetAsync(f->counters.p + C_DRAIN, 0, 5 * 8, s));   // drain, big-list, walk and giant counters
+        if (ipm) ML_CUDA(cudaMemsetAsync(f->giant.p, 0xff, (size_t)GIANT_CAP * 8, s));   // sentinels
         ML_TRY(mark());
         if (ipm) {
             if (f32) ML_LAUNCH(shoot_ipm_kernel<true>, grid, SHOOT_WARPS * 32, smem_ipm, s, S);
@@ -761,8 +802,9 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             }
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
             ML_LAUNCH(walk_kernel, nsm * 4, WALK_WARPS * 32, 0, s, S);
+            ML_LAUNCH(walk_giant_kernel, nsm * 8, 256, 0, s, S);
             ML_TRY(mark());
-            launches += 3;
+            launches += 4;
         } else {
             if (f32) ML_LAUNCH(shoot_irs_kernel<true>, grid, SHOOT_WARPS * 32, smem_irs, s, S);
             else ML_LAUNCH(shoot_irs_kernel<false>, grid, SHOOT_WARPS * 32, smem_irs, s, S);

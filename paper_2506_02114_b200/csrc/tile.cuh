@@ -25,7 +25,7 @@ static const int BN = 2 * ML_P1MAX;   // stride of the Pascal triangle
 
 // slots of ShootDev::counters
 enum { C_QUEUE = 0, C_TILE, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR,
-       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_BIG, C_WALK, C_NCOUNTERS };
+       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_BIG, C_WALK, C_GIANT, C_GWALK, C_NCOUNTERS };
 
 // What a shooting kernel needs besides the lens: the ray grid, the map, the accumulators.
 struct ShootDev {
@@ -40,6 +40,8 @@ struct ShootDev {
     int *qcount;                       // entries in each chunk
     unsigned int *biglist;             // queue entries whose triangles are walked edge by edge (walk_kernel)
     long long big_cap;
+    unsigned long long *giant;         // (walk-list index << 20 | chunk) of the triangles with too many steps for one warp
+    long long giant_cap;
     unsigned long long *counters;
     long long queue_cap;               // chunks
     double *dump1, *dump2;
