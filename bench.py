@@ -353,6 +353,27 @@ def run_ours(args):
         ff.close()
         del out32
 
+    # the map consumers (HBM-bound): histogram of a synthetic log-normal 8192^2 map (512 MiB > L2)
+    consumers = None
+    if world == 1:
+        big = torch.empty((8192, 8192), dtype=torch.float64, device=dev).log_normal_(0.0, 1.0)
+        ms = []
+        for _ in range(4):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); hh = ml.histogram(big, 1.0, -2.0, 2.0, 64); e1.record(stream); e1.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        gbs = big.numel() * 8 / (min(ms[1:]) * 1e-3) / 1e9
+        peak_hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs") if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        lc = ml.light_curve(map_ipm, g.ylo1, g.ylo2, g.p1, g.p2, (-0.9 * half, -0.7 * half), (0.9 * half, 0.8 * half), 1 << 20,
+                            interp=ml.INTERP_BILINEAR)
+        e1.record(stream); e1.synchronize()
+        consumers = {"histogram_ms": min(ms[1:]), "histogram_GBps": gbs, "hbm_peak_GBps": peak_hbm,
+                     "histogram_frac_of_hbm": (gbs / peak_hbm) if peak_hbm else None, "histogram_total": int(hh.sum()),
+                     "light_curve_1M_samples_ms": e0.elapsed_time(e1), "light_curve_mean_mu": float(lc.nanmean())}
+        del big
+
     maps = None
     if args.maps and world == 1:
         # BASELINE.json's second metric, map wall-time, on the other configurations (one warm-up, one timed run each)
@@ -413,7 +434,7 @@ def run_ours(args):
             "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
                                                   "n_queue_overflow", "n_px_clipped", "n_edge_steps", "n_rays_fallback")},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline, "cpu_baseline": cpu, "f32_mode": f32, "maps": maps,
+            "roofline": roofline, "cpu_baseline": cpu, "f32_mode": f32, "consumers": consumers, "maps": maps,
         }))
     if world > 1:
         dist.destroy_process_group()

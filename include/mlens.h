@@ -208,6 +208,27 @@ typedef struct {
 } mlens_tree_view;
 int mlens_field_get_tree(const mlens_field *f, mlens_tree_view *view);
 
+/* ---- Map consumers: what the paper reads off its maps ---------------------------------
+ * The map is double[npix2*npix1], row = y2 ascending, pixel (ix, iy) covering
+ * [ylo1 + ix p1, ylo1 + (ix+1) p1) x [ylo2 + iy p2, ylo2 + (iy+1) p2)   (mlens_grid: ylo1, ylo2, p1, p2).
+ *
+ * Light curve (Fig 4, Fig 8: the magnification along a straight source track): n >= 1 samples at
+ * y_i = ya + (yb - ya) i/(n-1) (i = 0 if n = 1).  interp = MLENS_INTERP_NEAREST: the value of the pixel holding
+ * y_i (floor rule, lower edge inclusive); MLENS_INTERP_BILINEAR: bilinear between the four nearest pixel CENTRES
+ * (indices clamped at the border).  A sample outside the map gives NaN.  mu: double[n]. */
+enum { MLENS_INTERP_NEAREST = 0, MLENS_INTERP_BILINEAR = 1 };
+int mlens_map_light_curve(const double *map, int32_t npix1, int32_t npix2, double ylo1, double ylo2, double p1, double p2,
+                          double ya1, double ya2, double yb1, double yb2, int64_t n, int32_t interp,
+                          double *mu, int32_t ptr_kind, void *stream);
+
+/* Magnification histogram (Fig 5, Fig 10): counts of x = log10(mu / mu_ref) in nbins equal bins of
+ * [lo, hi).  Bin j holds edge_j <= mu < edge_{j+1} with edge_j = mu_ref 10^(lo + j (hi-lo)/nbins) evaluated once in
+ * float64 on the host: the decision is a comparison of mu with those edges, never a logarithm of mu.
+ * counts: uint64[nbins + 2] = { below edge_0 (also mu <= 0 and NaN), the bins, at or above edge_nbins }; overwritten.
+ * 1 <= nbins <= 4096, n = number of pixels, mu_ref > 0, hi > lo. */
+int mlens_map_histogram(const double *map, int64_t n, double mu_ref, double lo, double hi, int32_t nbins,
+                        uint64_t *counts, int32_t ptr_kind, void *stream);
+
 /* Micro-benchmarks for the roofline denominators: sustained FP64 FMA rate [FLOP/s]
  * and FP64/u64 global atomic-add rate [adds/s] into a buffer of `n_slots` 8-byte slots. */
 int mlens_bench_dfma(double *flops_per_s, void *stream);

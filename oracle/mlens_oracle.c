@@ -12,7 +12,9 @@
  *   - the seeded star-field generator (own implementation of the counter RNG
  *     specified in DESIGN.md section 4);
  *   - the FMM expansion coefficients BY THEIR DEFINITIONS (eq C2, eq C6 summed
- *     over stars), used only to pin the CUDA operators.
+ *     over stars), used only to pin the CUDA operators;
+ *   - what the paper reads off a map: a light curve along a straight track (Fig 4 P:212,
+ *     Fig 8) and the histogram of log10(mu/mu_ref) (Fig 5, Fig 10).
  * It shares no code, header, table or constant with the CUDA library and is
  * never tuned.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline
  * / --impl reference legs may load it.
@@ -500,3 +502,52 @@ void orc_local_eval(const double *coef, int p, double cx, double cy, double L, d
     s = conjl(s) * (ld)theta * (ld)theta / (ld)L;
     *ax = (double)creall(s); *ay = (double)cimagl(s);
 }
+
+/* ---- map consumers --------------------------------------------------------
+ * Light curve: sample i of n at y = ya + (yb - ya) i/(n-1); pixel units u = (y - ylo)/p (true division).
+ * mode 0: value of the pixel holding the point (floor rule); mode 1: bilinear between the four nearest pixel
+ * centres (centres at integer + 1/2, indices clamped at the border).  Outside the map: NaN. */
+void orc_light_curve(const double *map, int32_t npix1, int32_t npix2, double ylo1, double ylo2, double p1, double p2,
+                     double ya1, double ya2, double yb1, double yb2, int64_t n, int32_t mode, double *mu)
+{
+    for (int64_t i = 0; i < n; ++i) {
+        double t = (n > 1) ? (double)i / (double)(n - 1) : 0.0;
+        double y1 = ya1 + (yb1 - ya1) * t, y2 = ya2 + (yb2 - ya2) * t;
+        double u = (y1 - ylo1) / p1, v = (y2 - ylo2) / p2;
+        mu[i] = NAN;
+        if (!(u >= 0.0 && v >= 0.0 && u < (double)npix1 && v < (double)npix2)) continue;
+        if (mode == 0) {
+            mu[i] = map[(size_t)floor(v) * (size_t)npix1 + (size_t)floor(u)];
+        } else {
+            double uc = u - 0.5, vc = v - 0.5;
+            long iu = (long)floor(uc), iv = (long)floor(vc);
+            double a = uc - (double)iu, b = vc - (double)iv;
+            long i0 = iu < 0 ? 0 : iu, i1 = iu + 1 > npix1 - 1 ? npix1 - 1 : iu + 1;
+            long j0 = iv < 0 ? 0 : iv, j1 = iv + 1 > npix2 - 1 ? npix2 - 1 : iv + 1;
+            double m00 = map[j0 * npix1 + i0], m10 = map[j0 * npix1 + i1], m01 = map[j1 * npix1 + i0], m11 = map[j1 * npix1 + i1];
+            mu[i] = (1.0 - b) * ((1.0 - a) * m00 + a * m10) + b * ((1.0 - a) * m01 + a * m11);
+        }
+    }
+}
+
+/* Histogram of x = log10(mu/mu_ref) in nbins equal bins of [lo, hi): bin j holds edge_j <= mu < edge_{j+1},
+ * edge_j = mu_ref 10^(lo + j (hi-lo)/nbins).  counts[0]: below edge_0 (also mu <= 0, NaN); counts[1+j]: bin j;
+ * counts[nbins+1]: at or above edge_nbins.  Plain linear scan over the edges. */
+void orc_histogram(const double *map, int64_t n, double mu_ref, double lo, double hi, int32_t nbins, uint64_t *counts)
+{
+    double *edge = (double *)malloc((size_t)(nbins + 1) * sizeof(double));
+    for (int j = 0; j <= nbins; ++j) edge[j] = mu_ref * pow(10.0, lo + (double)j * (hi - lo) / (double)nbins);
+    for (int j = 0; j < nbins + 2; ++j) counts[j] = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        double mu = map[i];
+        int slot = 0;
+        if (mu >= edge[0]) {
+            slot = nbins + 1;
+            for (int j = 0; j < nbins; ++j)
+                if (mu < edge[j + 1]) { slot = 1 + j; break; }
+        }
+        counts[slot]++;
+    }
+    free(edge);
+}
+

@@ -242,3 +242,22 @@ def local_eval(coef, cx, cy, L, zx, zy, theta=1.0):
     ax, ay = C.c_double(), C.c_double()
     lib().orc_local_eval(_p(buf), p, cx, cy, L, theta, zx, zy, C.byref(ax), C.byref(ay))
     return ax.value, ay.value
+
+
+def light_curve(map_, ylo1, ylo2, p1, p2, ya, yb, n, mode=0):
+    m = _d(map_)
+    npix2, npix1 = m.shape
+    out = np.empty(n)
+    lib().orc_light_curve(_p(m), C.c_int32(npix1), C.c_int32(npix2), C.c_double(ylo1), C.c_double(ylo2), C.c_double(p1),
+                          C.c_double(p2), C.c_double(ya[0]), C.c_double(ya[1]), C.c_double(yb[0]), C.c_double(yb[1]),
+                          C.c_int64(n), C.c_int32(mode), _p(out))
+    return out
+
+
+def histogram(map_, mu_ref, lo, hi, nbins):
+    m = _d(map_).ravel()
+    out = np.zeros(nbins + 2, dtype=np.uint64)
+    lib().orc_histogram(_p(m), C.c_int64(m.size), C.c_double(mu_ref), C.c_double(lo), C.c_double(hi), C.c_int32(nbins),
+                        out.ctypes.data_as(C.POINTER(C.c_uint64)))
+    return out
+

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libmlens.so")
-SOURCES = ["api.cu", "tree.cu", "fmm.cu", "eval.cu", "shoot.cu"]
+SOURCES = ["api.cu", "tree.cu", "fmm.cu", "eval.cu", "shoot.cu", "consume.cu"]
 HEADERS = ["common.cuh", "device.cuh", "tile.cuh", "deposit.cuh", os.path.join("..", "..", "include", "mlens.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

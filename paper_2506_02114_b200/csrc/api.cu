@@ -356,6 +356,43 @@ int mlens_shoot(mlens_field *f, const mlens_shoot_desc *d, double *map, uint64_t
     return MLENS_OK;
 }
 
+int mlens_map_light_curve(const double *map, int32_t npix1, int32_t npix2, double ylo1, double ylo2, double p1, double p2,
+                          double ya1, double ya2, double yb1, double yb2, int64_t n, int32_t interp,
+                          double *mu, int32_t ptr_kind, void *stream) {
+    ML_TRY(check_device());
+    if (!map || npix1 <= 0 || npix2 <= 0 || !(p1 > 0) || !(p2 > 0) || n < 0 || (n > 0 && !mu)) { set_error("bad arguments"); return MLENS_EINVAL; }
+    if (interp != MLENS_INTERP_NEAREST && interp != MLENS_INTERP_BILINEAR) { set_error("bad interpolation mode"); return MLENS_EINVAL; }
+    cudaStream_t s = (cudaStream_t)stream;
+    Stage st(s);
+    const size_t np = (size_t)npix1 * (size_t)npix2;
+    const double *dmap; double *dmu;
+    ML_TRY(st.in(map, np, ptr_kind, s, &dmap));
+    ML_TRY(st.out(mu, (size_t)n, ptr_kind, &dmu));
+    ML_TRY(map_light_curve(dmap, npix1, npix2, ylo1, ylo2, p1, p2, ya1, ya2, yb1, yb2, n, interp, dmu, s));
+    ML_TRY(st.back(mu, dmu, (size_t)n, ptr_kind, s));
+    if (ptr_kind == MLENS_PTR_HOST) ML_CUDA(cudaStreamSynchronize(s));
+    return MLENS_OK;
+}
+
+int mlens_map_histogram(const double *map, int64_t n, double mu_ref, double lo, double hi, int32_t nbins,
+                        uint64_t *counts, int32_t ptr_kind, void *stream) {
+    ML_TRY(check_device());
+    if (!counts || n < 0 || (n > 0 && !map) || nbins < 1 || nbins > 4096 || !(mu_ref > 0) || !(hi > lo)) { set_error("bad arguments"); return MLENS_EINVAL; }
+    cudaStream_t s = (cudaStream_t)stream;
+    Stage st(s);
+    std::vector<double> edges((size_t)nbins + 1);
+    for (int j = 0; j <= nbins; ++j) edges[j] = mu_ref * pow(10.0, lo + (double)j * (hi - lo) / (double)nbins);
+    for (int j = 1; j <= nbins; ++j) if (!(edges[j] > edges[j - 1])) { set_error("bins too narrow for float64 edges"); return MLENS_EINVAL; }
+    const double *dmap, *dedges; unsigned long long *dcounts;
+    ML_TRY(st.in(map, (size_t)n, ptr_kind, s, &dmap));
+    ML_TRY(st.in(edges.data(), edges.size(), MLENS_PTR_HOST, s, &dedges));
+    ML_TRY(st.out(reinterpret_cast<unsigned long long *>(counts), (size_t)nbins + 2, ptr_kind, &dcounts));
+    ML_TRY(map_histogram(dmap, n, dedges, nbins, dcounts, s));
+    ML_TRY(st.back(reinterpret_cast<unsigned long long *>(counts), dcounts, (size_t)nbins + 2, ptr_kind, s));
+    ML_CUDA(cudaStreamSynchronize(s));                              // `edges` is host memory of this call
+    return MLENS_OK;
+}
+
 int mlens_field_get_tree(const mlens_field *f, mlens_tree_view *v) {
     if (!f || !v) { set_error("null argument"); return MLENS_EINVAL; }
     ML_CUDA(cudaDeviceSynchronize());

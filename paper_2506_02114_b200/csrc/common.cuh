@@ -133,4 +133,8 @@ void scratch_take(mlens_field *f);
 int geometry(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid *g);
 int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double *map,
           unsigned long long *counts, mlens_stats *st, cudaStream_t s);
+// consume.cu
+int map_histogram(const double *map, long long n, const double *edges_dev, int nbins, unsigned long long *counts, cudaStream_t s);
+int map_light_curve(const double *map, int npix1, int npix2, double ylo1, double ylo2, double p1, double p2,
+                    double ya1, double ya2, double yb1, double yb2, long long n, int interp, double *mu, cudaStream_t s);
 }  // namespace ml

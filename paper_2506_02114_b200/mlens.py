@@ -113,6 +113,9 @@ def lib():
         L.mlens_field_get_tree.argtypes = [vp, C.POINTER(TreeView)]
         L.mlens_bench_dfma.argtypes = [_dp, vp]
         L.mlens_bench_atomics.argtypes = [i64, i32, _dp, vp]
+        dbl = C.c_double
+        L.mlens_map_light_curve.argtypes = [vp, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, dbl, dbl, i64, i32, vp, i32, vp]
+        L.mlens_map_histogram.argtypes = [vp, i64, dbl, dbl, dbl, i32, vp, i32, vp]
         _lib = L
     return _lib
 
@@ -355,3 +358,41 @@ def bench_atomics(n_slots, use_u64=True, stream=None):
     v = C.c_double()
     _check(lib().mlens_bench_atomics(n_slots, int(use_u64), C.byref(v), _stream(stream)))
     return v.value
+
+
+# ---- map consumers: marshalling only --------------------------------------------------
+INTERP_NEAREST, INTERP_BILINEAR = 0, 1
+
+
+def light_curve(map_, ylo1, ylo2, p1, p2, ya, yb, n, interp=INTERP_NEAREST, stream=None):
+    """mlens_map_light_curve: n samples of the map along the straight source track ya -> yb (numpy or CUDA tensor map)."""
+    npix2, npix1 = map_.shape
+    if _is_torch(map_):
+        import torch
+        out = torch.empty(n, dtype=torch.float64, device=map_.device)
+    else:
+        map_ = np.ascontiguousarray(map_, dtype=np.float64)
+        out = np.empty(n)
+    kind = _same_kind(map_, out)
+    _check(lib().mlens_map_light_curve(_ptr(map_)[0], C.c_int32(npix1), C.c_int32(npix2), C.c_double(ylo1), C.c_double(ylo2),
+                                       C.c_double(p1), C.c_double(p2), C.c_double(ya[0]), C.c_double(ya[1]),
+                                       C.c_double(yb[0]), C.c_double(yb[1]), C.c_int64(n), C.c_int32(interp),
+                                       _ptr(out)[0], C.c_int32(kind), _stream(stream)))
+    return out
+
+
+def histogram(map_, mu_ref, lo, hi, nbins, stream=None):
+    """mlens_map_histogram: counts of log10(mu/mu_ref) in nbins bins of [lo, hi): [below, bins..., above]."""
+    n = int(map_.numel()) if _is_torch(map_) else int(np.size(map_))
+    if _is_torch(map_):
+        import torch
+        map_ = map_.contiguous()
+        out = torch.zeros(nbins + 2, dtype=torch.int64, device=map_.device)      # same bits as uint64
+    else:
+        map_ = np.ascontiguousarray(map_, dtype=np.float64)
+        out = np.zeros(nbins + 2, dtype=np.uint64)
+    kind = _same_kind(map_, out)
+    _check(lib().mlens_map_histogram(_ptr(map_)[0], C.c_int64(n), C.c_double(mu_ref), C.c_double(lo), C.c_double(hi),
+                                     C.c_int32(nbins), _ptr(out)[0], C.c_int32(kind), _stream(stream)))
+    return out
+

@@ -458,3 +458,41 @@ def test_ipm_and_irs_agree_on_gpu(ml):
     sig = np.sqrt(np.maximum(irs, 1e-9) / 24.0 ** 2)
     assert np.mean(np.abs(irs - ipm) / sig) < 1.5 and np.max(np.abs(irs - ipm) / sig) < 8.0
     assert irs.mean() == pytest.approx(ipm.mean(), rel=5e-3)
+
+
+# ----------------------------------------------------------------------------- map consumers
+def test_map_consumers_parity(ml, orc):
+    """Light curve and magnification histogram of a real IPM map against the oracle: histogram counts bit-exact
+    (bins are decided by comparisons with float64 edges on both sides), light-curve samples equal up to the
+    contraction of a multiply-add (1e-13 relative), NaN outside the map on both sides; host and device buffers."""
+    import torch
+    cfg, gf, of, _ = _cfg_field(ml, orc, 0)
+    res = gf.shoot(cfg.half_y, cfg.npix, cfg.rays_per_pixel_length, border_mode=cfg.border_mode, border_param=cfg.border_param)
+    m, g = res.map, res.grid
+    mu_macro = 1.0 / abs((1 - cfg.kappa_tot) ** 2 - cfg.gamma ** 2)
+    for nb, lo, hi in ((1, -1.0, 1.0), (50, -1.5, 1.5), (4096, -2.0, 2.0), (7, 0.3, 0.31)):
+        want = orc.histogram(m, mu_macro, lo, hi, nb)
+        got = ml.histogram(m, mu_macro, lo, hi, nb)
+        assert np.array_equal(got, want) and int(got.sum()) == m.size
+        got_d = ml.histogram(torch.from_numpy(m).cuda(), mu_macro, lo, hi, nb).cpu().numpy().astype(np.uint64)
+        assert np.array_equal(got_d, want)
+    tracks = [((-4.0, -21.0 / 5.0), (4.9, 4.2), 1000),            # diagonal, inside
+              ((-6.0, 0.3), (6.0, 0.3), 513),                      # horizontal, leaves the map at both ends
+              ((-2.1, -5.0), (-2.1, 5.0 - 1e-9), 4096),            # vertical slice (Fig 8, P:317), edge to edge
+              ((1.0, 1.0), (1.0, 1.0), 1)]
+    for ya, yb, n in tracks:
+        for mode in (ml.INTERP_NEAREST, ml.INTERP_BILINEAR):
+            want = orc.light_curve(m, g.ylo1, g.ylo2, g.p1, g.p2, ya, yb, n, mode=mode)
+            got = ml.light_curve(m, g.ylo1, g.ylo2, g.p1, g.p2, ya, yb, n, interp=mode)
+            assert np.array_equal(np.isnan(got), np.isnan(want))
+            ok = ~np.isnan(want)
+            if mode == ml.INTERP_NEAREST:
+                assert np.array_equal(got[ok], want[ok])
+            else:
+                assert np.max(np.abs(got[ok] - want[ok]) / np.maximum(np.abs(want[ok]), 1e-300), initial=0.0) <= 1e-13
+            got_d = ml.light_curve(torch.from_numpy(m).cuda(), g.ylo1, g.ylo2, g.p1, g.p2, ya, yb, n, interp=mode).cpu().numpy()
+            assert np.array_equal(got_d, got, equal_nan=True)
+    with pytest.raises(ml.MlensError):
+        ml.histogram(m, -1.0, 0.0, 1.0, 4)
+    with pytest.raises(ml.MlensError):
+        ml.histogram(m, 1.0, 0.0, 1.0, 5000)
