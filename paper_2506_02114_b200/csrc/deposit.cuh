@@ -108,21 +108,6 @@ __device__ __forceinline__ double frac_below(double d0, double d1, double d2) {
     return lone_neg ? f : 1.0 - f;
 }
 
-// ---- warp ring buffers of pending work (entries of NW doubles, capacity MASK + 1; strips: always < 32 pending
-// before a push of at most 31; fallback triangles: always 0 pending before a push)
-struct Ring { int head = 0, count = 0; };
-
-template <int NW, int MASK>
-__device__ __forceinline__ void ring_push(Ring &R, double (*buf)[NW], bool pred, const double (&v)[NW]) {
-    const unsigned m = __ballot_sync(0xffffffffu, pred);
-    if (pred) {
-        int pos = (R.head + R.count + __popc(m & ((1u << (threadIdx.x & 31)) - 1u))) & MASK;
-#pragma unroll
-        for (int k = 0; k < NW; ++k) buf[pos][k] = v[k];
-    }
-    R.count += __popc(m);
-}
-
 // min / max by one compare and one select (fmin / fmax also order NaNs: a dozen instructions each on FP64)
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }     // operands are never NaN here
 __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
