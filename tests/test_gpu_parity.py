@@ -347,6 +347,47 @@ def test_subrange_and_accumulate(ml, orc):
     assert np.array_equal(dev.map.cpu().numpy(), whole.map)          # integer accumulation: bit-reproducible
 
 
+def test_full_size_config1_in_bench_configuration(ml, orc):
+    """BASELINE.json configs[1] whole, launched exactly as bench.py launches it (device-resident, default bands and
+    queue): properties that hold at any size tie it to the patches the oracle checks (`test_ipm_patches_big_configs`).
+    The map of the whole grid equals the sum of the maps of three row slabs (each slab takes other bands, tiles and
+    queue chunks: a slab anchors its ray tiles at its own first row, so its rays carry another 5 %-of-eps truncation
+    of the tile series, DESIGN s5.4 -- pixels agree to 1e-6, all but 0.1 % of them to 1e-9); IRS counts add up exactly
+    up to the rays that such a shift carries over a pixel edge;
+    two runs give the same bits; flux: every ray of the IRS grid is counted at most once and the mean magnification
+    matches 1/|(1-kappa)^2-gamma^2| within the 1 % deficit eq 16 allows plus sampling error."""
+    import torch
+    cfg = synth.get_config(1)
+    dev = torch.device("cuda")
+    f = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, cfg.seed, kappa_star=cfg.kappa_star)
+    kw = dict(border_mode=cfg.border_mode, border_param=cfg.border_param, device=dev)
+    args = (cfg.half_y, cfg.npix, cfg.rays_per_pixel_length)
+    whole = f.shoot(*args, **kw)
+    g = whole.grid
+    assert whole.stats["n_queue_overflow"] == 0 and whole.stats["n_cells"] == g.n1 * g.n2
+    again = f.shoot(*args, **kw)
+    assert torch.equal(whole.map, again.map)
+    cuts = [0, g.n2 // 5, g.n2 // 2 + 7, g.n2]
+    acc = torch.zeros_like(whole.map)
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        f.shoot(*args, sub=(0, g.n1, a, b), out=acc, accumulate=True, **kw)
+    rel = ((acc - whole.map).abs() / whole.map.clamp_min(0.1))
+    assert float(rel.max()) <= 1e-6 and float((rel > 1e-9).double().mean()) <= 1e-3, (float(rel.max()), float((rel > 1e-9).double().mean()))
+    mu_th = 1.0 / abs((1 - cfg.kappa_tot) ** 2 - cfg.gamma ** 2)
+    mean_ipm = float(whole.map.mean())
+    assert 0.96 * mu_th <= mean_ipm <= 1.02 * mu_th, (mean_ipm, mu_th)
+    # IRS: counts of the slabs add up exactly; IPM and IRS agree on the flux
+    irs = f.shoot(*args, map_mode=ml.MAP_IRS, want_counts=True, **kw)
+    tot = torch.zeros_like(irs.counts)
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        part = f.shoot(*args, map_mode=ml.MAP_IRS, want_counts=True, sub=(0, g.n1, a, b), **kw)
+        tot += part.counts
+    assert torch.equal(tot, irs.counts)
+    assert int(irs.counts.sum()) <= g.n1 * g.n2
+    assert float(irs.map.mean()) == pytest.approx(mean_ipm, rel=2e-3)
+    f.close()
+
+
 def test_errors(ml):
     z = np.zeros(1)
     with pytest.raises(ml.MlensError):
