@@ -162,33 +162,36 @@ __device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, doub
     const double fi = floor(xm);
     const int ic = (int)fi + bx;
     if (ic >= S.npix1) return;
+    unsigned long long *row = S.diff + (size_t)jr * S.npix1;
     long long r = tcov;                                        // left of the map: the whole cover enters at column 0
     int c0 = 0;
     if (ic >= 0) {
         const double m = clamp01(xm - fi);
         r = __double2ll_rn((double)tcov * m);
         c0 = ic + 1;
-        diff_add(S, ic, jr, (unsigned long long)(tcov - r));
+        if (tcov != r) atomicAdd(row + ic, (unsigned long long)(tcov - r));
     }
-    if (c0 < S.npix1) diff_add(S, c0, jr, (unsigned long long)r);
+    if (c0 < S.npix1 && r != 0) atomicAdd(row + c0, (unsigned long long)r);
 }
 
-// Step k of the edge (0 <= k < E.n): from major-axis grid line k-1 (or the clipped start) to grid line k (or the
+// Step k of an edge (0 <= k < n): from major-axis grid line k-1 (or the clipped start) to grid line k (or the
 // clipped end).  End points on a grid line take its exact value and an unclipped end the vertex itself, so
-// consecutive steps and consecutive edges share their end points bit for bit.
-__device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, int k, double cs, int bx, int by) {
-    const double d = E.majorY ? E.dy : E.dx, c0 = E.majorY ? E.y0 : E.x0, id = E.majorY ? E.idy : E.idx;
-    const double od = E.majorY ? E.dx : E.dy, oc0 = E.majorY ? E.x0 : E.y0, oid = E.majorY ? E.idx : E.idy;
-    // start and end in (major, other) coordinates
+// consecutive steps and consecutive edges share their end points bit for bit.  The edge comes in (major, other)
+// coordinates: c0 -> c1 along the axis that is walked, oc0 -> o1 along the other, id / oid the reciprocals of the
+// two extents (0 for an extent of 0), [ta, tb] the clipped parameter range, g0 the first grid line, sg the direction.
+__device__ __forceinline__ void edge_step_mo(const ShootDev &S, double c0, double oc0, double c1, double o1, double id, double oid,
+                                             double ta, double tb, double g0, double sg, bool my, int n, int k,
+                                             double cs, int bx, int by) {
+    const double d = c1 - c0, od = o1 - oc0;
     double ms, os, me, oe, ts, te;
-    if (k == 0) { ts = E.ta; ms = (ts == 0.0) ? c0 : fma(ts, d, c0); os = (ts == 0.0) ? oc0 : fma(ts, od, oc0); }
-    else { ms = E.g0 + E.sg * (double)(k - 1); ts = dmin(dmax((ms - c0) * id, E.ta), E.tb); os = fma(ts, od, oc0); }
-    if (k == E.n - 1) {
-        te = E.tb;
+    if (k == 0) { ts = ta; ms = (ts == 0.0) ? c0 : fma(ts, d, c0); os = (ts == 0.0) ? oc0 : fma(ts, od, oc0); }
+    else { ms = g0 + sg * (double)(k - 1); ts = dmin(dmax((ms - c0) * id, ta), tb); os = fma(ts, od, oc0); }
+    if (k == n - 1) {
+        te = tb;
         const bool vtx = (te == 1.0);
-        me = vtx ? (E.majorY ? E.y1 : E.x1) : fma(te, d, c0);
-        oe = vtx ? (E.majorY ? E.x1 : E.y1) : fma(te, od, oc0);
-    } else { me = E.g0 + E.sg * (double)k; te = dmin(dmax((me - c0) * id, E.ta), E.tb); oe = fma(te, od, oc0); }
+        me = vtx ? c1 : fma(te, d, c0);
+        oe = vtx ? o1 : fma(te, od, oc0);
+    } else { me = g0 + sg * (double)k; te = dmin(dmax((me - c0) * id, ta), tb); oe = fma(te, od, oc0); }
     // at most one grid line of the other axis lies strictly between os and oe
     const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
     const bool cross = (od != 0.0) && ((oe > os) ? (gl < oe) : (gl > oe)) && (oe != os);
@@ -199,9 +202,13 @@ __device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, 
     }
     // the axes are swapped back before the deposit, so that one copy of it serves all lanes: the first piece,
     // then the second of those that cross
-    const bool my = E.majorY != 0;
     piece_deposit(S, my ? os : ms, my ? ms : os, my ? og : mg, my ? mg : og, cs, bx, by);
     if (cross) piece_deposit(S, my ? og : mg, my ? mg : og, my ? oe : me, my ? me : oe, cs, bx, by);
+}
+__device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, int k, double cs, int bx, int by) {
+    const bool my = E.majorY != 0;
+    edge_step_mo(S, my ? E.y0 : E.x0, my ? E.x0 : E.y0, my ? E.y1 : E.x1, my ? E.x1 : E.y1, my ? E.idy : E.idx, my ? E.idx : E.idy,
+                 E.ta, E.tb, E.g0, E.sg, my, E.n, k, cs, bx, by);
 }
 
 struct TriSetup {

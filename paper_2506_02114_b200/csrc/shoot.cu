@@ -366,7 +366,9 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
                     const int e1 = (e == 2) ? 0 : e + 1;
                     const double *t = tr[ti];
                     edge_setup(E, t[2 * e], t[2 * e + 1], t[2 * e1], t[2 * e1 + 1], r0, r1, c1);
-                    q[0] = E.x0; q[1] = E.y0; q[2] = E.x1; q[3] = E.y1; q[4] = E.idx; q[5] = E.idy; q[6] = E.ta; q[7] = E.tb; q[8] = E.g0;
+                    const bool my = E.majorY != 0;                    // stored in (major, other) order: no selects per step
+                    q[0] = my ? E.y0 : E.x0; q[1] = my ? E.x0 : E.y0; q[2] = my ? E.y1 : E.x1; q[3] = my ? E.x1 : E.y1;
+                    q[4] = my ? E.idy : E.idx; q[5] = my ? E.idx : E.idy; q[6] = E.ta; q[7] = E.tb; q[8] = E.g0;
                 }
                 q[9] = __hiloint2double(E.n, E.majorY | (E.sg < 0.0 ? 2 : 0));
 
@@ -406,13 +408,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
                 const int e = (m >= n0 + n1) ? 2 : (m >= n0 ? 1 : 0);
                 m -= (e == 2) ? n0 + n1 : (e == 1 ? n0 : 0);
                 const double *q = er[3 * i + e];
-                EdgeWalk E;
-                E.x0 = q[0]; E.y0 = q[1]; E.x1 = q[2]; E.y1 = q[3]; E.dx = E.x1 - E.x0; E.dy = E.y1 - E.y0;
-                E.idx = q[4]; E.idy = q[5]; E.ta = q[6]; E.tb = q[7]; E.g0 = q[8];
                 const int fl = __double2loint(q[9]);
-                E.majorY = fl & 1; E.sg = (fl & 2) ? -1.0 : 1.0; E.n = __double2hiint(q[9]);
                 const double pk = tr[i][7];
-                edge_step(S, E, m, tr[i][6], __double2loint(pk), __double2hiint(pk));
+                edge_step_mo(S, q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7], q[8], (fl & 2) ? -1.0 : 1.0, (fl & 1) != 0,
+                             __double2hiint(q[9]), m, tr[i][6], __double2loint(pk), __double2hiint(pk));
             }
         }
         __syncwarp();
