@@ -332,6 +332,20 @@ def run_ours(args):
                 "launch_ms": dur * 1e3, "launches_per_map": n_l,
                 "share_of_step": st["ms_shoot"] * 1e-3 / sec}
 
+    # BASELINE.json metric: fraction of the atomic roofline for deposition.  Random 64-bit atomic adds into a buffer
+    # the size of config 1's accumulators (16 MB, L2-resident) and of config 4's (1.6 GB, HBM-resident), measured here,
+    # against what the apportioning kernels issued per second of their own time (one add per clipped pixel, two per
+    # edge step at least).
+    atomics = None
+    if world == 1:
+        st_i = state["ipm"]
+        a_l2 = ml.bench_atomics(2 * npix * npix, True)
+        a_hbm = ml.bench_atomics(200_000_000, True)
+        adds = st_i["n_px_clipped"] + 2 * st_i["n_edge_steps"]
+        rate = adds / (st_i["ms_drain"] * 1e-3)
+        atomics = {"l2_resident_adds_per_s": a_l2, "hbm_resident_adds_per_s": a_hbm, "apportioning_adds_per_s": rate,
+                   "frac_of_l2_atomic_rate": rate / a_l2, "apportioning_adds_per_map": adds}
+
     # the single-precision evaluator on the same workload, beside the float64 numbers
     f32 = None
     if world == 1:
@@ -434,7 +448,7 @@ def run_ours(args):
             "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
                                                   "n_queue_overflow", "n_px_clipped", "n_edge_steps", "n_rays_fallback")},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline, "cpu_baseline": cpu, "f32_mode": f32, "consumers": consumers, "maps": maps,
+            "roofline": roofline, "cpu_baseline": cpu, "atomics": atomics, "f32_mode": f32, "consumers": consumers, "maps": maps,
         }))
     if world > 1:
         dist.destroy_process_group()
