@@ -9,3 +9,4 @@ from .mlens import (  # noqa: F401
     BORDER_EQ16, BORDER_A6, BORDER_MARGIN, BORDER_EXPLICIT, MAX_ORDER, MAX_DIRECT,
     light_curve, histogram, INTERP_NEAREST, INTERP_BILINEAR,
 )
+from .starfile import read_star_file, write_star_file  # noqa: F401,E402

@@ -64,3 +64,24 @@ def test_product_does_not_import_oracle():
             if fn.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, fn)).read()
                 assert "oracle" not in txt.replace("a-posteriori", ""), fn
+
+
+def test_star_file_round_trip(tmp_path):
+    """Star files: text and .npy round trips are bit-exact; comments, commas and bad rows."""
+    import numpy as np
+    from paper_2506_02114_b200.starfile import read_star_file, write_star_file
+    rng = np.random.default_rng(3)
+    x, y, m = rng.normal(size=50) * 100, rng.normal(size=50) * 100, rng.uniform(0.08, 1.0, 50)
+    for name in ("stars.txt", "stars.npy"):
+        p = tmp_path / name
+        write_star_file(p, x, y, m)
+        rx, ry, rm = read_star_file(p)
+        assert np.array_equal(rx, x) and np.array_equal(ry, y) and np.array_equal(rm, m)
+    p = tmp_path / "hand.txt"
+    p.write_text("# x1 x2 m\n1.0, 2.0, 0.5  # first\n\n-3 4 1\n")
+    rx, ry, rm = read_star_file(p)
+    assert list(rx) == [1.0, -3.0] and list(ry) == [2.0, 4.0] and list(rm) == [0.5, 1.0]
+    p.write_text("1 2 -1\n")
+    with pytest.raises(ValueError):
+        read_star_file(p)
+
