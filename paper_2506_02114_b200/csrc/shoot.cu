@@ -712,9 +712,10 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if ((S.dump1 == nullptr) != (S.dump2 == nullptr)) { set_error("dump_w1 and dump_w2 go together"); return MLENS_EINVAL; }
     const bool f32 = d->eval_mode == MLENS_EVAL_FMM_F32;       // same tiles and slow paths as FMM; only the fast path differs
     S.eval_mode = f32 ? MLENS_EVAL_FMM : d->eval_mode;
-    S.tq = (int)env_ll("MLENS_TILE_ORDER", 12);
+    S.tq = (int)env_ll("MLENS_TILE_ORDER", 0);
     if (S.tq > TQMAX) S.tq = TQMAX;
-    if (S.tq < 2) S.tq = 2;
+    if (S.tq <= 0) S.tq = -1;                                   // chosen below, once the tile radius is known
+    else if (S.tq < 2) S.tq = 2;
     S.small_px = (int)env_ll("MLENS_SMALL_PX", 24);
     S.fd_tol = 1.0e-9 * (double)((d->npix1 > d->npix2) ? d->npix1 : d->npix2);
     // truncation budget of the tile series: 5 % of the deflection accuracy the field was built for
@@ -723,6 +724,17 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     S.dux = g->h1 * S.inv_rt; S.duy = g->h2 * S.inv_rt;
     S.a1_lin = S.L.one_minus_kappa + S.L.gamma + S.L.kappa_star; S.a2_lin = S.L.one_minus_kappa - S.L.gamma + S.L.kappa_star;
     S.eps_far = 0.02 * f->eps * f->theta;
+    if (S.tq < 0) {
+        // Order of the tile series: term j of a leaf's series shifted to a tile falls like (c rt / L)^j, L the leaf's
+        // half-length (c = 1.14 fits the measured optimum on the five configs; sources lie >= 3 L from the leaf's centre);
+        // the order that brings it under the truncation budget in the smallest leaves, plus two.  Fewer terms mean
+        // more of the near stars summed directly, more terms a longer Horner chain: measured optima 6 (config 3),
+        // 8-9 (config 1), 13+ (config 2, one ray per pixel).  Every tile still checks its own bound.
+        const double leaf_half_min = f->root_half / (double)(1 << (f->tree.n_levels > 0 ? f->tree.n_levels - 1 : 0));
+        const double x = fmin(0.5, 1.14 * S.rt / leaf_half_min);
+        int q = (int)ceil(log(0.5 * S.eps_far) / log(x)) - 1 + 2;
+        S.tq = q < 4 ? 4 : (q > TQMAX ? TQMAX : q);
+    }
     S.eps_star = 0.03 * f->eps * f->theta / (double)ML_NEAR;
     const int stepx = ipm ? TCX - 1 : TCX, stepy = ipm ? TCY - 1 : TCY;
     long long ntx = (i1 - i0 + stepx - 1) / stepx, nty = (j1 - j0 + stepy - 1) / stepy;
