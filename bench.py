@@ -410,6 +410,7 @@ def run_ours(args):
                     rec[name + "_rays"] = r.stats["n_rays"]
                     rec[name + "_evals_per_s"] = r.stats["n_rays"] / (r.stats["ms_total"] * 1e-3)
                     rec[name + "_shoot_ms"] = r.stats["ms_shoot"]
+                    rec["tile_order"] = r.stats["tile_order"]
                     if mode == ml.MAP_IPM:
                         rec["ipm_drain_walk_ms"] = r.stats["ms_drain"]
                         rec["ipm_bands"] = r.stats["n_bands"]
@@ -436,7 +437,7 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "rays_ipm": evals_ipm, "rays_irs": evals_irs,
-                       "stars_seed": seed, "order_p": p, "border": "eq16",
+                       "stars_seed": seed, "order_p": p, "tile_order": state["ipm"]["tile_order"], "border": "eq16",
                        "l2": "flushed between steps (512 MiB fill outside the per-step events)",
                        "parallelism": (f"{world} GPUs: star-weighted row slabs of one map + all-reduce of the map "
                                        f"(rank 0 rows {state['slab']})") if world > 1 else "1 GPU"},
