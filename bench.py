@@ -48,7 +48,7 @@ UNIT = "evals/s"
 # by mlens_bench_dfma in the same run is reported beside it as `peak_measured_dfma`.
 FP64_LANES_PER_SM = 64
 # dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/r01d_ncu_full.md: dram read + write of shoot_ipm_kernel, mean of the two launches of a map).
+# (profiles/r01e_launches.md: dram read + write of shoot_ipm_kernel, mean of the two launches of a map).
 NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.43e9
 
 
