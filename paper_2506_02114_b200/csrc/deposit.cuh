@@ -50,10 +50,6 @@ __device__ __forceinline__ void pix_add(const ShootDev &S, const Win &W, int px,
     if (W.w32 && lx < (unsigned)WX && ly < (unsigned)WY) shared_add64(W.w32, (int)(ly * WX + lx), v);
     else atomicAdd(&S.acc[(size_t)py * S.npix1 + px], v);
 }
-// diff[py][px] += v; the caller guarantees 0 <= px < npix1, 0 <= py < npix2
-__device__ __forceinline__ void diff_add(const ShootDev &S, int px, int py, unsigned long long v) {
-    if (v) atomicAdd(&S.diff[(size_t)py * S.npix1 + px], v);
-}
 __device__ __forceinline__ void flush_window(const ShootDev &S, const WarpShared &Ws, const Win &W) {
     const int lane = threadIdx.x & 31;
 #pragma unroll 4
