@@ -734,6 +734,15 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         const double x = fmin(0.5, 1.14 * S.rt / leaf_half_min);
         int q = (int)ceil(log(0.5 * S.eps_far) / log(x)) - 1 + 2;
         S.tq = q < 4 ? 4 : (q > TQMAX ? TQMAX : q);
+        // ... and the same rule for a tile in a larger leaf (tree level l): never more than in the smallest ones
+        for (int l = 0; l <= ML_MAXLEV; ++l) {
+            const double xl = fmin(0.5, 1.14 * S.rt / (f->root_half / (double)(1 << l)));
+            int ql = (int)ceil(log(0.5 * S.eps_far) / log(xl)) - 1 + 2;
+            ql = ql < 4 ? 4 : ql;
+            S.tq_lev[l] = (signed char)(ql > S.tq ? S.tq : ql);
+        }
+    } else {
+        for (int l = 0; l <= ML_MAXLEV; ++l) S.tq_lev[l] = (signed char)S.tq;       // MLENS_TILE_ORDER: one order everywhere
     }
     S.eps_star = 0.03 * f->eps * f->theta / (double)ML_NEAR;
     const int stepx = ipm ? TCX - 1 : TCX, stepy = ipm ? TCY - 1 : TCY;

@@ -49,7 +49,8 @@ struct ShootDev {
     int eval_mode;
     int ntx;                           // tiles along x1
     long long tile_row0, tile_rows;    // band of tile rows handled by this launch
-    int tq;                            // order of the tile series
+    int tq;                            // highest order of the tile series in this shoot (tiles in the smallest leaves)
+    signed char tq_lev[ML_MAXLEV + 1];  // order for a tile in a leaf of tree level l: larger leaves converge faster
     double eps_far, eps_star;          // truncation budgets of the tile series (absolute, units of theta)
     double rt, inv_rt;                 // radius of a ray tile (half its diagonal) and its reciprocal
     double a1_lin, a2_lin;             // inside the star disc w = (a1 x - Re alpha_star, a2 y - Im alpha_star): a = 1 - kappa +- gamma + kappa_star
@@ -69,7 +70,7 @@ struct WarpShared {
     double sx[NSLOT][ML_NEAR], sy[NSLOT][ML_NEAR], sm[NSLOT][ML_NEAR];   // direct stars (absolute positions, m theta^2)
     double2 e[ML_P1MAX];                                     // the leaf's derivative series (set-up scratch)
     uint32_t bx0[NSLOT], bx1[NSLOT], by0[NSLOT], by1[NSLOT];
-    int leaf[NSLOT], node[NSLOT], nd[NSLOT], mode[NSLOT];
+    int leaf[NSLOT], node[NSLOT], nd[NSLOT], mode[NSLOT], q[NSLOT];     // q: order of the slot's series
     double ctx[4];                                           // zt_x, zt_y, 1/rt, fast flag: what the set-up hands back
 };
 // ... plus what the IPM kernel needs for apportioning
@@ -101,9 +102,10 @@ __device__ __forceinline__ double warp_sum(double v) {
 __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &W, const TileCtx &C, int s, double rt) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
-    const int p = S.L.p, Q = S.tq;
+    const int p = S.L.p;
     const int leaf = W.leaf[s], node = W.node[s];
     const int lev = __ldg(&S.L.level[node]);
+    const int Q = S.tq_lev[min(lev, ML_MAXLEV)];
     const double half = S.L.root_half / (double)(1 << lev);
     const double cx = -S.L.root_half + (2.0 * __ldg(&S.L.ix[node]) + 1.0) * half;
     const double cy = -S.L.root_half + (2.0 * __ldg(&S.L.iy[node]) + 1.0) * half;
@@ -169,7 +171,7 @@ __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &
             int pos = __popc(dm & ((1u << k) - 1u));
             W.sx[s][pos] = x; W.sy[s][pos] = y; W.sm[s][pos] = m;
         }
-        if (k == 0) { W.nd[s] = __popc(dm); W.mode[s] = (tail <= S.eps_far) ? 0 : 1; }
+        if (k == 0) { W.nd[s] = __popc(dm); W.mode[s] = (tail <= S.eps_far) ? 0 : 1; W.q[s] = Q; }
         if (fm) {
             // FOLDJ series terms per pass: lane = star writes its terms, then the warp sums them over the stars
             for (int j0 = 0; j0 <= Q; j0 += FOLDJ) {
@@ -289,7 +291,7 @@ static __device__ __noinline__ double2 eval_one_ool(const ShootDev *Sp, const Wa
     }
     if (s >= 0 && T->mode[s] != 0) s = -1;
     if (s < 0) { *kind = -1; return alpha_fmm_global_ool(&Sp->L, x, y); }
-    const int Q = Sp->tq;
+    const int Q = T->q[s];
     double sr = T->t[s][Q].x, si = T->t[s][Q].y;
     for (int j = Q - 1; j >= 0; --j) {
         double2 c = T->t[s][j];
@@ -388,7 +390,7 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
         s = max(s, 0);
     }
     if (fastlane && F32) {
-        const int Q = S.tq;
+        const int Q = T.q[s];
         const double2 *t = T.t[s];
         const float uxf = (float)ux;
         float uyf[RPT], sr[RPT], si[RPT];
@@ -453,7 +455,7 @@ __device__ __forceinline__ void eval_rays(const ShootDev &S, const WarpShared &T
         }
     } else if (fastlane) {
         // the common case: the four rays in one leaf, RPT independent Horner chains share every coefficient load
-        const int Q = S.tq;
+        const int Q = T.q[s];
         const double2 *t = T.t[s];
         double sr[RPT], si[RPT];
         double2 c = t[Q];
