@@ -302,7 +302,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (fused evaluate + IPM deposit), DESIGN.md s7
     # Algorithmic work per lens-equation evaluation: the leaf's near-field list summed directly
     # (10 flop per star) + the leaf's order-p Taylor series by Horner (8 flop per term) + 10 flop macro and sheet.
-    # The kernel itself does less (it re-expands the series per 32x32-ray tile, order 12, and folds the distant
+    # The kernel itself does less (it re-expands the series per 32x32-ray tile, order 6-15 by geometry, and folds the distant
     # near-field stars into it): `flop_executed` counts what it really issues for the evaluation.
     st = state["ipm"]
     p = state["info"]["order"]
