@@ -314,7 +314,7 @@ static const int WB = 16;              // triangles per batch
 static const int EREC = 10;            // doubles per edge record
 static const int GIANT_STEPS = 1024;   // a triangle with more steps than this is not walked by one warp alone
 static const int GIANT_CHUNK = 512;    // but in chunks of this many steps, one warp each
-__global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_constant__ ShootDev S) {
+__global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_kernel(const __grid_constant__ ShootDev S) {
     __shared__ double er_s[WALK_WARPS][3 * WB][EREC];
     __shared__ double tr_s[WALK_WARPS][WB][8];           // local vertices, cs, (bx, by)
     double (*er)[EREC] = er_s[threadIdx.x >> 5];
