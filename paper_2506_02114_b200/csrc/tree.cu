@@ -204,7 +204,10 @@ __device__ __forceinline__ int count_in_cell(const TreeDev &T, int Q, int cx, in
 }
 
 // neighbours of every node of one level + the split decision
-__global__ void link_level_kernel(TreeDev T, int a, int b, int lev, int max_direct, int *flags, int *overflow) {
+// The nodes of level `lev` are [range[lev], range[lev+1]): the level sizes stay on the device while the tree is built
+// (the host launches every level with an upper bound of its size and reads the ranges back once).
+__global__ void link_level_kernel(TreeDev T, const int *range, int lev, int max_direct, int *flags, int *overflow) {
+    const int a = range[lev], b = range[lev + 1];
     int me = a + blockIdx.x * blockDim.x + threadIdx.x;
     if (me >= b) return;
     int ix = T.ix[me], iy = T.iy[me], P = T.parent[me];
@@ -234,13 +237,23 @@ __global__ void link_level_kernel(TreeDev T, int a, int b, int lev, int max_dire
     flags[me - a] = split;
 }
 
-__global__ void make_children_kernel(TreeDev T, int a, int b, int lev, const int *flags, const int *rank,
+// range[lev+2] = end of the next level: the split nodes' children, unless they would not fit the node arrays (then
+// nobody splits and *overflow is set: the host starts again with more room).
+__global__ void next_level_kernel(int *range, int lev, const int *nsplit, int cap, int *overflow) {
+    const int b = range[lev + 1];
+    long long nb = (long long)b + 4ll * (long long)(*nsplit);
+    if (nb > (long long)cap) { nb = b; atomicExch(overflow, 2); }
+    range[lev + 2] = (int)nb;
+}
+
+__global__ void make_children_kernel(TreeDev T, const int *range, int lev, const int *flags, const int *rank,
                                      const unsigned long long *keys) {
+    const int a = range[lev], b = range[lev + 1];
     int me = a + blockIdx.x * blockDim.x + threadIdx.x;
     if (me >= b) return;
     // flags were scanned in place into `rank`; a node splits iff rank[next] - rank[me] == 1, so the
     // caller passes the original flags separately
-    if (!flags[me - a]) { T.child0[me] = -1; return; }
+    if (!flags[me - a] || range[lev + 2] == b) { T.child0[me] = -1; return; }
     int c0 = b + 4 * rank[me - a];
     T.child0[me] = c0;
     int lo = T.lo[me], n = T.n[me];
@@ -402,55 +415,69 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     }
     const unsigned long long *keys = k0.p;   // sorted keys
 
-    // ---- levels
-    size_t cap = (size_t)n + 1024;
-    ML_TRY(reserve_nodes(t, cap, s));
-    {
-        int h_root[7] = {0, 0, 0, -1, -1, 0, n};
-        ML_CUDA(cudaMemcpyAsync(t.level.p, &h_root[0], 4, cudaMemcpyHostToDevice, s));
-        ML_CUDA(cudaMemcpyAsync(t.ix.p, &h_root[1], 4, cudaMemcpyHostToDevice, s));
-        ML_CUDA(cudaMemcpyAsync(t.iy.p, &h_root[2], 4, cudaMemcpyHostToDevice, s));
-        ML_CUDA(cudaMemcpyAsync(t.parent.p, &h_root[3], 4, cudaMemcpyHostToDevice, s));
-        ML_CUDA(cudaMemcpyAsync(t.child0.p, &h_root[4], 4, cudaMemcpyHostToDevice, s));
-        ML_CUDA(cudaMemcpyAsync(t.lo.p, &h_root[5], 4, cudaMemcpyHostToDevice, s));
-        ML_CUDA(cudaMemcpyAsync(t.n.p, &h_root[6], 4, cudaMemcpyHostToDevice, s));
-        ML_CUDA(cudaStreamSynchronize(s));
-    }
-    DevBuf<int> flags, rank, d_over;
-    ML_TRY(d_over.reserve(1, s)); ML_CUDA(cudaMemsetAsync(d_over.p, 0, 4, s));
-    int a = 0, b = 1, lev = 0;
-    t.level_off[0] = 0;
-    while (true) {
-        int cnt = b - a;
-        t.level_off[lev + 1] = b;
-        ML_TRY(flags.reserve(cnt + 1, s, false)); ML_TRY(rank.reserve(cnt + 1, s, false));
-        ML_TRY(scratch.reserve(scan_scratch_ints(cnt + 1), s, false));
+    // ---- levels: the loop runs on the device's own counts.  Level l is launched with an upper bound of its size
+    // (four times the bound of the level above, at most the node capacity); the ranges come back once per chunk of
+    // levels -- log4(n) + 3 levels in the first chunk, which is all of them for any star field that is not clustered.
+    DevBuf<int> flags, rank, d_over, d_range;
+    ML_TRY(d_over.reserve(1, s)); ML_TRY(d_range.reserve(ML_MAXLEV + 3, s));
+    size_t cap = 2 * (size_t)n + 4096;
+    int h_range[ML_MAXLEV + 3];
+    for (;;) {                                                   // (again with more room if the nodes did not fit)
+        if (cap > 0x7ffffff0u) { set_error("tree too large"); return MLENS_ERANGE; }
+        ML_TRY(reserve_nodes(t, cap, s));
+        {
+            const int h_root[7] = {0, 0, 0, -1, -1, 0, n};
+            ML_CUDA(cudaMemcpyAsync(t.level.p, &h_root[0], 4, cudaMemcpyHostToDevice, s));
+            ML_CUDA(cudaMemcpyAsync(t.ix.p, &h_root[1], 4, cudaMemcpyHostToDevice, s));
+            ML_CUDA(cudaMemcpyAsync(t.iy.p, &h_root[2], 4, cudaMemcpyHostToDevice, s));
+            ML_CUDA(cudaMemcpyAsync(t.parent.p, &h_root[3], 4, cudaMemcpyHostToDevice, s));
+            ML_CUDA(cudaMemcpyAsync(t.child0.p, &h_root[4], 4, cudaMemcpyHostToDevice, s));
+            ML_CUDA(cudaMemcpyAsync(t.lo.p, &h_root[5], 4, cudaMemcpyHostToDevice, s));
+            ML_CUDA(cudaMemcpyAsync(t.n.p, &h_root[6], 4, cudaMemcpyHostToDevice, s));
+            for (int l = 0; l < ML_MAXLEV + 3; ++l) h_range[l] = (l == 0) ? 0 : 1;      // level 0 = [0, 1); nothing below yet
+            ML_CUDA(cudaMemcpyAsync(d_range.p, h_range, sizeof(h_range), cudaMemcpyHostToDevice, s));
+            ML_CUDA(cudaMemsetAsync(d_over.p, 0, 4, s));
+        }
         TreeDev T{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, t.nbr.p, f->sqx.p, f->sqy.p};
-        ML_LAUNCH(link_level_kernel, (cnt + 127) / 128, 128, 0, s, T, a, b, lev, f->max_direct, flags.p, d_over.p);
-        ML_CUDA(cudaMemcpyAsync(rank.p, flags.p, (size_t)cnt * 4, cudaMemcpyDeviceToDevice, s));
-        ML_CUDA(cudaMemsetAsync(rank.p + cnt, 0, 4, s));
-        ML_TRY(exclusive_scan(rank.p, cnt + 1, scratch.p, s));
-        int nsplit = 0;
-        ML_CUDA(cudaMemcpyAsync(&nsplit, rank.p + cnt, 4, cudaMemcpyDeviceToHost, s));
-        ML_CUDA(cudaStreamSynchronize(s));
-        if ((size_t)b + 4 * (size_t)nsplit > 0x7ffffff0u) { set_error("tree too large"); return MLENS_ERANGE; }
-        ML_TRY(reserve_nodes(t, (size_t)b + 4 * (size_t)nsplit + 1, s));
-        TreeDev T2{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, t.nbr.p, f->sqx.p, f->sqy.p};
-        ML_LAUNCH(make_children_kernel, (cnt + 127) / 128, 128, 0, s, T2, a, b, lev, flags.p, rank.p, keys);
-        ML_CUDA(cudaGetLastError());
-        if (nsplit == 0) break;
-        a = b; b = b + 4 * nsplit; ++lev;
+        int lev = 0, h_over = 0, n_levels = 0;
+        long long ub = 1;                                        // upper bound of the size of level `lev`
+        int chunk = 3;
+        for (long long q = 1; q < (long long)n; q *= 4) ++chunk;
+        while (n_levels == 0) {
+            const int lev_end = (lev + chunk < ML_MAXLEV + 1) ? lev + chunk : ML_MAXLEV + 1;
+            for (; lev < lev_end; ++lev) {
+                const int u = (int)ub;
+                ML_TRY(flags.reserve((size_t)u + 1, s, false)); ML_TRY(rank.reserve((size_t)u + 1, s, false));
+                ML_TRY(scratch.reserve(scan_scratch_ints((size_t)u + 1), s, false));
+                ML_CUDA(cudaMemsetAsync(flags.p, 0, ((size_t)u + 1) * 4, s));
+                ML_LAUNCH(link_level_kernel, (u + 127) / 128, 128, 0, s, T, d_range.p, lev, f->max_direct, flags.p, d_over.p);
+                ML_CUDA(cudaMemcpyAsync(rank.p, flags.p, ((size_t)u + 1) * 4, cudaMemcpyDeviceToDevice, s));
+                ML_TRY(exclusive_scan(rank.p, u + 1, scratch.p, s));
+                ML_LAUNCH(next_level_kernel, 1, 1, 0, s, d_range.p, lev, rank.p + u, (int)cap, d_over.p);
+                ML_LAUNCH(make_children_kernel, (u + 127) / 128, 128, 0, s, T, d_range.p, lev, flags.p, rank.p, keys);
+                ub = (4 * ub < (long long)cap) ? 4 * ub : (long long)cap;
+            }
+            ML_CUDA(cudaGetLastError());
+            ML_CUDA(cudaMemcpyAsync(h_range, d_range.p, sizeof(h_range), cudaMemcpyDeviceToHost, s));
+            ML_CUDA(cudaMemcpyAsync(&h_over, d_over.p, 4, cudaMemcpyDeviceToHost, s));
+            ML_CUDA(cudaStreamSynchronize(s));
+            if (h_over) break;
+            for (int l = 0; l < lev; ++l)
+                if (h_range[l + 2] == h_range[l + 1]) { n_levels = l + 1; break; }       // level l split nobody: it is the last
+            if (n_levels == 0 && lev > ML_MAXLEV) n_levels = ML_MAXLEV + 1;
+            if (n_levels == 0) { ub = h_range[lev + 1] - h_range[lev]; chunk = 4; }       // go on from the true size of the next level
+        }
+        if (h_over == 1) {
+            set_error("more than max_direct stars within one cell of the deepest tree level (%d)", ML_MAXLEV);
+            return MLENS_ERANGE;
+        }
+        if (h_over == 2) { cap *= 2; continue; }
+        t.n_levels = n_levels;
+        for (int l = 0; l <= n_levels; ++l) t.level_off[l] = h_range[l];
+        t.n_nodes = h_range[n_levels];
+        break;
     }
-    t.n_levels = lev + 1;
-    t.n_nodes = b;
-    int h_over = 0;
-    ML_CUDA(cudaMemcpyAsync(&h_over, d_over.p, 4, cudaMemcpyDeviceToHost, s));
-    ML_CUDA(cudaStreamSynchronize(s));
-    d_over.release();
-    if (h_over) {
-        set_error("more than max_direct stars within one cell of the deepest tree level (%d)", ML_MAXLEV);
-        return MLENS_ERANGE;
-    }
+    d_over.release(); d_range.release();
 
     // ---- leaves and lists
     const int nn = t.n_nodes;
