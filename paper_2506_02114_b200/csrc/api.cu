@@ -257,7 +257,8 @@ int mlens_field_destroy(mlens_field *f) {
     if (!f) return MLENS_OK;
     cudaDeviceSynchronize();
     f->ox.release(); f->oy.release(); f->om.release(); f->sx.release(); f->sy.release(); f->sm.release();
-    f->sqx.release(); f->sqy.release(); f->binom.release(); f->tab.release(); f->acc.release(); f->diff.release();
+    f->sqx.release(); f->sqy.release(); f->acc.release(); f->diff.release();
+    f->binom.p = nullptr; f->tab.p = nullptr;                     // borrowed from the per-device tables (fmm.cu)
     scratch_park(f);
     f->queue.release(); f->qcount.release(); f->biglist.release(); f->giant.release(); f->counters.release();
     f->tree.release();

@@ -3,6 +3,7 @@
 // All coefficients are in units of the node half-length.  c_0 and every logarithm are
 // dropped: they never enter a deflection (reading G1).
 #include "device.cuh"
+#include <mutex>
 
 namespace ml {
 
@@ -13,7 +14,9 @@ static const int TAB_M2L = 8;                  // 49 rows: (-1/z0)^n, z0 = 2(dx 
 static const int TAB_ROWS = 8 + 49;
 static const int BN = 2 * ML_P1MAX;            // Pascal triangle stride
 
-int fmm_prepare_tables(mlens_field *f, cudaStream_t s) {
+// The tables depend on nothing but compile-time constants: they are built and uploaded once per device and process,
+// and every field borrows them (mlens_field_destroy does not free them).
+static int build_tables(DevBuf<double> &binom, DevBuf<double2> &tabd, cudaStream_t s) {
     std::vector<double> bin((size_t)BN * BN, 0.0);
     for (int n = 0; n < BN; ++n) {
         bin[(size_t)n * BN] = 1.0;
@@ -36,11 +39,24 @@ int fmm_prepare_tables(mlens_field *f, cudaStream_t s) {
             if (dx || dy) { double2 z0 = make_double2(2.0 * dx, 2.0 * dy); w = cinv(z0); w.x = -w.x; w.y = -w.y; }
             for (int n = 0; n < ML_P1MAX; ++n) tab[(size_t)row * ML_P1MAX + n] = cpowi(w, n);
         }
-    ML_TRY(f->binom.reserve(bin.size(), s, false));
-    ML_TRY(f->tab.reserve(tab.size(), s, false));
-    ML_CUDA(cudaMemcpyAsync(f->binom.p, bin.data(), bin.size() * sizeof(double), cudaMemcpyHostToDevice, s));
-    ML_CUDA(cudaMemcpyAsync(f->tab.p, tab.data(), tab.size() * sizeof(double2), cudaMemcpyHostToDevice, s));
+    ML_TRY(binom.reserve(bin.size(), s, false));
+    ML_TRY(tabd.reserve(tab.size(), s, false));
+    ML_CUDA(cudaMemcpyAsync(binom.p, bin.data(), bin.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+    ML_CUDA(cudaMemcpyAsync(tabd.p, tab.data(), tab.size() * sizeof(double2), cudaMemcpyHostToDevice, s));
     ML_CUDA(cudaStreamSynchronize(s));
+    return MLENS_OK;
+}
+
+int fmm_prepare_tables(mlens_field *f, cudaStream_t s) {
+    static const int MAXDEV = 64;
+    static std::mutex mtx;
+    static DevBuf<double> c_binom[MAXDEV];
+    static DevBuf<double2> c_tab[MAXDEV];
+    if (f->device < 0 || f->device >= MAXDEV) { set_error("device index out of range"); return MLENS_EINVAL; }
+    std::lock_guard<std::mutex> lock(mtx);
+    if (!c_binom[f->device].p || !c_tab[f->device].p) ML_TRY(build_tables(c_binom[f->device], c_tab[f->device], s));
+    f->binom.p = c_binom[f->device].p; f->binom.cap = 0;          // borrowed
+    f->tab.p = c_tab[f->device].p; f->tab.cap = 0;
     return MLENS_OK;
 }
 

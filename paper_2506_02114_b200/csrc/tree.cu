@@ -281,6 +281,11 @@ __global__ void make_children_kernel(TreeDev T, const int *range, int lev, const
     }
 }
 
+__global__ void init_tree_kernel(int *level, int *ix, int *iy, int *parent, int *child0, int *lo, int *nn, int n, int *range, int nr) {
+    if (threadIdx.x == 0) { level[0] = 0; ix[0] = 0; iy[0] = 0; parent[0] = -1; child0[0] = -1; lo[0] = 0; nn[0] = n; }
+    for (int l = threadIdx.x; l < nr; l += blockDim.x) range[l] = (l == 0) ? 0 : 1;
+}
+
 __global__ void leaf_flag_kernel(const int *child0, int n, int *flag) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) flag[i] = child0[i] < 0;
@@ -426,16 +431,10 @@ int build_tree(mlens_field *f, cudaStream_t s) {
         if (cap > 0x7ffffff0u) { set_error("tree too large"); return MLENS_ERANGE; }
         ML_TRY(reserve_nodes(t, cap, s));
         {
-            const int h_root[7] = {0, 0, 0, -1, -1, 0, n};
-            ML_CUDA(cudaMemcpyAsync(t.level.p, &h_root[0], 4, cudaMemcpyHostToDevice, s));
-            ML_CUDA(cudaMemcpyAsync(t.ix.p, &h_root[1], 4, cudaMemcpyHostToDevice, s));
-            ML_CUDA(cudaMemcpyAsync(t.iy.p, &h_root[2], 4, cudaMemcpyHostToDevice, s));
-            ML_CUDA(cudaMemcpyAsync(t.parent.p, &h_root[3], 4, cudaMemcpyHostToDevice, s));
-            ML_CUDA(cudaMemcpyAsync(t.child0.p, &h_root[4], 4, cudaMemcpyHostToDevice, s));
-            ML_CUDA(cudaMemcpyAsync(t.lo.p, &h_root[5], 4, cudaMemcpyHostToDevice, s));
-            ML_CUDA(cudaMemcpyAsync(t.n.p, &h_root[6], 4, cudaMemcpyHostToDevice, s));
-            for (int l = 0; l < ML_MAXLEV + 3; ++l) h_range[l] = (l == 0) ? 0 : 1;      // level 0 = [0, 1); nothing below yet
-            ML_CUDA(cudaMemcpyAsync(d_range.p, h_range, sizeof(h_range), cudaMemcpyHostToDevice, s));
+            // root node, level ranges (level 0 = [0, 1), nothing below yet) and flags, written by a kernel: copies
+            // from pageable host memory would make the host wait for the sort
+            ML_LAUNCH(init_tree_kernel, 1, 32, 0, s, t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, n,
+                      d_range.p, ML_MAXLEV + 3);
             ML_CUDA(cudaMemsetAsync(d_over.p, 0, 4, s));
         }
         TreeDev T{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, t.nbr.p, f->sqx.p, f->sqy.p};
