@@ -271,3 +271,47 @@ def test_subrange_shoot_adds_up(orc):
     orc.shoot(f, geo, 0, sub=(0, geo.n1, 0, jm), out=acc)
     orc.shoot(f, geo, 0, sub=(0, geo.n1, jm, geo.n2), out=acc)
     assert np.allclose(acc, whole, rtol=1e-12, atol=1e-14)
+
+
+def test_degenerate_triangle_rule_G12(orc):
+    """Reading G12: a mapped triangle whose signed area is exactly 0 puts its whole
+    weight into the pixel that holds vertex 0, if that pixel is in the map, and nothing anywhere else; no division.
+    Hand-built corner grids (2 x 2 corners = one cell = T1 (a, b, c) + T2 (a, c, d)) whose images are collinear."""
+    g = orc.geometry(0.0, 0.0, 0.0, 4.0, 8, 1.0, 3, He=(1.0, 1.0))      # 8 x 8 pixels of size 1, lower-left (-4, -4)
+    assert (g.p1, g.p2, g.ylo1, g.ylo2) == (1.0, 1.0, -4.0, -4.0)
+    w = g.weight
+
+    def cell(a, b, c, d):
+        wx = np.array([[a[0], b[0]], [d[0], c[0]]]) + g.ylo1          # row 0 = corners (i, j), (i+1, j); row 1 = (i, j+1), (i+1, j+1)
+        wy = np.array([[a[1], b[1]], [d[1], c[1]]]) + g.ylo2
+        return orc.deposit_ipm(wx, wy, g)
+
+    # the cell collapsed onto a horizontal segment spanning three pixels: both triangles go to vertex a's pixel (2, 1)
+    m = cell((2.3, 1.4), (3.3, 1.4), (4.3, 1.4), (2.8, 1.4))
+    assert m[1, 2] == 2 * w and m.sum() == 2 * w
+    # onto a diagonal segment (exactly representable, A = 0 exactly): vertex a in pixel (0, 0)
+    m = cell((0.5, 0.5), (1.5, 1.5), (2.5, 2.5), (3.5, 3.5))
+    assert m[0, 0] == 2 * w and m.sum() == 2 * w
+    # onto a single point
+    m = cell((5.25, 6.75), (5.25, 6.75), (5.25, 6.75), (5.25, 6.75))
+    assert m[6, 5] == 2 * w and m.sum() == 2 * w
+    # only T1 degenerate (a, b, c collinear), T2 = (a, c, d) a proper triangle inside pixel (1, 1): 2 w in all, one of them by G12
+    m = cell((1.25, 1.25), (1.5, 1.5), (1.75, 1.75), (1.25, 1.75))
+    assert m[1, 1] == pytest.approx(2 * w, rel=1e-15) and m.sum() == pytest.approx(2 * w, rel=1e-15)
+    # T1 degenerate with vertex a in pixel (1, 1) but b, c elsewhere; T2 proper over pixels of row 1..2: the degenerate
+    # weight goes to a's pixel, not to where the segment's other end lies
+    m = cell((1.5, 1.5), (2.5, 1.5), (3.5, 1.5), (1.5, 2.5))
+    t2 = np.zeros_like(m)
+    for qy in range(8):
+        for qx in range(8):
+            t2[qy, qx] = w * orc.triangle_pixel_area([1.5, 1.5, 3.5, 1.5, 1.5, 2.5], qx, qy) / 1.0   # |A| = 1
+    assert np.allclose(m - t2, np.where((np.arange(8)[:, None] == 1) & (np.arange(8)[None, :] == 1), w, 0.0), atol=1e-16)
+    # vertex 0 outside the map (the segment itself crosses the map): nothing is deposited
+    m = cell((-0.5, 3.5), (2.5, 3.5), (5.5, 3.5), (1.5, 3.5))
+    assert m.sum() == 0.0
+    # ... and the conservation of a whole map is unchanged by degenerate cells: a grid folded flat along x2 = const
+    # (every cell degenerate) carries exactly 2 w per cell whose vertex a lies in the map
+    xs = np.linspace(-3.9, 3.9, 14)
+    wx = np.tile(xs, (5, 1)); wy = np.full((5, 14), 0.3)
+    m = orc.deposit_ipm(wx, wy, g)
+    assert m.sum() == pytest.approx(2 * w * 4 * 13, rel=1e-14) and np.count_nonzero(m[:4]) == 0 and np.count_nonzero(m[5:]) == 0
