@@ -124,6 +124,20 @@ typedef struct {
     double *dump_w1, *dump_w2;     /* optional: mapped ray positions of the sub-range, written by the SAME
                                       kernel that deposits them.  IPM: (j1-j0+1) x (i1-i0+1) corners;
                                       IRS: (j1-j0) x (i1-i0) centres; row-major, x1 fastest. May be NULL. */
+    /* Tuning knobs; 0 = the library's default everywhere.  None of them changes what is computed: a map is the
+     * same to the last bit for any setting except tile_order (which moves the rays within the tile series'
+     * truncation budget, 5 % of eps_deflection) and small_px (which selects between two exact area formulas). */
+    int32_t queue_mb;              /* size of the general-triangle queue in MiB (default: up to 8192) */
+    int32_t tile_order;            /* order of the per-tile series, 2..15 (default: chosen per shoot from the tile size) */
+    int32_t small_px;              /* queued triangles whose box holds more pixels than this are walked along their
+                                      edges instead of clipped pixel by pixel (default 24) */
+    int32_t band_fixed;            /* 1: IPM bands of exactly band_cells cells (default: sized from the measured rate
+                                      of general triangles per cell) */
+    int64_t band_cells;            /* upper bound of the cells per band (default 2^30) */
+    int32_t tile_traversal;        /* order in which a band's ray tiles are handed out: 0 = default (column-major:
+                                      the deposits of the tiles in flight stay within a patch of the map that L2
+                                      holds), 1 = row-major */
+    int32_t pad_;
 } mlens_shoot_desc;
 
 typedef struct {
@@ -189,7 +203,11 @@ int mlens_lens_map(const mlens_field *f, int64_t n, const double *zx, const doub
 int mlens_grid_info(const mlens_field *f, const mlens_shoot_desc *desc, mlens_grid *out);
 
 /* Shoots the (sub-range of the) ray grid and builds the map.  map: double[npix2*npix1] or NULL;
- * counts: uint64[npix2*npix1] (IRS ray counts) or NULL; stats may be NULL. */
+ * counts: uint64[npix2*npix1], the IRS ray counts, or NULL -- it must be NULL for MLENS_MAP_IPM (MLENS_EINVAL
+ * otherwise: an IPM map has no counts); stats may be NULL.
+ * Ray tiles are anchored on the GLOBAL cell grid, so a ray has the same value to the last bit in whatever
+ * sub-range it is shot, and the maps of sub-ranges that tile the grid add up to the map of the whole grid
+ * exactly (integer accumulation): row slabs on several GPUs reproduce the one-GPU map bit for bit. */
 int mlens_shoot(mlens_field *f, const mlens_shoot_desc *desc, double *map, uint64_t *counts,
                 mlens_stats *stats, void *stream);
 
@@ -228,11 +246,6 @@ int mlens_map_light_curve(const double *map, int32_t npix1, int32_t npix2, doubl
  * 1 <= nbins <= 4096, n = number of pixels, mu_ref > 0, hi > lo. */
 int mlens_map_histogram(const double *map, int64_t n, double mu_ref, double lo, double hi, int32_t nbins,
                         uint64_t *counts, int32_t ptr_kind, void *stream);
-
-/* Micro-benchmarks for the roofline denominators: sustained FP64 FMA rate [FLOP/s]
- * and FP64/u64 global atomic-add rate [adds/s] into a buffer of `n_slots` 8-byte slots. */
-int mlens_bench_dfma(double *flops_per_s, void *stream);
-int mlens_bench_atomics(int64_t n_slots, int32_t use_u64, double *adds_per_s, void *stream);
 
 #ifdef __cplusplus
 }

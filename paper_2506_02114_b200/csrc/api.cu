@@ -16,15 +16,16 @@ void set_error(const char *fmt, ...) {
 }
 
 int pool_init() {
-    static std::atomic<int> done{0};
-    if (done.load()) return MLENS_OK;
+    static std::atomic<int> done[ML_MAXDEV];                        // per device (zero-initialised)
     int dev = 0;
     ML_CUDA(cudaGetDevice(&dev));
+    const int slot = device_slot();
+    if (done[slot].load()) return MLENS_OK;
     cudaMemPool_t pool;
     ML_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
     unsigned long long keep = ~0ull;
     ML_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-    done.store(1);
+    done[slot].store(1);
     return MLENS_OK;
 }
 
@@ -104,7 +105,7 @@ __global__ void max_diff_kernel(const double *ax, const double *ay, const double
 
 static int spot_check(mlens_field *f, cudaStream_t s, double *err) {
     const int NP = 1024;
-    DevBuf<double> b; DevBuf<unsigned long long> bits;
+    ScratchBuf<double> b; ScratchBuf<unsigned long long> bits;
     ML_TRY(b.reserve(6 * NP, s, false)); ML_TRY(bits.reserve(1, s, false));
     double *zx = b.p, *zy = b.p + NP, *ax = b.p + 2 * NP, *ay = b.p + 3 * NP, *bx = b.p + 4 * NP, *by = b.p + 5 * NP;
     double leaf_half = f->root_half / (double)(1 << (f->tree.n_levels - 1));
@@ -191,6 +192,7 @@ int mlens_field_create(const mlens_field_desc *d, mlens_field **out) {
     f->max_direct = (d->max_direct > 0) ? d->max_direct : MLENS_MAX_DIRECT;
     f->n_stars = d->n_stars;
     cudaGetDevice(&f->device);
+    f->last_stream = s;
     int rc = MLENS_OK;
     size_t n = (size_t)d->n_stars;
     cudaMemcpyKind kind = d->ptr_kind == MLENS_PTR_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
@@ -228,6 +230,7 @@ int mlens_field_create_seeded(const mlens_seed_desc *d, mlens_field **out) {
     f->max_direct = (d->max_direct > 0) ? d->max_direct : MLENS_MAX_DIRECT;
     f->n_stars = d->n_stars;
     cudaGetDevice(&f->device);
+    f->last_stream = s;
     // eq 9 with <m> = 1: area = pi theta^2 N / kappa_star
     double a1, a2 = 0.0;
     if (d->shape == MLENS_SHAPE_DISC) {
@@ -253,15 +256,22 @@ int mlens_field_create_seeded(const mlens_seed_desc *d, mlens_field **out) {
     return MLENS_OK;
 }
 
+// Everything a field owns is freed in stream order on the stream of the field's most recent call: no device-wide
+// synchronisation.  (A caller that used the field on several streams orders them before destroying it, as for
+// any other stream-ordered resource.)
 int mlens_field_destroy(mlens_field *f) {
     if (!f) return MLENS_OK;
-    cudaDeviceSynchronize();
-    f->ox.release(); f->oy.release(); f->om.release(); f->sx.release(); f->sy.release(); f->sm.release();
-    f->sqx.release(); f->sqy.release(); f->acc.release(); f->diff.release();
+    int cur = 0;
+    cudaGetDevice(&cur);
+    if (cur != f->device) cudaSetDevice(f->device);
+    cudaStream_t s = f->last_stream;
+    f->ox.release(s); f->oy.release(s); f->om.release(s); f->sx.release(s); f->sy.release(s); f->sm.release(s);
+    f->sqx.release(s); f->sqy.release(s); f->acc.release(s); f->diff.release(s);
     f->binom.p = nullptr; f->tab.p = nullptr;                     // borrowed from the per-device tables (fmm.cu)
-    scratch_park(f);
-    f->queue.release(); f->qcount.release(); f->biglist.release(); f->giant.release(); f->counters.release();
-    f->tree.release();
+    scratch_park(f, s);
+    f->queue.release(s); f->qcount.release(s); f->biglist.release(s); f->giant.release(s); f->counters.release(s);
+    f->tree.release(s);
+    if (cur != f->device) cudaSetDevice(cur);
     delete f;
     return MLENS_OK;
 }
@@ -300,6 +310,7 @@ static int points_call(const mlens_field *f, int64_t n, const double *zx, const 
     if (!f || n < 0 || (n > 0 && (!zx || !zy || !ox || !oy))) { set_error("bad arguments"); return MLENS_EINVAL; }
     if (eval_mode != MLENS_EVAL_FMM && eval_mode != MLENS_EVAL_DIRECT) { set_error("bad eval mode"); return MLENS_EINVAL; }
     cudaStream_t s = (cudaStream_t)stream;
+    const_cast<mlens_field *>(f)->last_stream = s;
     Stage st(s);
     const double *dzx, *dzy; double *dox, *doy;
     ML_TRY(st.in(zx, (size_t)n, ptr_kind, s, &dzx)); ML_TRY(st.in(zy, (size_t)n, ptr_kind, s, &dzy));
@@ -328,9 +339,11 @@ int mlens_shoot(mlens_field *f, const mlens_shoot_desc *d, double *map, uint64_t
     if (!f || !d) { set_error("null argument"); return MLENS_EINVAL; }
     if (d->map_mode != MLENS_MAP_IPM && d->map_mode != MLENS_MAP_IRS) { set_error("bad map mode"); return MLENS_EINVAL; }
     if (d->eval_mode != MLENS_EVAL_FMM && d->eval_mode != MLENS_EVAL_DIRECT && d->eval_mode != MLENS_EVAL_FMM_F32) { set_error("bad eval mode"); return MLENS_EINVAL; }
+    if (d->map_mode == MLENS_MAP_IPM && counts) { set_error("an IPM map has no ray counts: counts must be NULL"); return MLENS_EINVAL; }
     mlens_grid g;
     ML_TRY(geometry(f, d, &g));
     cudaStream_t s = (cudaStream_t)stream;
+    f->last_stream = s;
     size_t npix = (size_t)d->npix1 * d->npix2;
     Stage st(s);
     double *dmap = nullptr; unsigned long long *dcnt = nullptr;
@@ -396,7 +409,7 @@ int mlens_map_histogram(const double *map, int64_t n, double mu_ref, double lo, 
 
 int mlens_field_get_tree(const mlens_field *f, mlens_tree_view *v) {
     if (!f || !v) { set_error("null argument"); return MLENS_EINVAL; }
-    ML_CUDA(cudaDeviceSynchronize());
+    ML_CUDA(cudaStreamSynchronize(f->last_stream));
     const Tree &t = f->tree;
     size_t nn = (size_t)t.n_nodes, nl = (size_t)t.n_leaves, p1 = (size_t)f->order + 1, ns = (size_t)f->n_stars;
 #define CP(dst, src, count) if (dst && (count)) ML_CUDA(cudaMemcpy(dst, src, (count) * sizeof(*(dst)), cudaMemcpyDeviceToHost))
@@ -410,74 +423,6 @@ int mlens_field_get_tree(const mlens_field *f, mlens_tree_view *v) {
     CP(v->near_x, t.near_x.p, nl * ML_NEAR); CP(v->near_y, t.near_y.p, nl * ML_NEAR); CP(v->near_m, t.near_m.p, nl * ML_NEAR);
     CP(v->sorted_x, f->sx.p, ns); CP(v->sorted_y, f->sy.p, ns); CP(v->sorted_m, f->sm.p, ns);
 #undef CP
-    return MLENS_OK;
-}
-
-// ---- roofline denominators -------------------------------------------------------------------
-__global__ void dfma_kernel(double *out, int iters) {
-    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-    const double b = 1.0000001, c = 1e-9;
-    for (int i = 0; i < iters; ++i) {
-        a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
-        a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
-    }
-    double r = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-    if (r == 123.456) out[0] = r;
-}
-
-int mlens_bench_dfma(double *flops_per_s, void *stream) {
-    if (!flops_per_s) return MLENS_EINVAL;
-    ML_TRY(check_device());
-    cudaStream_t s = (cudaStream_t)stream;
-    int nsm = 148; cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
-    double *d = nullptr; ML_CUDA(cudaMalloc(&d, 8));
-    const int iters = 1 << 15, blocks = nsm * 8, threads = 256;
-    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    ML_LAUNCH(dfma_kernel, blocks, threads, 0, s, d, 1024);
-    float best = 1e30f;
-    for (int r = 0; r < 5; ++r) {
-        cudaEventRecord(e0, s);
-        ML_LAUNCH(dfma_kernel, blocks, threads, 0, s, d, iters);
-        cudaEventRecord(e1, s);
-        ML_CUDA(cudaEventSynchronize(e1));
-        float ms; cudaEventElapsedTime(&ms, e0, e1);
-        if (ms < best) best = ms;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
-    *flops_per_s = 2.0 * 8.0 * (double)iters * blocks * threads / (best * 1e-3);
-    return MLENS_OK;
-}
-
-__global__ void atomics_kernel(unsigned long long *bu, double *bd, long long n_slots, int use_u64, int per_thread) {
-    unsigned long long h = (blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x + 1) * 0x9E3779B97F4A7C15ull;
-    for (int i = 0; i < per_thread; ++i) {
-        h ^= h >> 29; h *= 0xBF58476D1CE4E5B9ull; h ^= h >> 32;
-        long long slot = (long long)(h % (unsigned long long)n_slots);
-        if (use_u64) atomicAdd(&bu[slot], 1ull); else atomicAdd(&bd[slot], 1.0);
-    }
-}
-
-int mlens_bench_atomics(int64_t n_slots, int32_t use_u64, double *adds_per_s, void *stream) {
-    if (!adds_per_s || n_slots <= 0) return MLENS_EINVAL;
-    ML_TRY(check_device());
-    cudaStream_t s = (cudaStream_t)stream;
-    void *buf = nullptr; ML_CUDA(cudaMalloc(&buf, (size_t)n_slots * 8));
-    ML_CUDA(cudaMemsetAsync(buf, 0, (size_t)n_slots * 8, s));
-    int nsm = 148; cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
-    const int blocks = nsm * 16, threads = 256, per = 256;
-    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    ML_LAUNCH(atomics_kernel, blocks, threads, 0, s, (unsigned long long *)buf, (double *)buf, n_slots, use_u64, 8);
-    float best = 1e30f;
-    for (int r = 0; r < 3; ++r) {
-        cudaEventRecord(e0, s);
-        ML_LAUNCH(atomics_kernel, blocks, threads, 0, s, (unsigned long long *)buf, (double *)buf, n_slots, use_u64, per);
-        cudaEventRecord(e1, s);
-        ML_CUDA(cudaEventSynchronize(e1));
-        float ms; cudaEventElapsedTime(&ms, e0, e1);
-        if (ms < best) best = ms;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
-    *adds_per_s = (double)blocks * threads * per / (best * 1e-3);
     return MLENS_OK;
 }
 

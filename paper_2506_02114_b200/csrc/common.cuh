@@ -46,12 +46,25 @@ extern std::atomic<long long> g_launches;
 // what is freed: creating and destroying fields in a loop then costs no driver allocation at all.
 int pool_init();
 
-// Growable device array that keeps its contents on reserve().
+// One-time set-ups (memory-pool threshold, kernel attributes) are per DEVICE, not per process: a process may drive
+// several GPUs.  Returns the current device's slot in such tables.
+static const int ML_MAXDEV = 64;
+inline int device_slot() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return (dev >= 0 && dev < ML_MAXDEV) ? dev : ML_MAXDEV - 1;
+}
+
+// Growable device array that keeps its contents on reserve().  Memory is stream-ordered: `s_own` is the stream of
+// the last reserve (all of the library's work on a buffer is enqueued on the caller's stream), and a release is
+// ordered after the work already enqueued there -- no device-wide synchronisation anywhere.
 template <typename T>
 struct DevBuf {
     T *p = nullptr;
     size_t cap = 0;
+    cudaStream_t s_own = nullptr;
     int reserve(size_t n, cudaStream_t s, bool keep = true) {
+        s_own = s;
         if (n <= cap) return MLENS_OK;
         ML_TRY(pool_init());
         size_t ncap = n + n / 4 + 64;
@@ -62,8 +75,16 @@ struct DevBuf {
         p = q; cap = ncap;
         return MLENS_OK;
     }
-    // callers synchronise the streams that used the buffer before releasing it
-    void release() { if (p) cudaFreeAsync(p, 0); p = nullptr; cap = 0; }
+    void release(cudaStream_t s) { if (p) cudaFreeAsync(p, s); p = nullptr; cap = 0; }
+    void release() { release(s_own); }
+};
+// Local scratch of a host function: freed (stream-ordered) on every way out of the scope, early returns included.
+template <typename T>
+struct ScratchBuf : DevBuf<T> {
+    ScratchBuf() = default;
+    ScratchBuf(const ScratchBuf &) = delete;
+    ScratchBuf &operator=(const ScratchBuf &) = delete;
+    ~ScratchBuf() { this->release(); }
 };
 
 struct Tree {
@@ -76,7 +97,7 @@ struct Tree {
     DevBuf<int> near_cnt;                        // n_leaves
     DevBuf<double> near_x, near_y, near_m;       // n_leaves * ML_NEAR
     DevBuf<double2> ecoef;                       // n_leaves * P1: (l+1) c_{l+1} theta^2/L, l = 0..p-1
-    void release();
+    void release(cudaStream_t s);
 };
 
 }  // namespace ml
@@ -110,6 +131,7 @@ struct mlens_field {
     ml::DevBuf<unsigned long long> giant; // chunks of the giant triangles among them
     ml::DevBuf<unsigned long long> counters;
     int device = 0;
+    cudaStream_t last_stream = nullptr;   // stream of the most recent call on this field: destroy frees in its order
 };
 
 namespace ml {
@@ -126,10 +148,10 @@ int generate_stars(uint64_t seed, int64_t n, int shape, double a1, double a2, in
                    double lo, double hi, double *x, double *y, double *m, cudaStream_t s);
 // shoot.cu
 // The general-triangle queue is gigabytes of scratch that belongs to no field in particular: a destroyed field
-// parks it here (after the device has been synchronised) and the next field that shoots on that device takes it,
+// parks it here (with an event on its stream) and the next field that shoots on that device takes it (after the event),
 // so that creating and destroying fields in a loop never allocates it again.
-void scratch_park(mlens_field *f);
-void scratch_take(mlens_field *f);
+void scratch_park(mlens_field *f, cudaStream_t s);
+void scratch_take(mlens_field *f, cudaStream_t s);
 int geometry(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid *g);
 int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double *map,
           unsigned long long *counts, mlens_stats *st, cudaStream_t s);

@@ -65,10 +65,10 @@ int map_histogram(const double *map, long long n, const double *edges_dev, int n
     int rep = 16;                                                  // copies of every counter: as many as 48 KB allow
     while (rep > 1 && (size_t)(nbins + 1) * 8 + (size_t)(nbins + 2) * 4 * rep > 48 * 1024) rep >>= 1;
     const size_t smem = (size_t)(nbins + 1) * 8 + (size_t)(nbins + 2) * 4 * rep;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static std::atomic<int> attr_set[ML_MAXDEV];                   // kernel attributes are per device (context)
+    if (!attr_set[device_slot()].load()) {
         ML_CUDA(cudaFuncSetAttribute(histogram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (HIST_MAXBINS + 1) * 8 + (HIST_MAXBINS + 2) * 4));
-        attr_set = true;
+        attr_set[device_slot()].store(1);
     }
     if (n / grid >= (1ll << 32)) { set_error("map too large for the histogram's 32-bit block counters"); return MLENS_EINVAL; }
     ML_LAUNCH(histogram_kernel, grid, HIST_T, smem, s, map, n, edges_dev, nbins, rep, counts);

@@ -12,7 +12,8 @@
 //     and dy of every pixel to its right in row j (m = mean x of the piece within the pixel), i.e.
 //     diff[j][i] += c dy (1 - m), diff[j][i+1] += c dy m  with c = -sign(A) ONE/|A|.  The three edges' covers
 //     cancel to the right of the triangle; they cancel EXACTLY because c dy is computed as G(y_end) - G(y_start)
-//     with G(y) = round(c y) evaluated on values shared by consecutive pieces (vertices, grid lines).
+//     with G(y) = round(c y) evaluated on values shared by consecutive pieces (vertices, grid lines, and the exact
+//     row line where the first or last row of the map cuts an edge).
 //     Cost is proportional to the triangle's perimeter in pixels, never to its area, and the result is the same
 //     area of intersection as clipping every pixel, up to rounding.
 #pragma once
@@ -118,19 +119,19 @@ struct EdgeWalk {                     // one triangle edge, clipped to the map r
     double g0, sg;                    // first grid line crossed along the major axis and the step (+-1)
     int majorY;                       // 1: walk rows (|dy| >= |dx|), 0: walk columns
     int n;                            // steps = crossings of major-axis grid lines + 1, or 0
+    int cf;                           // ends cut by a border row of the map: bits 0-1 the start (1: row line ry0, 2: ry1), bits 2-3 the end
 };
 
 // local coordinates: pixel units relative to the integer point (bx, by); rows [ry0, ry1] and columns <= cx1 are the map
 __device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, double x1, double y1, double ry0, double ry1, double cx1) {
     E.x0 = x0; E.y0 = y0; E.x1 = x1; E.y1 = y1; E.dx = x1 - x0; E.dy = y1 - y0;
-    E.n = 0; E.ta = 0.0; E.tb = 1.0; E.idx = 0.0; E.idy = 0.0; E.g0 = 0.0; E.sg = 1.0; E.majorY = 1;
+    E.n = 0; E.ta = 0.0; E.tb = 1.0; E.idx = 0.0; E.idy = 0.0; E.g0 = 0.0; E.sg = 1.0; E.majorY = 1; E.cf = 0;
     if (E.dy == 0.0) return;                                   // a horizontal edge covers nothing
     E.idy = 1.0 / E.dy;
     double ta = 0.0, tb = 1.0;
-    {
-        double t0 = (ry0 - y0) * E.idy, t1 = (ry1 - y0) * E.idy;
-        ta = fmax(ta, fmin(t0, t1)); tb = fmin(tb, fmax(t0, t1));
-    }
+    const double t0 = (ry0 - y0) * E.idy, t1 = (ry1 - y0) * E.idy;
+    const double tlo = fmin(t0, t1), thi = fmax(t0, t1);       // where the edge enters and leaves the rows of the map
+    ta = fmax(ta, tlo); tb = fmin(tb, thi);
     if (E.dx != 0.0) {
         E.idx = 1.0 / E.dx;
         double tc = (cx1 - x0) * E.idx;
@@ -138,9 +139,20 @@ __device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, do
     } else if (x0 >= cx1) return;
     if (!(tb > ta)) return;
     E.ta = ta; E.tb = tb;
+    // An end cut by a border row of the map lies ON that row line: it takes the line's exact (integer) value of y,
+    // as the ends on grid lines and vertices do, so that the covers G(y) of all the edges that cross the border
+    // telescope there too.  (A row line cuts an edge strictly inside only if it is the map's first or last one.)
+    int cf = 0;
+    if (ta == tlo && ta > 0.0) cf |= (E.dy > 0.0) ? 1 : 2;
+    if (tb == thi && tb < 1.0) cf |= (E.dy > 0.0) ? 8 : 4;
+    E.cf = cf;
     E.majorY = fabs(E.dy) >= fabs(E.dx);
     const double d = E.majorY ? E.dy : E.dx, c0 = E.majorY ? y0 : x0;
-    const double a = fma(ta, d, c0), b = fma(tb, d, c0);       // major coordinate at the clipped ends
+    double a = fma(ta, d, c0), b = fma(tb, d, c0);             // major coordinate at the clipped ends
+    if (E.majorY) {
+        if (cf & 3) a = (cf & 1) ? ry0 : ry1;
+        if (cf & 12) b = (cf & 4) ? ry0 : ry1;
+    }
     double nc;
     if (d > 0.0) { E.sg = 1.0; E.g0 = floor(a) + 1.0; nc = ceil(b) - 1.0 - floor(a); }
     else { E.sg = -1.0; E.g0 = ceil(a) - 1.0; nc = ceil(a) - 1.0 - floor(b); }
@@ -176,17 +188,26 @@ __device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, doub
 // coordinates: c0 -> c1 along the axis that is walked, oc0 -> o1 along the other, id / oid the reciprocals of the
 // two extents (0 for an extent of 0), [ta, tb] the clipped parameter range, g0 the first grid line, sg the direction.
 __device__ __forceinline__ void edge_step_mo(const ShootDev &S, double c0, double oc0, double c1, double o1, double id, double oid,
-                                             double ta, double tb, double g0, double sg, bool my, int n, int k,
+                                             double ta, double tb, double g0, double sg, bool my, int cf, int n, int k,
                                              double cs, int bx, int by) {
     const double d = c1 - c0, od = o1 - oc0;
     double ms, os, me, oe, ts, te;
-    if (k == 0) { ts = ta; ms = (ts == 0.0) ? c0 : fma(ts, d, c0); os = (ts == 0.0) ? oc0 : fma(ts, od, oc0); }
-    else { ms = g0 + sg * (double)(k - 1); ts = dmin(dmax((ms - c0) * id, ta), tb); os = fma(ts, od, oc0); }
+    if (k == 0) {
+        ts = ta; ms = (ts == 0.0) ? c0 : fma(ts, d, c0); os = (ts == 0.0) ? oc0 : fma(ts, od, oc0);
+        if (cf & 3) {                                          // start on a border row of the map: exactly on it
+            const double yl = (cf & 1) ? (double)(-by) : (double)(S.npix2 - by);
+            if (my) ms = yl; else os = yl;
+        }
+    } else { ms = g0 + sg * (double)(k - 1); ts = dmin(dmax((ms - c0) * id, ta), tb); os = fma(ts, od, oc0); }
     if (k == n - 1) {
         te = tb;
         const bool vtx = (te == 1.0);
         me = vtx ? c1 : fma(te, d, c0);
         oe = vtx ? o1 : fma(te, od, oc0);
+        if (cf & 12) {
+            const double yl = (cf & 4) ? (double)(-by) : (double)(S.npix2 - by);
+            if (my) me = yl; else oe = yl;
+        }
     } else { me = g0 + sg * (double)k; te = dmin(dmax((me - c0) * id, ta), tb); oe = fma(te, od, oc0); }
     // at most one grid line of the other axis lies strictly between os and oe
     const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
@@ -204,7 +225,7 @@ __device__ __forceinline__ void edge_step_mo(const ShootDev &S, double c0, doubl
 __device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, int k, double cs, int bx, int by) {
     const bool my = E.majorY != 0;
     edge_step_mo(S, my ? E.y0 : E.x0, my ? E.x0 : E.y0, my ? E.y1 : E.x1, my ? E.x1 : E.y1, my ? E.idy : E.idx, my ? E.idx : E.idy,
-                 E.ta, E.tb, E.g0, E.sg, my, E.n, k, cs, bx, by);
+                 E.ta, E.tb, E.g0, E.sg, my, E.cf, E.n, k, cs, bx, by);
 }
 
 struct TriSetup {
@@ -406,7 +427,7 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
         edge_setup(E, xa - fbx, ya - fby, xb - fbx, yb - fby, ry0, ry1, cx1);
         double *q = scratch + 16 * lane;
         q[0] = E.x0; q[1] = E.y0; q[2] = E.x1; q[3] = E.y1; q[4] = E.dx; q[5] = E.dy; q[6] = E.idx; q[7] = E.idy;
-        q[8] = E.ta; q[9] = E.tb; q[10] = E.g0; q[11] = E.sg; q[12] = __hiloint2double(E.n, E.majorY);
+        q[8] = E.ta; q[9] = E.tb; q[10] = E.g0; q[11] = E.sg; q[12] = __hiloint2double(E.n, E.majorY | (E.cf << 1));
         ne = E.n;
     }
     const int n0 = __shfl_sync(full, ne, 0), n1 = __shfl_sync(full, ne, 1), n2 = __shfl_sync(full, ne, 2);
@@ -419,7 +440,7 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
         const double *q = scratch + 16 * e;
         EdgeWalk E;
         E.x0 = q[0]; E.y0 = q[1]; E.x1 = q[2]; E.y1 = q[3]; E.dx = q[4]; E.dy = q[5]; E.idx = q[6]; E.idy = q[7];
-        E.ta = q[8]; E.tb = q[9]; E.g0 = q[10]; E.sg = q[11]; E.majorY = __double2loint(q[12]); E.n = __double2hiint(q[12]);
+        E.ta = q[8]; E.tb = q[9]; E.g0 = q[10]; E.sg = q[11]; E.majorY = __double2loint(q[12]) & 1; E.cf = __double2loint(q[12]) >> 1; E.n = __double2hiint(q[12]);
         edge_step(S, E, k - (e == 2 ? n0 + n1 : (e == 1 ? n0 : 0)), cs, bx, by);
     }
     __syncwarp();

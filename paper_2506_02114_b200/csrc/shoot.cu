@@ -91,11 +91,21 @@ __device__ __forceinline__ void queue_push(const ShootDev &S, const Win &W, Warp
 }
 
 // Optional copy of the mapped rays to the caller (tests); out of line: never part of a production run.
-static __device__ __noinline__ void dump_rays(const ShootDev *Sp, size_t d0, size_t stride, unsigned validmask, double w0x, double w0y,
+static __device__ __noinline__ void dump_rays(const ShootDev *Sp, long long d0, long long stride, unsigned validmask, double w0x, double w0y,
                                               double w1x, double w1y, double w2x, double w2y, double w3x, double w3y) {
     const double wx[4] = {w0x, w1x, w2x, w3x}, wy[4] = {w0y, w1y, w2y, w3y};
     for (int r = 0; r < 4; ++r)
-        if ((validmask >> r) & 1u) { Sp->dump1[d0 + (size_t)r * stride] = wx[r]; Sp->dump2[d0 + (size_t)r * stride] = wy[r]; }
+        if ((validmask >> r) & 1u) { Sp->dump1[d0 + (long long)r * stride] = wx[r]; Sp->dump2[d0 + (long long)r * stride] = wy[r]; }
+}
+
+// Tile `t` of the band in flight -> its indices on the GLOBAL tile grid.  Column-major by default: the tiles in
+// flight at any moment then form a patch of the image plane whose mapped cells fall into a patch of the map that
+// L2 holds, whereas a row of tiles spans the whole width of the map.
+__device__ __forceinline__ void tile_indices(const ShootDev &S, long long t, long long &tx, long long &ty) {
+    long long a, b;
+    if (S.colmajor) { a = t / S.tile_rows; b = t - a * S.tile_rows; }
+    else { b = t / S.ntx; a = t - b * S.ntx; }
+    tx = S.txb + a; ty = S.tyb + S.tile_row0 + b;
 }
 
 // The cell row between corner rows `prev` and `prev + 1` of the staged group: lane = cell column.
@@ -187,20 +197,27 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
     const long long ncx = S.i1 - S.i0 + 1;               // corners per dump row
     int npend = 0;
 
+    // Tiles are anchored on the GLOBAL cell grid (tile (tx, ty) holds the corners [31 tx, 31 tx + 31] x [31 ty, ..]),
+    // and a tile evaluates its rays whether or not they belong to the sub-range: a ray then has the same value to the
+    // last bit in whatever sub-range it is shot.  Only the cells of the sub-range are deposited.
     for (long long tile = fetch_tile(S); tile < ntiles;) {
         const long long tile_next = fetch_tile(S);       // the hand-out latency hides behind this tile's work
-        const long long ty = S.tile_row0 + tile / S.ntx;
-        const int tx = (int)(tile % S.ntx);
-        const long long ci0 = S.i0 + (long long)tx * (TCX - 1), cj0 = S.j0 + ty * (TCY - 1);
-        const long long ci1 = min(ci0 + TCX - 1, S.i1), cj1 = min(cj0 + TCY - 1, S.j1);   // last corner of the tile
+        long long tx, ty;
+        tile_indices(S, tile, tx, ty);
+        const long long ci0 = tx * (TCX - 1), cj0 = ty * (TCY - 1);
+        const long long ci1 = min(ci0 + TCX - 1, S.n1), cj1 = min(cj0 + TCY - 1, S.n2);   // last corner of the tile
         wtile_setup(S, Ws, C, ci0, cj0, ci1, cj1, 0.0);
 
         const long long ci = ci0 + lane;
-        const bool colv = ci <= S.i1, cellv = (lane < TCX - 1) && (ci < S.i1);
+        const bool colv = ci <= S.n1, cellv = (lane < TCX - 1) && (ci >= S.i0) && (ci < S.i1);
+        const bool dumpc = (ci >= S.i0) && (ci <= S.i1);
         const double x = corner_x(S, ci), ux = ((double)lane - 0.5 * (TCX - 1)) * S.dux;
+        // row groups that hold a corner row of the sub-range
+        const int g_lo = (S.j0 > cj0) ? (int)((S.j0 - cj0) / RPT) : 0;
+        const int g_hi = (int)((min(S.j1, cj1) - cj0) / RPT);
 #pragma unroll 1
-        for (int g = 0; g < NGRP; ++g) {
-            if (cj0 + g * RPT > S.j1) break;                             // warp-uniform
+        for (int g = g_lo; g <= g_hi && g < NGRP; ++g) {
+            const bool first = (g == g_lo);
             // ---- hot loop A: map RPT corner rows (eq 12)
             double y[RPT], uy[RPT], wx[RPT], wy[RPT];
             bool valid[RPT];
@@ -208,7 +225,7 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
             for (int r = 0; r < RPT; ++r) {
                 const int row = g * RPT + r;
                 const long long cj = cj0 + row;
-                valid[r] = colv && (cj <= S.j1);
+                valid[r] = colv && (cj <= S.n2);
                 y[r] = corner_y(S, cj);
                 uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.duy;
             }
@@ -216,8 +233,11 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
             if (S.dump1) {
                 unsigned vm = 0;
 #pragma unroll
-                for (int r = 0; r < RPT; ++r) vm |= valid[r] ? (1u << r) : 0u;
-                dump_rays(&S, (size_t)(cj0 + g * RPT - S.j0) * ncx + (size_t)(ci - S.i0), (size_t)ncx, vm,
+                for (int r = 0; r < RPT; ++r) {
+                    const long long cj = cj0 + g * RPT + r;
+                    vm |= (valid[r] && dumpc && cj >= S.j0 && cj <= S.j1) ? (1u << r) : 0u;
+                }
+                dump_rays(&S, (cj0 + g * RPT - S.j0) * ncx + (ci - S.i0), ncx, vm,
                           wx[0], wy[0], wx[1], wy[1], wx[2], wy[2], wx[3], wy[3]);
             }
 #pragma unroll
@@ -225,19 +245,22 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
                 const double u = (wx[r] - S.ylo1) * S.inv_p1, v = (wy[r] - S.ylo2) * S.inv_p2;
                 const int pk = pack_px(u, v);
                 Ws.stu[r + 1][lane] = u; Ws.stv[r + 1][lane] = v; Ws.stp[r + 1][lane] = pk; Ws.sto[r + 1][lane] = out_code(pk, S.npix1, S.npix2);
-                if (g == 0 && r == 1) {
-                    // window anchor: the tile centre extrapolated from its first two rows (any anchor is correct)
+                if (first && r == 1) {
+                    // window anchor: the tile centre extrapolated from the first two rows evaluated (any anchor is correct)
                     const double u0 = Ws.stu[1][lane], v0 = Ws.stv[1][lane];
-                    const double cu = __shfl_sync(full, u0 + 0.5 * (TCY - 1) * (u - u0), TCX / 2);
-                    const double cv = __shfl_sync(full, v0 + 0.5 * (TCY - 1) * (v - v0), TCX / 2);
+                    const double rows = 0.5 * (TCY - 1) - (double)(g * RPT);
+                    const double cu = __shfl_sync(full, u0 + rows * (u - u0), TCX / 2);
+                    const double cv = __shfl_sync(full, v0 + rows * (v - v0), TCX / 2);
                     W.ax = floor_to_int(cu) - WX / 2; W.ay = floor_to_int(cv) - WY / 2;
                 }
             }
             __syncwarp();
-            // ---- hot loop B: the cell rows between consecutive corner rows
+            // ---- hot loop B: the cell rows between consecutive corner rows (cell row cjp lies between corner rows cjp, cjp + 1)
 #pragma unroll 1
-            for (int r = (g == 0) ? 1 : 0; r < RPT; ++r) {
-                if (cj0 + g * RPT + r > S.j1) break;                     // warp-uniform
+            for (int r = first ? 1 : 0; r < RPT; ++r) {
+                const long long cjp = cj0 + g * RPT + r - 1;
+                if (cjp >= S.j1) break;                                  // warp-uniform
+                if (cjp < S.j0) continue;
                 cell_row(S, W, Ws, npend, r, cellv, tc);
             }
             process_pending(S, W, Ws, P, npend, tc);
@@ -360,7 +383,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_kernel(const __grid_c
             const double r0 = __shfl_sync(full, ry0, tis), r1 = __shfl_sync(full, ry1, tis), c1 = __shfl_sync(full, cx1, tis);
             if (ed < 3 * WB) {
                 EdgeWalk E;
-                E.n = 0; E.majorY = 1; E.sg = 1.0;
+                E.n = 0; E.majorY = 1; E.sg = 1.0; E.cf = 0;
                 double *q = er[ed];
                 if (st == 1) {
                     const int e1 = (e == 2) ? 0 : e + 1;
@@ -370,7 +393,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_kernel(const __grid_c
                     q[0] = my ? E.y0 : E.x0; q[1] = my ? E.x0 : E.y0; q[2] = my ? E.y1 : E.x1; q[3] = my ? E.x1 : E.y1;
                     q[4] = my ? E.idy : E.idx; q[5] = my ? E.idx : E.idy; q[6] = E.ta; q[7] = E.tb; q[8] = E.g0;
                 }
-                q[9] = __hiloint2double(E.n, E.majorY | (E.sg < 0.0 ? 2 : 0));
+                q[9] = __hiloint2double(E.n, E.majorY | (E.sg < 0.0 ? 2 : 0) | (E.cf << 2));
 
             }
         }
@@ -410,7 +433,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_kernel(const __grid_c
                 const double *q = er[3 * i + e];
                 const int fl = __double2loint(q[9]);
                 const double pk = tr[i][7];
-                edge_step_mo(S, q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7], q[8], (fl & 2) ? -1.0 : 1.0, (fl & 1) != 0,
+                edge_step_mo(S, q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7], q[8], (fl & 2) ? -1.0 : 1.0, (fl & 1) != 0, fl >> 2,
                              __double2hiint(q[9]), m, tr[i][6], __double2loint(pk), __double2hiint(pk));
             }
         }
@@ -478,53 +501,63 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 12) shoot_irs_kernel(const _
     const long long ntiles = (long long)S.ntx * S.tile_rows;
     const long long nrx = S.i1 - S.i0;
 
+    // global tile anchoring as in the IPM kernel: tile (tx, ty) holds the cells [32 tx, 32 tx + 32) x [32 ty, ..)
     for (long long tile = fetch_tile(S); tile < ntiles;) {
         const long long tile_next = fetch_tile(S);
-        const long long ty = S.tile_row0 + tile / S.ntx;
-        const int tx = (int)(tile % S.ntx);
-        const long long ci0 = S.i0 + (long long)tx * TCX, cj0 = S.j0 + ty * TCY;
-        const long long ci1 = min(ci0 + TCX, S.i1) - 1, cj1 = min(cj0 + TCY, S.j1) - 1;      // last cell of the tile
+        long long tx, ty;
+        tile_indices(S, tile, tx, ty);
+        const long long ci0 = tx * TCX, cj0 = ty * TCY;
+        const long long ci1 = min(ci0 + TCX, S.n1) - 1, cj1 = min(cj0 + TCY, S.n2) - 1;      // last cell of the tile
         wtile_setup(S, Ws, C, ci0, cj0, ci1, cj1, 0.5);
         const long long ci = ci0 + lane;
+        const bool insub = (ci >= S.i0) && (ci < S.i1);
         const double x = corner_x(S, ci) + 0.5 * S.h1, ux = ((double)lane - 0.5 * (TCX - 1)) * S.dux;
+        const int g_lo = (S.j0 > cj0) ? (int)((S.j0 - cj0) / RPT) : 0;
+        const int g_hi = (int)((min(S.j1 - 1, cj1) - cj0) / RPT);
 #pragma unroll 1
-        for (int g = 0; g < NGRP; ++g) {
-            if (cj0 + g * RPT >= S.j1) break;
+        for (int g = g_lo; g <= g_hi && g < NGRP; ++g) {
             double y[RPT], uy[RPT], wx[RPT], wy[RPT];
             bool valid[RPT];
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 const int row = g * RPT + r;
                 const long long cj = cj0 + row;
-                valid[r] = (ci < S.i1) && (cj < S.j1);
+                valid[r] = (ci < S.n1) && (cj < S.n2);
                 y[r] = corner_y(S, cj) + 0.5 * S.h2;
                 uy[r] = ((double)row - 0.5 * (TCY - 1)) * S.duy;
             }
             eval_rays<F32>(S, Ws, C, x, ux, y, uy, valid, wx, wy, tc);
+            bool cnt[RPT];                                                  // the rays of the sub-range
+#pragma unroll
+            for (int r = 0; r < RPT; ++r) {
+                const long long cj = cj0 + g * RPT + r;
+                cnt[r] = valid[r] && insub && (cj >= S.j0) && (cj < S.j1);
+            }
             int fx[RPT], fy[RPT];
             if (S.dump1) {
                 unsigned vm = 0;
 #pragma unroll
-                for (int r = 0; r < RPT; ++r) vm |= valid[r] ? (1u << r) : 0u;
-                dump_rays(&S, (size_t)(cj0 + g * RPT - S.j0) * nrx + (size_t)(ci - S.i0), (size_t)nrx, vm,
+                for (int r = 0; r < RPT; ++r) vm |= cnt[r] ? (1u << r) : 0u;
+                dump_rays(&S, (cj0 + g * RPT - S.j0) * nrx + (ci - S.i0), nrx, vm,
                           wx[0], wy[0], wx[1], wy[1], wx[2], wy[2], wx[3], wy[3]);
             }
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 fx[r] = floor_div(wx[r] - S.ylo1, S.p1, S.inv_p1, S.fd_tol); fy[r] = floor_div(wy[r] - S.ylo2, S.p2, S.inv_p2, S.fd_tol);
             }
-            if (g == 0) {
-                // window anchor: the tile centre extrapolated from its first two rows (any anchor is correct)
+            if (g == g_lo) {
+                // window anchor: the tile centre extrapolated from the first two rows evaluated (any anchor is correct)
                 const int ax0 = max(min(fx[0], 40000), -40000), ax1 = max(min(fx[1], 40000), -40000);
                 const int ay0 = max(min(fy[0], 40000), -40000), ay1 = max(min(fy[1], 40000), -40000);
-                const int cu = __shfl_sync(full, ax0 + ((TCY - 1) * (ax1 - ax0)) / 2, TCX / 2);
-                const int cv = __shfl_sync(full, ay0 + ((TCY - 1) * (ay1 - ay0)) / 2, TCX / 2);
+                const int rows2 = (TCY - 1) - 2 * g * RPT;                  // twice the rows from the first one to the centre
+                const int cu = __shfl_sync(full, ax0 + (rows2 * (ax1 - ax0)) / 2, TCX / 2);
+                const int cv = __shfl_sync(full, ay0 + (rows2 * (ay1 - ay0)) / 2, TCX / 2);
                 W.ax = cu - WX / 2; W.ay = cv - WY / 2;
             }
 #pragma unroll
             for (int r = 0; r < RPT; ++r) {
                 int key = -1;
-                if (valid[r] && (unsigned)fx[r] < (unsigned)S.npix1 && (unsigned)fy[r] < (unsigned)S.npix2) {
+                if (cnt[r] && (unsigned)fx[r] < (unsigned)S.npix1 && (unsigned)fy[r] < (unsigned)S.npix2) {
                     key = (fy[r] << 16) | fx[r];
                     ++tc.single;
                 }
@@ -577,7 +610,11 @@ __global__ void __launch_bounds__(FIN_T) finalise_kernel(const unsigned long lon
             __syncthreads();
         }
         if (i < npix1) {
-            if (map) { double v = (double)a * scale; map[row + i] = accumulate ? map[row + i] + v : v; }
+            // The sum is read as SIGNED and clamped at 0: in a map that holds only part of the grid's triangles (a
+            // slab, a patch) a pixel may be left with a rounding residue of a few quanta below zero by the large
+            // triangles that cross it; as an unsigned number that would be 2^64.
+            const long long sa = (long long)a;
+            if (map) { double v = (double)(sa < 0 ? 0ll : sa) * scale; map[row + i] = accumulate ? map[row + i] + v : v; }
             if (counts) counts[row + i] = accumulate ? counts[row + i] + a : a;
         }
     }
@@ -632,34 +669,37 @@ int geometry(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid *g) {
 
 
 namespace {
-struct ParkedScratch { DevBuf<double> queue; DevBuf<int> qcount; DevBuf<unsigned int> biglist; int device = -1; };
-ParkedScratch g_parked;
+// `ready` is recorded on the stream the parked buffers were last used on; whoever takes or frees them waits for it.
+struct ParkedScratch { DevBuf<double> queue; DevBuf<int> qcount; DevBuf<unsigned int> biglist; int device = -1; cudaEvent_t ready = nullptr; };
+ParkedScratch g_parked[ML_MAXDEV];
 std::mutex g_parked_mutex;
 }  // namespace
 
-void scratch_park(mlens_field *f) {
+void scratch_park(mlens_field *f, cudaStream_t s) {
     std::lock_guard<std::mutex> lock(g_parked_mutex);
-    if (!f->queue.p || f->queue.cap <= g_parked.queue.cap) return;              // the larger one is kept
-    g_parked.queue.release(); g_parked.qcount.release(); g_parked.biglist.release();
-    g_parked.queue = f->queue; g_parked.qcount = f->qcount; g_parked.biglist = f->biglist; g_parked.device = f->device;
+    ParkedScratch &P = g_parked[(f->device >= 0 && f->device < ML_MAXDEV) ? f->device : ML_MAXDEV - 1];
+    if (!f->queue.p || f->queue.cap <= P.queue.cap) return;                     // the larger one is kept
+    if (P.queue.p) {
+        if (P.ready) cudaStreamWaitEvent(s, P.ready, 0);
+        P.queue.release(s); P.qcount.release(s); P.biglist.release(s);
+    }
+    if (!P.ready && cudaEventCreateWithFlags(&P.ready, cudaEventDisableTiming) != cudaSuccess) { P.ready = nullptr; cudaGetLastError(); return; }
+    P.queue = f->queue; P.qcount = f->qcount; P.biglist = f->biglist; P.device = f->device;
+    cudaEventRecord(P.ready, s);
     f->queue = DevBuf<double>(); f->qcount = DevBuf<int>(); f->biglist = DevBuf<unsigned int>();
 }
 
-void scratch_take(mlens_field *f) {
+void scratch_take(mlens_field *f, cudaStream_t s) {
     std::lock_guard<std::mutex> lock(g_parked_mutex);
-    if (f->queue.p || !g_parked.queue.p || g_parked.device != f->device) return;
-    f->queue = g_parked.queue; f->qcount = g_parked.qcount; f->biglist = g_parked.biglist;
-    g_parked.queue = DevBuf<double>(); g_parked.qcount = DevBuf<int>(); g_parked.biglist = DevBuf<unsigned int>();
+    ParkedScratch &P = g_parked[(f->device >= 0 && f->device < ML_MAXDEV) ? f->device : ML_MAXDEV - 1];
+    if (f->queue.p || !P.queue.p || P.device != f->device) return;
+    if (P.ready) cudaStreamWaitEvent(s, P.ready, 0);
+    f->queue = P.queue; f->qcount = P.qcount; f->biglist = P.biglist;
+    f->queue.s_own = s; f->qcount.s_own = s; f->biglist.s_own = s;
+    P.queue = DevBuf<double>(); P.qcount = DevBuf<int>(); P.biglist = DevBuf<unsigned int>();
 }
 
 static const long long GIANT_CAP = 1ll << 20;       // chunk slots per band (8 MB)
-
-static long long env_ll(const char *name, long long dflt) {
-    const char *v = getenv(name);
-    if (!v || !*v) return dflt;
-    long long x = atoll(v);
-    return x > 0 ? x : dflt;
-}
 
 int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double *map,
           unsigned long long *counts, mlens_stats *st, cudaStream_t s) {
@@ -678,16 +718,16 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         ML_CUDA(cudaMemsetAsync(f->diff.p, 0, (size_t)npix * 8, s));
         // Queue of general triangles: every band ends with the tails of three kernels, so bands should be few and
         // the queue large -- 8 GiB unless the device is small, never more than the worst case of this map (two
-        // triangles per cell); halved until it can be had.  MLENS_QUEUE_MB overrides.
+        // triangles per cell); halved until it can be had.  desc.queue_mb overrides.
         size_t mem_free = 0, mem_total = 0;
         cudaMemGetInfo(&mem_free, &mem_total);
         long long qmb = 8192;
         if (mem_total > 0 && (long long)(mem_total >> 24) < qmb) qmb = (long long)(mem_total >> 24);   // <= 1/16 of the device
         const double need_mb = 3.2 * (double)(i1 - i0) * (double)(j1 - j0) * (QENT * 8) / 1048576.0 + 64.0;
         if ((double)qmb > need_mb) qmb = (long long)need_mb;
-        const long long qmb_env = env_ll("MLENS_QUEUE_MB", 0);
+        const long long qmb_env = d->queue_mb > 0 ? d->queue_mb : 0;       // the caller's choice, taken as it is
         if (qmb_env > 0) qmb = qmb_env;
-        scratch_take(f);
+        scratch_take(f, s);
         for (;;) {
             qcap = qmb * (1ll << 20) / (QCHUNK * QENT * 8);          // chunks
             int rc = f->queue.reserve((size_t)qcap * QCHUNK * QENT, s, false);
@@ -703,7 +743,8 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     ShootDev S;
     S.L = make_lens_dev(f);
     S.x0_1 = g->x0_1; S.x0_2 = g->x0_2; S.h1 = g->h1; S.h2 = g->h2;
-    S.i0 = i0; S.i1 = i1; S.j0 = j0; S.j1 = j1;
+    S.i0 = i0; S.i1 = i1; S.j0 = j0; S.j1 = j1; S.n1 = g->n1; S.n2 = g->n2;
+    S.colmajor = d->tile_traversal == 1 ? 0 : 1;
     S.ylo1 = g->ylo1; S.ylo2 = g->ylo2; S.p1 = g->p1; S.p2 = g->p2; S.inv_p1 = 1.0 / g->p1; S.inv_p2 = 1.0 / g->p2;
     S.npix1 = d->npix1; S.npix2 = d->npix2;
     S.acc = f->acc.p; S.diff = f->diff.p; S.queue = f->queue.p; S.qcount = f->qcount.p; S.biglist = f->biglist.p; S.big_cap = qcap * QCHUNK / 4; S.giant = f->giant.p; S.giant_cap = ipm ? GIANT_CAP : 0; S.counters = f->counters.p; S.queue_cap = qcap;
@@ -712,11 +753,11 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     if ((S.dump1 == nullptr) != (S.dump2 == nullptr)) { set_error("dump_w1 and dump_w2 go together"); return MLENS_EINVAL; }
     const bool f32 = d->eval_mode == MLENS_EVAL_FMM_F32;       // same tiles and slow paths as FMM; only the fast path differs
     S.eval_mode = f32 ? MLENS_EVAL_FMM : d->eval_mode;
-    S.tq = (int)env_ll("MLENS_TILE_ORDER", 0);
+    S.tq = d->tile_order;
     if (S.tq > TQMAX) S.tq = TQMAX;
     if (S.tq <= 0) S.tq = -1;                                   // chosen below, once the tile radius is known
     else if (S.tq < 2) S.tq = 2;
-    S.small_px = (int)env_ll("MLENS_SMALL_PX", 24);
+    S.small_px = d->small_px > 0 ? d->small_px : 24;
     S.fd_tol = 1.0e-9 * (double)((d->npix1 > d->npix2) ? d->npix1 : d->npix2);
     // truncation budget of the tile series: 5 % of the deflection accuracy the field was built for
     S.rt = 0.5 * sqrt((double)((TCX - 1) * (TCX - 1)) * g->h1 * g->h1 + (double)((TCY - 1) * (TCY - 1)) * g->h2 * g->h2) * (1.0 + 1e-9);
@@ -742,20 +783,22 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             S.tq_lev[l] = (signed char)(ql > S.tq ? S.tq : ql);
         }
     } else {
-        for (int l = 0; l <= ML_MAXLEV; ++l) S.tq_lev[l] = (signed char)S.tq;       // MLENS_TILE_ORDER: one order everywhere
+        for (int l = 0; l <= ML_MAXLEV; ++l) S.tq_lev[l] = (signed char)S.tq;       // desc.tile_order: one order everywhere
     }
     S.eps_star = 0.03 * f->eps * f->theta / (double)ML_NEAR;
     const int stepx = ipm ? TCX - 1 : TCX, stepy = ipm ? TCY - 1 : TCY;
-    long long ntx = (i1 - i0 + stepx - 1) / stepx, nty = (j1 - j0 + stepy - 1) / stepy;
+    // tiles of the GLOBAL tile grid that hold a cell of the sub-range
+    S.txb = i0 / stepx; S.tyb = j0 / stepy;
+    long long ntx = (i1 - 1) / stepx - S.txb + 1, nty = (j1 - 1) / stepy - S.tyb + 1;
     if (ntx > 0x7fffffffLL) { set_error("too many tiles per row"); return MLENS_EINVAL; }
     S.ntx = (int)ntx;
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    long long band_cells = env_ll("MLENS_BAND_CELLS", 1ll << 30);
+    long long band_cells = d->band_cells > 0 ? d->band_cells : (1ll << 30);
     long long rows_per_band = band_cells / (ntx * stepx * stepy);
     if (rows_per_band < 1) rows_per_band = 1;
-    if (!ipm && env_ll("MLENS_BAND_FIXED", 0) == 0) rows_per_band = nty;      // IRS has no queue to bound: one launch
+    if (!ipm && !d->band_fixed) rows_per_band = nty;                          // IRS has no queue to bound: one launch
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     const bool timed = st && (d->sync || d->ptr_kind == MLENS_PTR_HOST);
     if (timed) { ML_CUDA(cudaEventCreate(&e0)); ML_CUDA(cudaEventCreate(&e1)); ML_CUDA(cudaEventRecord(e0, s)); }
@@ -768,13 +811,13 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         return MLENS_OK;
     };
     const size_t smem_ipm = SHOOT_WARPS * sizeof(WarpSharedIpm), smem_irs = SHOOT_WARPS * sizeof(WarpShared);
-    static bool attr_set = false;
-    if (!attr_set) {
+    static std::atomic<int> attr_set[ML_MAXDEV];                     // kernel attributes are per device (context)
+    if (!attr_set[device_slot()].load()) {
         ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
         ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_irs));
         ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
         ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_irs));
-        attr_set = true;
+        attr_set[device_slot()].store(1);
     }
     int bps_ipm = 1, bps_irs = 1;
     ML_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps_ipm, shoot_ipm_kernel<false>, SHOOT_WARPS * 32, smem_ipm));
@@ -787,7 +830,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     const long long nwarps_res = (long long)nsm * (ipm ? bps_ipm : bps_irs) * SHOOT_WARPS;
     const double cap_entries = ipm ? fmax(0.0, 0.8 * (double)qcap - (double)nwarps_res) * (double)QCHUNK * 0.85 : 0.0;
     double rate = -1.0;                                            // general triangles per cell, measured
-    const bool adapt = env_ll("MLENS_BAND_FIXED", 0) == 0;          // MLENS_BAND_FIXED=1: always MLENS_BAND_CELLS (tests)
+    const bool adapt = !d->band_fixed;                              // desc.band_fixed: always desc.band_cells (tests)
     unsigned long long q_before = 0;
     for (long long r0 = 0; r0 < nty; r0 += rows_per_band, ++bands) {
         if (ipm && adapt) {

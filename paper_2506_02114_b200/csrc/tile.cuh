@@ -32,6 +32,9 @@ struct ShootDev {
     LensDev L;
     double x0_1, x0_2, h1, h2;
     long long i0, i1, j0, j1;          // cell sub-range
+    long long n1, n2;                  // cells of the whole grid: tiles are anchored on it, whatever the sub-range
+    long long txb, tyb;                // first tile column / row (global tile indices) that holds a cell of the sub-range
+    int colmajor;                      // tiles of a band are handed out column by column (else row by row)
     double ylo1, ylo2, p1, p2, inv_p1, inv_p2;
     int npix1, npix2;
     unsigned long long *acc;           // fixed-point pixel sums (IPM) or ray counts (IRS)

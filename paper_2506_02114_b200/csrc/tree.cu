@@ -347,11 +347,11 @@ __global__ void lists_kernel(TreeDev T, int n_nodes, int *leaf_id /* in: exclusi
 }
 
 // ------------------------------------------------------------------------------------------------
-void Tree::release() {
-    level.release(); ix.release(); iy.release(); parent.release(); child0.release(); lo.release(); n.release();
-    leaf_id.release(); nbr.release(); m2l_cnt.release(); m2l_list.release(); p2l_cnt.release(); p2l_list.release();
-    mp.release(); loc.release(); leaf_node.release(); near_cnt.release(); near_x.release(); near_y.release();
-    near_m.release(); ecoef.release();
+void Tree::release(cudaStream_t s) {
+    level.release(s); ix.release(s); iy.release(s); parent.release(s); child0.release(s); lo.release(s); n.release(s);
+    leaf_id.release(s); nbr.release(s); m2l_cnt.release(s); m2l_list.release(s); p2l_cnt.release(s); p2l_list.release(s);
+    mp.release(s); loc.release(s); leaf_node.release(s); near_cnt.release(s); near_x.release(s); near_y.release(s);
+    near_m.release(s); ecoef.release(s);
 }
 
 static int reserve_nodes(Tree &t, size_t n, cudaStream_t s) {
@@ -368,7 +368,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     Tree &t = f->tree;
 
     // ---- extent, moments
-    DevBuf<unsigned long long> d_bits; DevBuf<double> d_mom;
+    ScratchBuf<unsigned long long> d_bits; ScratchBuf<double> d_mom;
     ML_TRY(d_bits.reserve(1, s)); ML_TRY(d_mom.reserve(2, s));
     ML_CUDA(cudaMemsetAsync(d_bits.p, 0, sizeof(unsigned long long), s));
     ML_CUDA(cudaMemsetAsync(d_mom.p, 0, 2 * sizeof(double), s));
@@ -397,7 +397,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     // ---- Morton sort
     ML_TRY(f->sx.reserve(n + 1, s, false)); ML_TRY(f->sy.reserve(n + 1, s, false)); ML_TRY(f->sm.reserve(n + 1, s, false));
     ML_TRY(f->sqx.reserve(n + 1, s, false)); ML_TRY(f->sqy.reserve(n + 1, s, false));
-    DevBuf<unsigned long long> k0, k1; DevBuf<int> v0, v1, hist, scratch;
+    ScratchBuf<unsigned long long> k0, k1; ScratchBuf<int> v0, v1, hist, scratch;
     if (n > 0) {
         ML_TRY(k0.reserve(n, s, false)); ML_TRY(k1.reserve(n, s, false));
         ML_TRY(v0.reserve(n, s, false)); ML_TRY(v1.reserve(n, s, false));
@@ -423,7 +423,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     // ---- levels: the loop runs on the device's own counts.  Level l is launched with an upper bound of its size
     // (four times the bound of the level above, at most the node capacity); the ranges come back once per chunk of
     // levels -- log4(n) + 3 levels in the first chunk, which is all of them for any star field that is not clustered.
-    DevBuf<int> flags, rank, d_over, d_range;
+    ScratchBuf<int> flags, rank, d_over, d_range;
     ML_TRY(d_over.reserve(1, s)); ML_TRY(d_range.reserve(ML_MAXLEV + 3, s));
     size_t cap = 2 * (size_t)n + 4096;
     int h_range[ML_MAXLEV + 3];
@@ -498,7 +498,7 @@ int build_tree(mlens_field *f, cudaStream_t s) {
     ML_CUDA(cudaMemsetAsync(t.near_x.p, 0, (size_t)nleaf * ML_NEAR * 8, s));
     ML_CUDA(cudaMemsetAsync(t.near_y.p, 0, (size_t)nleaf * ML_NEAR * 8, s));
     ML_CUDA(cudaMemsetAsync(t.near_m.p, 0, (size_t)nleaf * ML_NEAR * 8, s));
-    DevBuf<int> maxima; ML_TRY(maxima.reserve(4, s)); ML_CUDA(cudaMemsetAsync(maxima.p, 0, 16, s));
+    ScratchBuf<int> maxima; ML_TRY(maxima.reserve(4, s)); ML_CUDA(cudaMemsetAsync(maxima.p, 0, 16, s));
     TreeDev T{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p, t.nbr.p, f->sqx.p, f->sqy.p};
     ML_LAUNCH(lists_kernel, (nn + 127) / 128, 128, 0, s, T, nn, t.leaf_id.p, t.leaf_node.p, t.m2l_cnt.p, t.m2l_list.p,
                                                   t.p2l_cnt.p, t.p2l_list.p, t.near_cnt.p, t.near_x.p, t.near_y.p,

@@ -10,7 +10,9 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libmlens.so")
+_BENCH_SO = os.path.join(_HERE, "libmlens_bench.so")
 _lib = None
+_bench_lib = None
 
 SHAPE_DISC, SHAPE_RECT = 0, 1
 MASS_EQUAL, MASS_POWER = 0, 1
@@ -59,7 +61,9 @@ class ShootDesc(C.Structure):
                 ("map_mode", C.c_int32), ("eval_mode", C.c_int32), ("border_mode", C.c_int32), ("accumulate", C.c_int32),
                 ("border_param", C.c_double), ("He1", C.c_double), ("He2", C.c_double),
                 ("i0", C.c_int64), ("i1", C.c_int64), ("j0", C.c_int64), ("j1", C.c_int64),
-                ("ptr_kind", C.c_int32), ("sync", C.c_int32), ("dump_w1", C.c_void_p), ("dump_w2", C.c_void_p)]
+                ("ptr_kind", C.c_int32), ("sync", C.c_int32), ("dump_w1", C.c_void_p), ("dump_w2", C.c_void_p),
+                ("queue_mb", C.c_int32), ("tile_order", C.c_int32), ("small_px", C.c_int32), ("band_fixed", C.c_int32),
+                ("band_cells", C.c_int64), ("tile_traversal", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Grid(C.Structure):
@@ -111,8 +115,6 @@ def lib():
         L.mlens_grid_info.argtypes = [vp, C.POINTER(ShootDesc), C.POINTER(Grid)]
         L.mlens_shoot.argtypes = [vp, C.POINTER(ShootDesc), vp, vp, C.POINTER(Stats), vp]
         L.mlens_field_get_tree.argtypes = [vp, C.POINTER(TreeView)]
-        L.mlens_bench_dfma.argtypes = [_dp, vp]
-        L.mlens_bench_atomics.argtypes = [i64, i32, _dp, vp]
         dbl = C.c_double
         L.mlens_map_light_curve.argtypes = [vp, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, dbl, dbl, i64, i32, vp, i32, vp]
         L.mlens_map_histogram.argtypes = [vp, i64, dbl, dbl, dbl, i32, vp, i32, vp]
@@ -265,7 +267,8 @@ class Field:
     # ---- shooting ------------------------------------------------------------------------------
     @staticmethod
     def _desc(half_y, npix, k, *, map_mode=MAP_IPM, eval_mode=EVAL_FMM, border_mode=BORDER_A6, border_param=1e-3,
-              center=(0.0, 0.0), He=(0.0, 0.0), sub=None, accumulate=False, sync=True):
+              center=(0.0, 0.0), He=(0.0, 0.0), sub=None, accumulate=False, sync=True,
+              queue_mb=0, tile_order=0, small_px=0, band_fixed=False, band_cells=0, tile_traversal=0):
         d = ShootDesc()
         hy = half_y if isinstance(half_y, (tuple, list)) else (half_y, half_y)
         npx = npix if isinstance(npix, (tuple, list)) else (npix, npix)
@@ -276,6 +279,8 @@ class Field:
         d.map_mode, d.eval_mode, d.border_mode, d.border_param = map_mode, eval_mode, border_mode, border_param
         d.He1, d.He2 = He
         d.accumulate, d.sync = int(accumulate), int(sync)
+        d.queue_mb, d.tile_order, d.small_px, d.band_fixed = queue_mb, tile_order, small_px, int(band_fixed)
+        d.band_cells, d.tile_traversal = band_cells, tile_traversal
         if sub is not None:
             d.i0, d.i1, d.j0, d.j1 = sub
         return d
@@ -348,15 +353,33 @@ class Field:
         return a
 
 
+def bench_lib():
+    """Loads libmlens_bench.so (include/mlens_bench.h): the roofline micro-benchmarks, a library of their own."""
+    global _bench_lib
+    if _bench_lib is None:
+        if not os.path.exists(_BENCH_SO):
+            raise MlensError(f"{_BENCH_SO} is missing: run `python -m paper_2506_02114_b200.build`")
+        L = C.CDLL(_BENCH_SO)
+        L.mlens_bench_dfma.argtypes = [_dp, C.c_void_p]
+        L.mlens_bench_atomics.argtypes = [C.c_int64, C.c_int32, _dp, C.c_void_p]
+        _bench_lib = L
+    return _bench_lib
+
+
+def _bench_check(rc):
+    if rc != 0:
+        raise MlensError(f"libmlens_bench: CUDA error {-rc}")
+
+
 def bench_dfma(stream=None):
     v = C.c_double()
-    _check(lib().mlens_bench_dfma(C.byref(v), _stream(stream)))
+    _bench_check(bench_lib().mlens_bench_dfma(C.byref(v), _stream(stream)))
     return v.value
 
 
 def bench_atomics(n_slots, use_u64=True, stream=None):
     v = C.c_double()
-    _check(lib().mlens_bench_atomics(n_slots, int(use_u64), C.byref(v), _stream(stream)))
+    _bench_check(bench_lib().mlens_bench_atomics(n_slots, int(use_u64), C.byref(v), _stream(stream)))
     return v.value
 
 

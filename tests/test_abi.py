@@ -27,6 +27,15 @@ def test_exports_every_declared_symbol(so):
         assert hasattr(L, n), n
     L.mlens_version.restype = ctypes.c_int
     assert L.mlens_version() == 100
+    # the roofline micro-benchmarks are a library of their own (include/mlens_bench.h), not part of the product ABI
+    assert not hasattr(L, "mlens_bench_dfma") and not hasattr(L, "mlens_bench_atomics")
+    bh = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "mlens_bench.h")).read(), flags=re.S)
+    bnames = set(re.findall(r"\b(mlens_[a-z_0-9]+)\s*\(", bh))
+    assert bnames == {"mlens_bench_dfma", "mlens_bench_atomics"}
+    from paper_2506_02114_b200 import build
+    B = ctypes.CDLL(build.BENCH_SO)
+    for n in bnames:
+        assert hasattr(B, n), n
 
 
 def test_struct_sizes_match_header(so):
@@ -55,6 +64,13 @@ def test_no_cpu_fallback(so):
         ml.Field.from_stars(0.4, 0.2, z, z, z, kappa_star=0.2, R=1.0)
     with pytest.raises(ml.MlensError):
         ml.bench_dfma()
+
+
+def test_no_environment_knobs():
+    """The library is configured through its C structs only ("plain C structs; no config files"): no getenv."""
+    csrc = os.path.join(ROOT, "paper_2506_02114_b200", "csrc")
+    for fn in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, fn)).read(), fn
 
 
 def test_product_does_not_import_oracle():
