@@ -3,29 +3,30 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--impl ours|reference]
 
-One STEP is one pass of the whole hot path over one synthetic workload (BASELINE.json configs[1] by
-default, the configuration the metric is quoted on):
+One STEP is one pass of the whole hot path over one synthetic workload -- by default BASELINE.json configs[4],
+the largest configuration that fits one GPU (`metric` names no configuration; 1e7 Salpeter stars, 10^4 x 10^4
+pixels, 10 rays per pixel length: the paper's production regime):
 
     seeded star field -> Morton sort -> quadtree + lists -> P2M/M2M -> M2L/P2L/L2L -> leaf series
     -> fused ray evaluation + IPM deposit (map 1)  -> fused ray evaluation + IRS count (map 2)
 
 all of it in libmlens' CUDA kernels, called through the C ABI (include/mlens.h).  `value` is lens-equation
-evaluations per second over the whole step (unique rays of both maps / step time), inputs resident in
-HBM (the star field is generated on the device from the seed).  `e2e` repeats the step with HOST
-buffers: stars handed over as pinned host arrays, maps returned into pinned host arrays, the library
-doing the copies inside the timed region.
+evaluations per second over the whole step (unique rays of both maps / step time), inputs resident in HBM (the
+star field is generated on the device from the seed).  `e2e` repeats the step with HOST buffers: stars handed
+over as pinned host arrays, maps returned into pinned host arrays, the library doing the copies inside the
+timed region.  The `maps` object carries create / IPM / IRS wall times of the other four configurations
+(BASELINE.json's second metric, map wall-time), `roofline` the FP64 account of the fused evaluate + deposit
+kernel and `roofline_atomics` the atomic account of the apportioning kernels.
 
-N > 1 (torchrun): the SAME map on N GPUs: stars and tree replicated, the cell grid cut
-into star-weighted row slabs (paper_2506_02114_b200/multi.py), one all-reduce (sum, float64) of each
-map over NCCL -- the path's only exchange step; total work is fixed, so scaling is "strong";
-time = max over ranks.
+N > 1 (torchrun): the SAME map on N GPUs: stars and tree replicated, the cell grid cut into
+row slabs (paper_2506_02114_b200/multi.py), one all-reduce (sum, float64) of each map over NCCL -- the path's
+only exchange step; total work is fixed, so scaling is "strong"; time = max over ranks.
 
-`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
-workload, on the host cores of this box.  It is a deliberately slow baseline, not the target.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload, on the
+host cores of this box.  It is a deliberately slow baseline, not the target.
 """
 import argparse
 import json
-import math
 import os
 import subprocess
 import sys
@@ -43,25 +44,27 @@ import synth  # noqa: E402
 METRIC = "lens_eq_evals_per_s"
 UNIT = "evals/s"
 
-# B200 FP64 vector peak used as the "alu" roofline denominator: 148 SMs x 64 DFMA
-# lanes/SM/clk x 2 flop x 1.965 GHz (clocks.max.sm of MEASURED_PEAKS.json).  The DFMA rate measured
-# by mlens_bench_dfma in the same run is reported beside it as `peak_measured_dfma`.
+# B200 FP64 vector units: 64 DFMA lanes per SM (guide); the derived peak is reported beside the DFMA rate measured
+# by libmlens_bench in the same run, which is the roofline denominator.
 FP64_LANES_PER_SM = 64
-# dram bytes per launch of the dominant kernel from the committed `ncu --set full` capture
-# (profiles/r01e_launches.md: dram read + write of shoot_ipm_kernel, mean of the two launches of a map).
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 3.43e9
+# Algorithmic work per lens-equation evaluation in the paper's per-ray scheme:
+#   n_near x (9 flop + 1 reciprocal) + (p - 1) complex Horner steps x 8 flop + 10 flop (macro + sheet terms)
+FLOP_PER_NEAR_STAR, FLOP_PER_TERM, FLOP_MACRO = 9.0, 8.0, 10.0
+QUEUE_ENTRY_BYTES = 48
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default 4: the largest single-GPU one)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--maps", default="", help="also time whole maps of these configs, e.g. 0,2,3,4 (create, IPM, IRS wall ms)")
+    ap.add_argument("--maps", default="0,1,2,3,rect1", help="also time whole maps of these configs (create, IPM, IRS wall ms); "
+                    "'rect1' = config 1 with a rectangular star region; '' = none")
+    ap.add_argument("--no-extras", action="store_true", help="skip the f32, consumers and slab-balance objects")
     return ap.parse_args()
 
 
@@ -99,7 +102,7 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except subprocess.TimeoutExpired:
             self.proc.kill()
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         try:
             for line in open(self.path):
@@ -107,7 +110,7 @@ class ClockSampler:
                 if len(c) < 9:
                     continue
                 try:
-                    sm.append(float(c[1])); mx.append(float(c[2]))
+                    sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
                 except ValueError:
                     continue
                 for nm, v in zip(names, c[5:9]):
@@ -117,21 +120,27 @@ class ClockSampler:
         except OSError:
             pass
         if sm:
-            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm), power_w_median=float(np.median(pw)))
         out["reasons"] = sorted(reasons)
         return out
 
 
 # ------------------------------------------------------------------------------------------------
+_ORACLE_FIELD = {}
+
+
 def oracle_sample(cfg, patch, want_irs=True):
     """Times the CPU oracle on a patch of `patch` = (ni, nj) cells at the window centre: the whole path
-    (direct sum over all stars + brute-force clipping; IRS binning).  Returns (evals, seconds, threads)."""
+    (direct sum over all stars + brute-force clipping; IRS binning).  Returns (evals, seconds, threads, sub).
+    The star field (an input) is drawn once per process."""
     import oracle
     oracle.build()
     R = cfg.R_star
-    xs, ys, ms = oracle.starfield(cfg.seed, cfg.n_stars, shape=0, a1=R, mass_law=cfg.mass_law,
-                                  a=cfg.mass_a, lo=cfg.mass_lo, hi=cfg.mass_hi)
-    of = oracle.Field.make(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, xs, ys, ms, R=R)
+    if cfg.name not in _ORACLE_FIELD:
+        xs, ys, ms = oracle.starfield(cfg.seed, cfg.n_stars, shape=0, a1=R, mass_law=cfg.mass_law,
+                                      a=cfg.mass_a, lo=cfg.mass_lo, hi=cfg.mass_hi)
+        _ORACLE_FIELD[cfg.name] = oracle.Field.make(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, xs, ys, ms, R=R)
+    of = _ORACLE_FIELD[cfg.name]
     g = oracle.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, cfg.npix, cfg.rays_per_pixel_length,
                         cfg.border_mode, cfg.border_param, m2_over_m=cfg.m2_over_m)
     ni, nj = min(patch[0], g.n1), min(patch[1], g.n2)
@@ -146,14 +155,23 @@ def oracle_sample(cfg, patch, want_irs=True):
     return evals, time.perf_counter() - t0, oracle.num_threads(), sub
 
 
+def oracle_patch_for(cfg, seconds, cores=16):
+    """Patch side such that the oracle's direct sum (~1.2e-8 core-seconds per star and ray, long double) takes about
+    `seconds` on `cores` cores."""
+    evals = seconds * cores / (1.2e-8 * cfg.n_stars)
+    side = int(max(8, min(384, (evals / 2.0) ** 0.5)))
+    return (side, side)
+
+
 def run_reference(args):
     """--impl reference: the oracle, as it stands, on this box's host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     cfg = synth.get_config(args.config)
-    patch = (128, 128)
+    cores = os.cpu_count() or 16
+    patch = oracle_patch_for(cfg, 8.0, cores)
     for _ in range(args.warmup):
-        oracle_sample(cfg, (32, 32))
+        oracle_sample(cfg, (8, 8))
     tot_e, tot_t, thr, sub = 0, 0.0, 1, None
     for _ in range(args.steps):
         e, t, thr, sub = oracle_sample(cfg, patch)
@@ -194,14 +212,17 @@ def run_ours(args):
     half, npix, k = cfg.half_y, cfg.npix, cfg.rays_per_pixel_length
     stream = torch.cuda.current_stream()
 
+    def seeded(c):
+        return ml.Field.seeded(c.kappa_tot, c.gamma, c.n_stars, c.seed, kappa_star=c.kappa_star,
+                               mass_law=c.mass_law, mass_a=c.mass_a, mass_lo=c.mass_lo, mass_hi=c.mass_hi)
+
     map_ipm = torch.zeros((npix, npix), dtype=torch.float64, device=dev)
     map_irs = torch.zeros((npix, npix), dtype=torch.float64, device=dev)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     state = {}
 
     def step_device():
-        f = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, seed, kappa_star=cfg.kappa_star,
-                            mass_law=cfg.mass_law, mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
+        f = seeded(cfg)
         if world > 1 and "weights" not in state:     # slab cost model from the star rows (same on every rank; cached)
             g0 = f.grid(half, npix, k, **kw)
             state["weights"] = multi.star_row_weights(f.stars()[1], g0.x0_2, g0.h2, int(g0.n2))
@@ -210,16 +231,6 @@ def run_ours(args):
         _, _, s2 = multi.shoot_distributed(f, half, npix, k, weights=state.get("weights"), out=map_irs,
                                            map_mode=ml.MAP_IRS, **kw)
         state.update(info=f.info(), ipm=s1, irs=s2, slab=slab, grid=f.grid(half, npix, k, **kw))
-        if "near_mean" not in state:                 # mean near-field list of a ray's leaf (area-weighted over the window)
-            t = f.tree()
-            g_ = state["grid"]
-            leaves = np.where(t["child0"] < 0)[0]
-            half_l = t["root_half"] / 2.0 ** t["level"][leaves]
-            cx = -t["root_half"] + (2 * t["ix"][leaves] + 1) * half_l
-            cy = -t["root_half"] + (2 * t["iy"][leaves] + 1) * half_l
-            inside = (np.abs(cx - g_.X1) < g_.H1) & (np.abs(cy - g_.X2) < g_.H2)
-            wgt = (half_l ** 2) * inside
-            state["near_mean"] = float(np.sum(wgt * t["near_cnt"][t["leaf_id"][leaves]]) / max(np.sum(wgt), 1e-300))
         f.close()
 
     # host-side buffers of the e2e leg: pinned, numpy views handed to the C ABI as HOST pointers
@@ -273,7 +284,8 @@ def run_ours(args):
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         step_device()
     l0 = ml.launch_count()
     sec = timed(step_device, args.steps)
@@ -289,87 +301,115 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         # the stars of the e2e leg come from the library's own generator (read back once, outside the timing)
-        f0 = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, seed, kappa_star=cfg.kappa_star,
-                             mass_law=cfg.mass_law, mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
+        f0 = seeded(cfg)
         sx, sy, sm = f0.stars()
         f0.close()
         hx.numpy()[:], hy.numpy()[:], hm.numpy()[:] = sx, sy, sm
+        del sx, sy, sm
         step_host()
-        sec_h = timed(step_host, args.steps)
-        e2e = {"value": evals / sec_h, "unit": UNIT, "ms_per_step": sec_h * 1e3,
+        e2e_steps = args.steps if sec * args.steps < 60.0 else max(2, min(args.steps, int(60.0 / sec)))
+        sec_h = timed(step_host, e2e_steps)
+        e2e = {"value": evals / sec_h, "unit": UNIT, "ms_per_step": sec_h * 1e3, "steps": e2e_steps,
                "h2d_bytes_per_step": 3 * 8 * cfg.n_stars, "d2h_bytes_per_step": 2 * 8 * npix * npix}
 
-    # ---- roofline of the dominant kernel (fused evaluate + IPM deposit), DESIGN.md s7
-    # Algorithmic work per lens-equation evaluation: the leaf's near-field list summed directly
-    # (10 flop per star) + the leaf's order-p Taylor series by Horner (8 flop per term) + 10 flop macro and sheet.
-    # The kernel itself does less (it re-expands the series per 32x32-ray tile, order 6-15 by geometry, and folds the distant
-    # near-field stars into it): `flop_executed` counts what it really issues for the evaluation.
-    st = state["ipm"]
-    p = state["info"]["order"]
-    n_near_leaf = state["near_mean"]
-    rays_k = st["n_rays"]                                        # evaluations the kernel performed
-    flop_alg = rays_k * (10.0 * n_near_leaf + 8.0 * (p - 1) + 10.0)
-    flop_exec = 10.0 * st["n_near_terms"] + (8.0 * st["tile_order"] + 10.0) * rays_k
-    n_l = max(1, st["n_shoot_launches"])
-    dur = st["ms_shoot"] * 1e-3 / n_l
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except OSError:
         pass
+
+    # ---- roofline of the fused evaluate + IPM deposit kernel: bound by plain FP64 ALU work.
+    # Work = SURVEY 8(d)'s algorithmic flops of the paper's per-ray scheme x the UNIQUE rays of the map (tile-border
+    # corners that the kernel evaluates twice are not counted): the mean near-field list of a ray's leaf (measured in
+    # the run, per tile) summed directly + the leaf's order-p series by Horner + the macro and sheet terms.
+    # The kernel itself executes less (series re-expanded per 32 x 32-ray tile at order 6-15, distant near-field stars
+    # folded into it): `achieved_executed` counts what it really issues for the evaluation.
+    st = state["ipm"]
+    p = state["info"]["order"]
+    n_near_leaf = st["n_near_leaf_sum"] / max(1, st["n_tiles"])
+    flop_per_eval = FLOP_PER_NEAR_STAR * n_near_leaf + FLOP_PER_TERM * (p - 1) + FLOP_MACRO
+    rays_unique = evals_ipm if world == 1 else st["n_cells"]                 # N > 1: this rank's slab
+    flop_alg = rays_unique * flop_per_eval
+    flop_exec = FLOP_PER_NEAR_STAR * st["n_near_terms"] + (FLOP_PER_TERM * st["tile_order"] + FLOP_MACRO) * st["n_rays"]
+    n_l = max(1, st["n_shoot_launches"])
+    t_shoot = st["ms_shoot"] * 1e-3
     sm_max = peaks.get("sm_max_mhz", 1965.0)
     nsm = torch.cuda.get_device_properties(dev).multi_processor_count
-    peak_tf = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-    achieved_tf = flop_alg / n_l / dur / 1e12 if dur > 0 else 0.0
-    roofline = {"bound": "alu", "kernel": "shoot_ipm_kernel", "achieved": achieved_tf, "peak": peak_tf,
-                "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                "peak_source": f"{nsm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz (derived, DESIGN.md s7)",
-                "peak_measured_dfma": ml.bench_dfma() / 1e12,
-                "flop_per_eval_algorithmic": flop_alg / rays_k, "near_stars_per_leaf_mean": n_near_leaf,
+    peak_derived = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    peak_dfma = ml.bench_dfma() / 1e12
+    achieved_tf = flop_alg / t_shoot / 1e12 if t_shoot > 0 else 0.0
+    # DRAM traffic of the launches, from the run's own counters: every queued triangle is written once (48 B) by this
+    # kernel; the per-tile leaf data and the map windows are L2 hits
+    traffic = st["n_tri_queued"] * QUEUE_ENTRY_BYTES / n_l
+    roofline = {"bound": "alu", "kernel": "shoot_ipm_kernel", "achieved": achieved_tf, "peak": peak_dfma,
+                "unit": "TFLOP/s", "frac": achieved_tf / peak_dfma if peak_dfma > 0 else None,
+                "traffic": traffic,
+                "traffic_source": "n_tri_queued x 48 B of queue writes / launches (mlens_stats of the timed run); ncu dram bytes of a capture are in profiles/",
+                "peak_source": "FP64 FMA rate measured by libmlens_bench (mlens_bench_dfma) in this run",
+                "peak_derived": peak_derived,
+                "peak_derived_source": f"{nsm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz",
+                "flop_per_eval_algorithmic": flop_per_eval, "near_stars_per_leaf_mean": n_near_leaf, "order_p": p,
+                "unique_rays": rays_unique, "rays_evaluated": st["n_rays"],
                 "flop_per_launch": flop_alg / n_l, "flop_executed_per_launch": flop_exec / n_l,
-                "achieved_executed": flop_exec / n_l / dur / 1e12 if dur > 0 else 0.0,
-                "launch_ms": dur * 1e3, "launches_per_map": n_l,
-                "share_of_step": st["ms_shoot"] * 1e-3 / sec}
+                "achieved_executed": flop_exec / t_shoot / 1e12 if t_shoot > 0 else 0.0,
+                "launch_ms": t_shoot * 1e3 / n_l, "launches_per_map": n_l, "kernel_ms_per_map": st["ms_shoot"],
+                "share_of_step": t_shoot / sec}
 
-    # BASELINE.json metric: fraction of the atomic roofline for deposition.  Random 64-bit atomic adds into a buffer
-    # the size of config 1's accumulators (16 MB, L2-resident) and of config 4's (1.6 GB, HBM-resident), measured here,
-    # against what the apportioning kernels issued per second of their own time (one add per clipped pixel, two per
-    # edge step at least).
-    atomics = None
+    # ---- BASELINE.json metric: fraction of the atomic roofline for deposition.  Adds the apportioning kernels (drain,
+    # walk, giant walk) issue: one per clipped (triangle, pixel) pair, two per edge step at least -- against the rate of
+    # random 64-bit atomic adds measured here into a buffer that L2 holds (16 MB) and into one the size of this map's
+    # accumulators (HBM-resident when larger than L2).
+    roofline_atomics = None
     if world == 1:
-        st_i = state["ipm"]
-        a_l2 = ml.bench_atomics(2 * npix * npix, True)
-        a_hbm = ml.bench_atomics(200_000_000, True)
-        adds = st_i["n_px_clipped"] + 2 * st_i["n_edge_steps"]
-        rate = adds / (st_i["ms_drain"] * 1e-3)
-        atomics = {"l2_resident_adds_per_s": a_l2, "hbm_resident_adds_per_s": a_hbm, "apportioning_adds_per_s": rate,
-                   "frac_of_l2_atomic_rate": rate / a_l2, "apportioning_adds_per_map": adds}
+        a_l2 = ml.bench_atomics(2_000_000, True)
+        a_map = ml.bench_atomics(max(2 * npix * npix, 2_000_000), True)
+        adds = st["n_px_clipped"] + 2 * st["n_edge_steps"]
+        t_ap = st["ms_drain"] * 1e-3
+        rate = adds / t_ap if t_ap > 0 else 0.0
+        queue_bytes = st["n_tri_queued"] * QUEUE_ENTRY_BYTES + st["n_tri_walked"] * (QUEUE_ENTRY_BYTES + 8)
+        roofline_atomics = {"bound": "atomics", "kernels": "drain_kernel + walk_kernel + walk_giant_kernel",
+                            "achieved": rate, "peak": a_l2, "unit": "adds/s", "frac": rate / a_l2,
+                            "peak_source": "random u64 atomic adds into a 16 MB (L2-resident) buffer, libmlens_bench, this run",
+                            "map_sized_buffer_adds_per_s": a_map, "map_accumulator_bytes": 16 * npix * npix,
+                            "frac_of_map_sized_rate": rate / a_map,
+                            "adds_per_map": adds, "n_px_clipped": st["n_px_clipped"], "n_edge_steps": st["n_edge_steps"],
+                            "kernel_ms_per_map": st["ms_drain"], "walk_ms": st["ms_walk"], "giant_ms": st["ms_giant"],
+                            "traffic": queue_bytes, "traffic_source": "queue reads: n_tri_queued x 48 B + walk list n_tri_walked x 56 B (whole map)",
+                            "traffic_GBps": queue_bytes / t_ap / 1e9 if t_ap > 0 else None,
+                            "hbm_peak_GBps": peaks.get("hbm_gbs"), "share_of_step": t_ap / sec}
 
-    # the single-precision evaluator on the same workload, beside the float64 numbers
+    extras = world == 1 and not args.no_extras
+    # ---- the single-precision evaluator where the paper says single precision fails
+    # (the cluster regime, config 3) and on config 1, beside the float64 numbers
     f32 = None
-    if world == 1:
-        ff = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, seed, kappa_star=cfg.kappa_star,
-                             mass_law=cfg.mass_law, mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
-        out32 = torch.zeros((npix, npix), dtype=torch.float64, device=dev)
+    if extras:
         f32 = {}
-        for name, mode in (("ipm", ml.MAP_IPM), ("irs", ml.MAP_IRS)):
-            for _ in range(2):
-                r32 = ff.shoot(half, npix, k, out=out32, map_mode=mode, eval_mode=ml.EVAL_FMM_F32, **kw)
-            f32[name + "_map_ms"] = r32.stats["ms_total"]
-            f32[name + "_shoot_ms"] = r32.stats["ms_shoot"]
-            ref64 = map_ipm if mode == ml.MAP_IPM else map_irs
-            sel = ref64 >= 0.1
-            rel = ((out32 - ref64).abs()[sel] / ref64[sel])
-            f32[name + "_pixels_beyond_1e-3_of_f64"] = float((rel > 1e-3).double().mean())
-            f32[name + "_median_rel_dev_of_f64"] = float(rel.median())
-        f32["f64_ipm_shoot_ms"] = state["ipm"]["ms_shoot"]; f32["f64_irs_shoot_ms"] = state["irs"]["ms_shoot"]
-        ff.close()
-        del out32
+        for ci in (1, 3):
+            c2 = synth.get_config(ci)
+            kw2 = dict(border_mode=c2.border_mode, border_param=c2.border_param)
+            ff = seeded(c2)
+            a2 = (c2.half_y, c2.npix, c2.rays_per_pixel_length)
+            o64 = torch.zeros((c2.npix, c2.npix), dtype=torch.float64, device=dev)
+            o32 = torch.zeros_like(o64)
+            rec = {}
+            for name, mode in (("ipm", ml.MAP_IPM), ("irs", ml.MAP_IRS)):
+                for _ in range(2):
+                    r64 = ff.shoot(*a2, out=o64, map_mode=mode, **kw2)
+                    r32 = ff.shoot(*a2, out=o32, map_mode=mode, eval_mode=ml.EVAL_FMM_F32, **kw2)
+                rec[name + "_shoot_ms_f64"] = r64.stats["ms_shoot"]; rec[name + "_shoot_ms_f32"] = r32.stats["ms_shoot"]
+                rec[name + "_map_ms_f64"] = r64.stats["ms_total"]; rec[name + "_map_ms_f32"] = r32.stats["ms_total"]
+                sel = o64 >= 0.1
+                rel = ((o32 - o64).abs()[sel] / o64[sel])
+                rec[name + "_median_rel_dev_of_f64"] = float(rel.median())
+                rec[name + "_pixels_beyond_1e-3_of_f64"] = float((rel > 1e-3).double().mean())
+                rec[name + "_max_rel_dev_of_f64"] = float(rel.max())
+            ff.close()
+            f32[c2.name] = rec
+            del o64, o32
 
-    # the map consumers (HBM-bound): histogram of a synthetic log-normal 8192^2 map (512 MiB > L2)
+    # ---- the map consumers (HBM-bound): histogram of a synthetic log-normal 8192^2 map (512 MiB > L2)
     consumers = None
-    if world == 1:
+    if extras:
         big = torch.empty((8192, 8192), dtype=torch.float64, device=dev).log_normal_(0.0, 1.0)
         ms = []
         for _ in range(4):
@@ -377,7 +417,7 @@ def run_ours(args):
             e0.record(stream); hh = ml.histogram(big, 1.0, -2.0, 2.0, 64); e1.record(stream); e1.synchronize()
             ms.append(e0.elapsed_time(e1))
         gbs = big.numel() * 8 / (min(ms[1:]) * 1e-3) / 1e9
-        peak_hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs") if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+        peak_hbm = peaks.get("hbm_gbs")
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         lc = ml.light_curve(map_ipm, g.ylo1, g.ylo2, g.p1, g.p2, (-0.9 * half, -0.7 * half), (0.9 * half, 0.8 * half), 1 << 20,
@@ -388,20 +428,30 @@ def run_ours(args):
                      "light_curve_1M_samples_ms": e0.elapsed_time(e1), "light_curve_mean_mu": float(lc.nanmean())}
         del big
 
+    # ---- BASELINE.json's second metric, map wall-time, on the other configurations (one warm-up, one timed run each)
     maps = None
     if args.maps and world == 1:
-        # BASELINE.json's second metric, map wall-time, on the other configurations (one warm-up, one timed run each)
         maps = {}
-        for ci in [int(c) for c in args.maps.split(",") if c != ""]:
-            c2 = synth.get_config(ci)
+        for tok in [c for c in args.maps.split(",") if c != ""]:
+            rect = tok.startswith("rect")
+            c2 = synth.get_config(int(tok[4:]) if rect else int(tok))
             kw2 = dict(border_mode=c2.border_mode, border_param=c2.border_param)
             out2 = torch.zeros((c2.npix, c2.npix), dtype=torch.float64, device=dev)
             rec = {}
             for rep in range(2):
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
-                f2 = ml.Field.seeded(c2.kappa_tot, c2.gamma, c2.n_stars, c2.seed, kappa_star=c2.kappa_star,
-                                     mass_law=c2.mass_law, mass_a=c2.mass_a, mass_lo=c2.mass_lo, mass_hi=c2.mass_hi)
+                if rect:
+                    # the same lens with a RECTANGULAR star region sized for the same map (eq 20/21): side ratio
+                    # of the shooting window, area from the rectangle's own corner formula, stars at the same density
+                    g2 = seeded(c2).grid(c2.half_y, c2.npix, c2.rays_per_pixel_length, **kw2)
+                    c1r, c2r = 1.2 * g2.H1 + 10.0, 1.2 * g2.H2 + 10.0
+                    n_rect = int(round(c2.kappa_star * 4 * c1r * c2r / np.pi))
+                    f2 = ml.Field.seeded(c2.kappa_tot, c2.gamma, n_rect, c2.seed, kappa_star=c2.kappa_star, shape=ml.SHAPE_RECT,
+                                         rect_aspect=c1r / c2r, mass_law=c2.mass_law, mass_a=c2.mass_a, mass_lo=c2.mass_lo, mass_hi=c2.mass_hi)
+                    rec["n_stars_rect"] = n_rect
+                else:
+                    f2 = seeded(c2)
                 e1.record(stream); e1.synchronize()
                 rec["create_ms"] = e0.elapsed_time(e1)
                 for name, mode in (("ipm", ml.MAP_IPM), ("irs", ml.MAP_IRS)):
@@ -414,27 +464,65 @@ def run_ours(args):
                     if mode == ml.MAP_IPM:
                         rec["ipm_drain_walk_ms"] = r.stats["ms_drain"]
                         rec["ipm_bands"] = r.stats["n_bands"]
-                        rec["tri"] = {k: r.stats[k] for k in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
-                                                              "n_px_clipped", "n_edge_steps")}
+                        rec["tri"] = {k_: r.stats[k_] for k_ in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
+                                                                  "n_px_clipped", "n_edge_steps")}
                         rec["queue_overflow"] = r.stats["n_queue_overflow"]
                         rec["mean_mu"] = float(out2.mean())
                 rec["order_p"] = f2.info()["order"]
+                rec["n_levels"] = f2.info()["n_levels"]
                 f2.close()
-            maps[workload_name(c2)] = rec
+            maps[("rect variant of " if rect else "") + workload_name(c2)] = rec
             del out2
+
+    # ---- load balance of row slabs without a second GPU: 8 slabs of config 1 shot one after another, equal
+    # rows against star-weighted rows (the weight per star fitted from the equal-row times)
+    slab_balance = None
+    if extras:
+        c2 = synth.get_config(1)
+        kw2 = dict(border_mode=c2.border_mode, border_param=c2.border_param)
+        f2 = seeded(c2)
+        a2 = (c2.half_y, c2.npix, c2.rays_per_pixel_length)
+        g2 = f2.grid(*a2, **kw2)
+        ys = f2.stars()[1]
+        out2 = torch.zeros((c2.npix, c2.npix), dtype=torch.float64, device=dev)
+        n2 = int(g2.n2)
+
+        def slab_times(weights, nslab=8):
+            ts, rows, stars = [], [], []
+            for r in range(nslab):
+                j0, j1 = multi.slab_bounds(n2, nslab, r, weights=weights)
+                for _ in range(2):
+                    rr = f2.shoot(*a2, sub=(0, int(g2.n1), j0, j1), out=out2, **kw2)
+                ts.append(rr.stats["ms_total"]); rows.append(j1 - j0)
+                jj = np.floor((ys - g2.x0_2) / g2.h2)
+                stars.append(int(np.sum((jj >= j0) & (jj < j1))))
+            return np.array(ts), np.array(rows, dtype=float), np.array(stars, dtype=float)
+
+        t_eq, rows_eq, stars_eq = slab_times(None)
+        A = np.stack([rows_eq, stars_eq], axis=1)
+        coef, *_ = np.linalg.lstsq(A, t_eq, rcond=None)
+        per_star = float(max(coef[1], 0.0) / coef[0]) if coef[0] > 0 else 0.0
+        t_w, _, _ = slab_times(multi.star_row_weights(ys, g2.x0_2, g2.h2, n2, per_star=per_star))
+        slab_balance = {"workload": workload_name(c2), "slabs": 8,
+                        "equal_rows_ms": [float(v) for v in t_eq], "equal_rows_max_over_mean": float(t_eq.max() / t_eq.mean()),
+                        "fitted_ms_per_row": float(coef[0]), "fitted_ms_per_star": float(coef[1]), "per_star_in_rows": per_star,
+                        "weighted_ms": [float(v) for v in t_w], "weighted_max_over_mean": float(t_w.max() / t_w.mean())}
+        f2.close()
+        del out2
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        e, t, thr, sub = oracle_sample(cfg, (384, 384))
+        patch = oracle_patch_for(cfg, 20.0, os.cpu_count() or 16)
+        e, t, thr, sub = oracle_sample(cfg, patch)
         cpu = {"value": e / t, "unit": UNIT, "cores": thr, "kind": "oracle", "seconds": t,
-               "sample": f"IPM + IRS on the 384x384-cell patch {sub} at the window centre "
+               "sample": f"IPM + IRS on the {patch[0]}x{patch[1]}-cell patch {sub} at the window centre "
                          f"({e} evaluations, each a direct sum over all {cfg.n_stars} stars)"}
 
     if rank == 0:
         irs = state["irs"]
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "strong",
+            "warmup": warm, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "strong",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "rays_ipm": evals_ipm, "rays_irs": evals_irs,
                        "stars_seed": seed, "order_p": p, "tile_order": state["ipm"]["tile_order"], "border": "eq16",
@@ -442,14 +530,17 @@ def run_ours(args):
                        "parallelism": (f"{world} GPUs: star-weighted row slabs of one map + all-reduce of the map "
                                        f"(rank 0 rows {state['slab']})") if world > 1 else "1 GPU"},
             "phases_ms": {"ipm_map": st["ms_total"], "ipm_shoot_kernels": st["ms_shoot"], "ipm_drain_and_walk_kernels": st["ms_drain"],
+                          "ipm_walk_kernel": st["ms_walk"], "ipm_giant_kernel": st["ms_giant"], "ipm_bands": st["n_bands"],
                           "irs_map": irs["ms_total"], "irs_shoot_kernels": irs["ms_shoot"],
                           "create_and_rest": sec * 1e3 - st["ms_total"] - irs["ms_total"]},
-            "ipm_map_wall_ms": st["ms_total"],
-            "evals_per_s_ipm_kernel": rays_k / (st["ms_shoot"] * 1e-3) if st["ms_shoot"] > 0 else None,
+            "ipm_map_wall_ms": st["ms_total"], "irs_map_wall_ms": irs["ms_total"],
+            "evals_per_s_ipm_kernel": evals_ipm / t_shoot if t_shoot > 0 and world == 1 else None,
+            "evals_per_s_irs_kernel": evals_irs / (irs["ms_shoot"] * 1e-3) if irs["ms_shoot"] > 0 and world == 1 else None,
             "triangles": {k_: st[k_] for k_ in ("n_tri_single", "n_tri_strip", "n_tri_queued", "n_tri_walked",
-                                                  "n_queue_overflow", "n_px_clipped", "n_edge_steps", "n_rays_fallback")},
+                                                  "n_queue_overflow", "n_px_clipped", "n_edge_steps", "n_giant_chunks", "n_rays_fallback")},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-            "roofline": roofline, "cpu_baseline": cpu, "atomics": atomics, "f32_mode": f32, "consumers": consumers, "maps": maps,
+            "roofline": roofline, "roofline_atomics": roofline_atomics, "cpu_baseline": cpu,
+            "f32_mode": f32, "consumers": consumers, "maps": maps, "slab_balance": slab_balance,
         }))
     if world > 1:
         dist.destroy_process_group()

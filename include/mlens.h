@@ -175,6 +175,12 @@ typedef struct {
     int64_t n_tiles_full;          /* tile slots whose truncation bound failed (evaluated with the leaf's full series) */
     int32_t tile_order;            /* order of the per-tile series */
     int32_t pad_;
+    float ms_walk;                 /* of ms_drain: the edge-walk launches (walk_kernel) */
+    float ms_giant;                /* of ms_drain: the launches that walk the giant triangles chunk by chunk */
+    int64_t n_giant_chunks;        /* chunks of edge steps the giant triangles were shared out in */
+    int64_t n_tiles;               /* ray tiles (32 x 32 rays) evaluated with a leaf under their first corner */
+    int64_t n_near_leaf_sum;       /* sum over those tiles of the near-field list length of that leaf: divided by n_tiles,
+                                      the mean number of stars the paper's per-ray scheme sums directly (eq 23) */
 } mlens_stats;
 
 int mlens_version(void);

@@ -141,10 +141,14 @@ __device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, do
     E.ta = ta; E.tb = tb;
     // An end cut by a border row of the map lies ON that row line: it takes the line's exact (integer) value of y,
     // as the ends on grid lines and vertices do, so that the covers G(y) of all the edges that cross the border
-    // telescope there too.  (A row line cuts an edge strictly inside only if it is the map's first or last one.)
+    // telescope there too.  A row line lies strictly between the edge's ends only if it is the map's first or last
+    // one (ry0 = 0 and ry1 = the top of the bounding box never do: every vertex lies between them) -- decided on the
+    // coordinates themselves, not on the parameters, whose rounding can put a vertex that sits ON such a line inside.
     int cf = 0;
-    if (ta == tlo && ta > 0.0) cf |= (E.dy > 0.0) ? 1 : 2;
-    if (tb == thi && tb < 1.0) cf |= (E.dy > 0.0) ? 8 : 4;
+    const double ylo = fmin(y0, y1), yhi = fmax(y0, y1);
+    const double ls = (E.dy > 0.0) ? ry0 : ry1, le = (E.dy > 0.0) ? ry1 : ry0;     // row lines where the edge enters / leaves the map
+    if (ta == tlo && ls > ylo && ls < yhi) cf |= (E.dy > 0.0) ? 1 : 2;
+    if (tb == thi && le > ylo && le < yhi) cf |= (E.dy > 0.0) ? 8 : 4;
     E.cf = cf;
     E.majorY = fabs(E.dy) >= fabs(E.dx);
     const double d = E.majorY ? E.dy : E.dx, c0 = E.majorY ? y0 : x0;

@@ -210,7 +210,9 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
 
         const long long ci = ci0 + lane;
         const bool colv = ci <= S.n1, cellv = (lane < TCX - 1) && (ci >= S.i0) && (ci < S.i1);
-        const bool dumpc = (ci >= S.i0) && (ci <= S.i1);
+        // (a corner on a tile border is evaluated by both tiles, each with its own series: the dump takes it from the
+        // tile that holds the cell to its left / below, so that it does not depend on which tile runs last)
+        const bool dumpc = (ci >= S.i0) && (ci <= S.i1) && (lane > 0 || ci == S.i0);
         const double x = corner_x(S, ci), ux = ((double)lane - 0.5 * (TCX - 1)) * S.dux;
         // row groups that hold a corner row of the sub-range
         const int g_lo = (S.j0 > cj0) ? (int)((S.j0 - cj0) / RPT) : 0;
@@ -235,7 +237,7 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
 #pragma unroll
                 for (int r = 0; r < RPT; ++r) {
                     const long long cj = cj0 + g * RPT + r;
-                    vm |= (valid[r] && dumpc && cj >= S.j0 && cj <= S.j1) ? (1u << r) : 0u;
+                    vm |= (valid[r] && dumpc && cj >= S.j0 && cj <= S.j1 && (g * RPT + r > 0 || cj == S.j0)) ? (1u << r) : 0u;
                 }
                 dump_rays(&S, (cj0 + g * RPT - S.j0) * ncx + (ci - S.i0), ncx, vm,
                           wx[0], wy[0], wx[1], wy[1], wx[2], wy[2], wx[3], wy[3]);
@@ -453,6 +455,7 @@ __global__ void __launch_bounds__(256) walk_giant_kernel(const __grid_constant__
     const int lane = threadIdx.x & 31;
     long long n = (long long)S.counters[C_GIANT];
     if (n > S.giant_cap) n = S.giant_cap;
+    if (blockIdx.x == 0 && threadIdx.x == 0 && n) atomicAdd(&S.counters[C_ROWS], (unsigned long long)n);    // chunks, all bands
     unsigned long long n_pieces = 0;
     while (true) {
         long long i = 0;
@@ -864,7 +867,9 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
                 rate = (rate < 0.0) ? 1.25 * r_new : fmax(1.25 * r_new, 0.7 * rate);   // head-room; forget slowly
             }
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
+            ML_TRY(mark());
             ML_LAUNCH(walk_kernel, nsm * 4, WALK_WARPS * 32, 0, s, S);
+            ML_TRY(mark());
             ML_LAUNCH(walk_giant_kernel, nsm * 8, 256, 0, s, S);
             ML_TRY(mark());
             launches += 4;
@@ -898,15 +903,21 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         st->n_px_strip = (int64_t)h[C_PX_SMALL]; st->n_px_clipped = (int64_t)h[C_PX_INT];
         st->n_edge_steps = (int64_t)h[C_PX_EDGE];
         st->n_tiles_full = (int64_t)h[C_TILES_FULL];
+        st->n_giant_chunks = (int64_t)h[C_ROWS];
+        st->n_tiles = (int64_t)h[C_TILES]; st->n_near_leaf_sum = (int64_t)h[C_NEAR_LEAF];
         st->tile_order = S.tq;
         st->n_bands = bands; st->gpu_launches = launches; st->n_shoot_launches = bands;
         if (timed) {
             ML_CUDA(cudaEventElapsedTime(&st->ms_total, e0, e1)); cudaEventDestroy(e0); cudaEventDestroy(e1);
-            const size_t per = ipm ? 3 : 2;              // events per band
+            const size_t per = ipm ? 5 : 2;              // events per band
             for (int b = 0; b < bands; ++b) {
                 float ms = 0;
                 ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per], ev[b * per + 1])); st->ms_shoot += ms;
-                if (ipm) { ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 1], ev[b * per + 2])); st->ms_drain += ms; }
+                if (ipm) {
+                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 1], ev[b * per + 4])); st->ms_drain += ms;
+                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 2], ev[b * per + 3])); st->ms_walk += ms;
+                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 3], ev[b * per + 4])); st->ms_giant += ms;
+                }
             }
             float ms = 0;
             ML_CUDA(cudaEventElapsedTime(&ms, ev[ev.size() - 2], ev[ev.size() - 1])); st->ms_finalise = ms;

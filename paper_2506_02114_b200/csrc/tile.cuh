@@ -25,7 +25,7 @@ static const int BN = 2 * ML_P1MAX;   // stride of the Pascal triangle
 
 // slots of ShootDev::counters
 enum { C_QUEUE = 0, C_TILE, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR,
-       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_BIG, C_WALK, C_GIANT, C_GWALK, C_NCOUNTERS };
+       C_PX_SMALL, C_PX_INT, C_PX_EDGE, C_ROWS, C_TILES_FULL, C_DRAIN, C_BIG, C_WALK, C_GIANT, C_GWALK, C_TILES, C_NEAR_LEAF, C_NCOUNTERS };
 
 // What a shooting kernel needs besides the lens: the ray grid, the map, the accumulators.
 struct ShootDev {
@@ -261,6 +261,11 @@ static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShar
         if (W.leaf[s] < 0) continue;                              // warp-uniform
         wtile_build_slot(S, W, C, s, rt);
         if (lane == 0 && W.mode[s] == 1 && full_counter) atomicAdd(full_counter, 1ull);
+    }
+    if (lane == 0 && W.leaf[0] >= 0) {
+        // statistics: the near-field list a ray of this tile would sum in the paper's per-ray scheme (roofline accounting)
+        atomicAdd(&S.counters[C_TILES], 1ull);
+        atomicAdd(&S.counters[C_NEAR_LEAF], (unsigned long long)__ldg(&S.L.near_cnt[W.leaf[0]]));
     }
     zero_window(W);
     // eq 19 inside the disc is linear in z: the farthest ray of the tile decides (the disc is convex)

@@ -80,7 +80,9 @@ class Stats(C.Structure):
                 ("ms_total", C.c_float), ("ms_shoot", C.c_float), ("ms_drain", C.c_float),
                 ("ms_finalise", C.c_float), ("n_shoot_launches", C.c_int32), ("n_near_terms", C.c_int64),
                 ("n_px_strip", C.c_int64), ("n_px_clipped", C.c_int64), ("n_edge_steps", C.c_int64), ("reserved_", C.c_int64),
-                ("n_tiles_full", C.c_int64), ("tile_order", C.c_int32), ("pad_", C.c_int32)]
+                ("n_tiles_full", C.c_int64), ("tile_order", C.c_int32), ("pad_", C.c_int32),
+                ("ms_walk", C.c_float), ("ms_giant", C.c_float), ("n_giant_chunks", C.c_int64),
+                ("n_tiles", C.c_int64), ("n_near_leaf_sum", C.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
