@@ -163,22 +163,22 @@ __device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, do
     E.n = ((nc > 0.0) ? (int)fmin(nc, 1.0e7) : 0) + 1;
 }
 
-// One piece of an edge, from (xs, ys) to (xe, ye), inside one pixel.  cs = -sign(A) ONE/|A|; (bx, by) = integer
-// origin of the local coordinates.  The cover G(ye) - G(ys) telescopes exactly along the triangle's boundary.
-__device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, double ys, double xe, double ye, double cs, int bx, int by) {
-    const long long tcov = __double2ll_rn(cs * ye) - __double2ll_rn(cs * ys);
+// One piece of an edge, from (xs, ys) to (xe, ye), inside one pixel, with cover tcov = G(ye) - G(ys), G(y) = rn(cs y),
+// cs = -sign(A) ONE/|A|; (bx, by) = integer origin of the local coordinates.  The covers telescope exactly along the
+// triangle's boundary because consecutive pieces share the value of G at the point where they meet.
+__device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, double ys, double xe, double ye, long long tcov, int bx, int by) {
     if (tcov == 0) return;
     const double ym = 0.5 * (ys + ye), xm = 0.5 * (xs + xe);
-    const int jr = (int)floor(ym) + by;
+    const int jr = __double2int_rd(ym) + by;                   // (coordinates are bounded by 1e9: no saturation)
     if ((unsigned)jr >= (unsigned)S.npix2) return;
-    const double fi = floor(xm);
-    const int ic = (int)fi + bx;
+    const int il = __double2int_rd(xm);
+    const int ic = il + bx;
     if (ic >= S.npix1) return;
     unsigned long long *row = S.diff + (size_t)jr * S.npix1;
     long long r = tcov;                                        // left of the map: the whole cover enters at column 0
     int c0 = 0;
     if (ic >= 0) {
-        const double m = clamp01(xm - fi);
+        const double m = clamp01(xm - (double)il);
         r = __double2ll_rn((double)tcov * m);
         c0 = ic + 1;
         if (tcov != r) atomicAdd(row + ic, (unsigned long long)(tcov - r));
@@ -186,50 +186,70 @@ __device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, doub
     if (c0 < S.npix1 && r != 0) atomicAdd(row + c0, (unsigned long long)r);
 }
 
-// Step k of an edge (0 <= k < n): from major-axis grid line k-1 (or the clipped start) to grid line k (or the
-// clipped end).  End points on a grid line take its exact value and an unclipped end the vertex itself, so
-// consecutive steps and consecutive edges share their end points bit for bit.  The edge comes in (major, other)
-// coordinates: c0 -> c1 along the axis that is walked, oc0 -> o1 along the other, id / oid the reciprocals of the
-// two extents (0 for an extent of 0), [ta, tb] the clipped parameter range, g0 the first grid line, sg the direction.
-__device__ __forceinline__ void edge_step_mo(const ShootDev &S, double c0, double oc0, double c1, double o1, double id, double oid,
-                                             double ta, double tb, double g0, double sg, bool my, int cf, int n, int k,
-                                             double cs, int bx, int by) {
+// An edge in (major, other) order, as the walk reads it (EREC doubles, e.g. in shared memory): c0 -> c1 along the axis
+// that is walked, oc0 -> o1 along the other, id / oid the reciprocals of the two extents (0 for an extent of 0),
+// [ta, tb] the clipped parameter range, g0 the first grid line; q[9] packs the step count n (high word) with the
+// flags: bit 0 major axis is y, bit 1 walking towards smaller coordinates, bits 2-5 the border-row flags cf.
+static const int EREC = 10;
+__device__ __forceinline__ void edge_record(const EdgeWalk &E, double *q) {
+    const bool my = E.majorY != 0;
+    q[0] = my ? E.y0 : E.x0; q[1] = my ? E.x0 : E.y0; q[2] = my ? E.y1 : E.x1; q[3] = my ? E.x1 : E.y1;
+    q[4] = my ? E.idy : E.idx; q[5] = my ? E.idx : E.idy; q[6] = E.ta; q[7] = E.tb; q[8] = E.g0;
+    q[9] = __hiloint2double(E.n, E.majorY | (E.sg < 0.0 ? 2 : 0) | (E.cf << 2));
+}
+__device__ __forceinline__ int edge_record_steps(const double *q) { return __double2hiint(q[9]); }
+
+// Steps [m0, m1) of an edge, 0 <= m0 < m1 <= n.  Step k runs from major-axis grid line k-1 (or the clipped start) to
+// grid line k (or the clipped end).  End points on a grid line take its exact value, an unclipped end the vertex
+// itself, an end cut by a border row of the map that row line's value: consecutive steps and consecutive edges share
+// their end points bit for bit.  A lane walks CONSECUTIVE steps: the end of a step (its coordinates and G) is carried
+// into the next one, so that every point of the edge is computed once.
+__device__ __forceinline__ void edge_run(const ShootDev &S, const double *q, int m0, int m1, double cs, int bx, int by) {
+    const double c0 = q[0], oc0 = q[1], c1 = q[2], o1 = q[3], id = q[4], oid = q[5], ta = q[6], tb = q[7], g0 = q[8];
+    const int fl = __double2loint(q[9]), n = __double2hiint(q[9]);
+    const bool my = (fl & 1) != 0;
+    const double sg = (fl & 2) ? -1.0 : 1.0;
+    const int cf = fl >> 2;
     const double d = c1 - c0, od = o1 - oc0;
-    double ms, os, me, oe, ts, te;
-    if (k == 0) {
+    double ms, os, ts;
+    if (m0 == 0) {
         ts = ta; ms = (ts == 0.0) ? c0 : fma(ts, d, c0); os = (ts == 0.0) ? oc0 : fma(ts, od, oc0);
         if (cf & 3) {                                          // start on a border row of the map: exactly on it
             const double yl = (cf & 1) ? (double)(-by) : (double)(S.npix2 - by);
             if (my) ms = yl; else os = yl;
         }
-    } else { ms = g0 + sg * (double)(k - 1); ts = dmin(dmax((ms - c0) * id, ta), tb); os = fma(ts, od, oc0); }
-    if (k == n - 1) {
-        te = tb;
-        const bool vtx = (te == 1.0);
-        me = vtx ? c1 : fma(te, d, c0);
-        oe = vtx ? o1 : fma(te, od, oc0);
-        if (cf & 12) {
-            const double yl = (cf & 4) ? (double)(-by) : (double)(S.npix2 - by);
-            if (my) me = yl; else oe = yl;
+    } else { ms = g0 + sg * (double)(m0 - 1); ts = dmin(dmax((ms - c0) * id, ta), tb); os = fma(ts, od, oc0); }
+    long long Gs = __double2ll_rn(cs * (my ? ms : os));
+#pragma unroll 1
+    for (int k = m0; k < m1; ++k) {
+        double me, oe, te;
+        if (k == n - 1) {
+            te = tb;
+            const bool vtx = (te == 1.0);
+            me = vtx ? c1 : fma(te, d, c0);
+            oe = vtx ? o1 : fma(te, od, oc0);
+            if (cf & 12) {
+                const double yl = (cf & 4) ? (double)(-by) : (double)(S.npix2 - by);
+                if (my) me = yl; else oe = yl;
+            }
+        } else { me = g0 + sg * (double)k; te = dmin(dmax((me - c0) * id, ta), tb); oe = fma(te, od, oc0); }
+        const long long Ge = __double2ll_rn(cs * (my ? me : oe));
+        // at most one grid line of the other axis lies strictly between os and oe
+        const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
+        const bool cross = (od != 0.0) && ((oe > os) ? (gl < oe) : (gl > oe)) && (oe != os);
+        double mg = me, og = oe;                               // where the first piece ends
+        long long Gg = Ge;
+        if (cross) {
+            const double tg = dmin(dmax((gl - oc0) * oid, ts), te);
+            mg = fma(tg, d, c0); og = gl;
+            Gg = __double2ll_rn(cs * (my ? mg : og));
         }
-    } else { me = g0 + sg * (double)k; te = dmin(dmax((me - c0) * id, ta), tb); oe = fma(te, od, oc0); }
-    // at most one grid line of the other axis lies strictly between os and oe
-    const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
-    const bool cross = (od != 0.0) && ((oe > os) ? (gl < oe) : (gl > oe)) && (oe != os);
-    double mg = me, og = oe;                                   // where the first piece ends
-    if (cross) {
-        const double tg = dmin(dmax((gl - oc0) * oid, ts), te);
-        mg = fma(tg, d, c0); og = gl;
+        // the axes are swapped back before the deposit, so that one copy of it serves all lanes: the first piece,
+        // then the second of those that cross
+        piece_deposit(S, my ? os : ms, my ? ms : os, my ? og : mg, my ? mg : og, Gg - Gs, bx, by);
+        if (cross) piece_deposit(S, my ? og : mg, my ? mg : og, my ? oe : me, my ? me : oe, Ge - Gg, bx, by);
+        ms = me; os = oe; ts = te; Gs = Ge;
     }
-    // the axes are swapped back before the deposit, so that one copy of it serves all lanes: the first piece,
-    // then the second of those that cross
-    piece_deposit(S, my ? os : ms, my ? ms : os, my ? og : mg, my ? mg : og, cs, bx, by);
-    if (cross) piece_deposit(S, my ? og : mg, my ? mg : og, my ? oe : me, my ? me : oe, cs, bx, by);
-}
-__device__ __forceinline__ void edge_step(const ShootDev &S, const EdgeWalk &E, int k, double cs, int bx, int by) {
-    const bool my = E.majorY != 0;
-    edge_step_mo(S, my ? E.y0 : E.x0, my ? E.x0 : E.y0, my ? E.y1 : E.x1, my ? E.x1 : E.y1, my ? E.idy : E.idx, my ? E.idx : E.idy,
-                 E.ta, E.tb, E.g0, E.sg, my, E.cf, E.n, k, cs, bx, by);
 }
 
 struct TriSetup {
@@ -401,14 +421,11 @@ __device__ __forceinline__ unsigned apportion_batch(const ShootDev &S, const Win
     return bigmask;
 }
 
-// Warp-cooperative edge walk of one large triangle (v = its 3 vertices in pixel units, same in all lanes).
-// Lanes 0-2 set up one edge each into `scratch` (3 x 16 doubles of the warp's shared memory); then the steps
-// of all three edges form one index space the lanes stride over, so a triangle of a few dozen steps still
-// fills the warp.
-// Only the steps [k_lo, k_hi) of the triangle's step index space are walked (a giant triangle is shared out in
-// chunks; every chunk sets the same edges up, so the chunks' end points still agree bit for bit).
-__device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT], double *scratch,
-                                                            int k_lo = 0, int k_hi = 0x7fffffff) {
+// Warp-cooperative edge walk of one large triangle (v = its 3 vertices in pixel units, same in all lanes): the cold
+// copy, for the triangles that found the walk list or the queue full.  Lanes 0-2 set up one edge each into `scratch`
+// (3 x EREC doubles of the warp's shared memory); then the lanes take runs of consecutive steps of each edge in turn.
+static const int RUN = 8;             // consecutive steps of an edge a lane walks at a time
+__device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT], double *scratch) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
@@ -422,33 +439,26 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
     const double fbx = (double)bx, fby = (double)by;
     const double hgt = fmax(v[1], fmax(v[3], v[5])) - fby + 1.0;
     const double ry0 = fmax(0.0, -fby), ry1 = fmin(hgt, (double)S.npix2 - fby), cx1 = (double)S.npix1 - fbx;
-    int ne = 0;
     __syncwarp();
     if (lane < 3) {
         const double xa = (lane == 0) ? v[0] : (lane == 1) ? v[2] : v[4], ya = (lane == 0) ? v[1] : (lane == 1) ? v[3] : v[5];
         const double xb = (lane == 0) ? v[2] : (lane == 1) ? v[4] : v[0], yb = (lane == 0) ? v[3] : (lane == 1) ? v[5] : v[1];
         EdgeWalk E;
         edge_setup(E, xa - fbx, ya - fby, xb - fbx, yb - fby, ry0, ry1, cx1);
-        double *q = scratch + 16 * lane;
-        q[0] = E.x0; q[1] = E.y0; q[2] = E.x1; q[3] = E.y1; q[4] = E.dx; q[5] = E.dy; q[6] = E.idx; q[7] = E.idy;
-        q[8] = E.ta; q[9] = E.tb; q[10] = E.g0; q[11] = E.sg; q[12] = __hiloint2double(E.n, E.majorY | (E.cf << 1));
-        ne = E.n;
+        edge_record(E, scratch + EREC * lane);
     }
-    const int n0 = __shfl_sync(full, ne, 0), n1 = __shfl_sync(full, ne, 1), n2 = __shfl_sync(full, ne, 2);
-    const int total = n0 + n1 + n2;
     __syncwarp();
-    const int k_end = min(total, k_hi);
+    unsigned long long total = 0;
 #pragma unroll 1
-    for (int k = k_lo + lane; k < k_end; k += 32) {
-        const int e = (k >= n0 + n1) ? 2 : (k >= n0 ? 1 : 0);
-        const double *q = scratch + 16 * e;
-        EdgeWalk E;
-        E.x0 = q[0]; E.y0 = q[1]; E.x1 = q[2]; E.y1 = q[3]; E.dx = q[4]; E.dy = q[5]; E.idx = q[6]; E.idy = q[7];
-        E.ta = q[8]; E.tb = q[9]; E.g0 = q[10]; E.sg = q[11]; E.majorY = __double2loint(q[12]) & 1; E.cf = __double2loint(q[12]) >> 1; E.n = __double2hiint(q[12]);
-        edge_step(S, E, k - (e == 2 ? n0 + n1 : (e == 1 ? n0 : 0)), cs, bx, by);
+    for (int e = 0; e < 3; ++e) {
+        const double *q = scratch + EREC * e;
+        const int n = edge_record_steps(q);
+        total += (unsigned long long)n;
+#pragma unroll 1
+        for (int m0 = lane * RUN; m0 < n; m0 += 32 * RUN) edge_run(S, q, m0, min(m0 + RUN, n), cs, bx, by);
     }
     __syncwarp();
-    return (unsigned long long)max(k_end - k_lo, 0);
+    return total;
 }
 
 // The shooting kernel's own copy, for the triangles it could not hand to the global queue (queue full).

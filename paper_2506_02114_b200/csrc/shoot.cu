@@ -330,20 +330,24 @@ __global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_co
     if (lane == 0 && n_clipped) atomicAdd(&S.counters[C_PX_INT], (unsigned long long)n_clipped);
 }
 
-// Edge walk of the large triangles the drain set aside.  A warp takes WB triangles at a time: lane = triangle
-// for the local frame, lane = edge for the clipped edges (records in shared memory); then the steps of all the
-// edges form one index space the lanes stride over, so the set-up is shared by a whole batch and a triangle
-// of a few dozen steps costs a few dozen lane-steps.  The next batch is fetched while this one is walked.
+// Edge walk of the large triangles the drain set aside.  A warp takes WB triangles at a time, in list order (the
+// list follows the order of the tiles, so the triangles in flight at any moment deposit into neighbouring rows of
+// `diff`): lane = triangle for the local frame, lane = edge for the clipped edges (records in shared memory); then the
+// RUNS of consecutive steps of all the edges form one index space the lanes stride over, so the set-up is shared by a
+// whole batch, a triangle of a few dozen steps costs a few dozen lane-steps, and a lane that walks consecutive steps
+// computes every point of its edge once (deposit.cuh).  The next batch is fetched while this one is walked.
 static const int WALK_WARPS = 8;
 static const int WB = 16;              // triangles per batch
-static const int EREC = 10;            // doubles per edge record
 static const int GIANT_STEPS = 1024;   // a triangle with more steps than this is not walked by one warp alone
-static const int GIANT_CHUNK = 512;    // but in chunks of this many steps, one warp each
-__global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_kernel(const __grid_constant__ ShootDev S) {
+static const int GIANT_CHUNK = 512;    // but edge by edge in chunks of this many steps: 32 lanes x GIANT_RUN consecutive steps
+static const int GIANT_RUN = GIANT_CHUNK / 32;
+__global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_constant__ ShootDev S) {
     __shared__ double er_s[WALK_WARPS][3 * WB][EREC];
     __shared__ double tr_s[WALK_WARPS][WB][8];           // local vertices, cs, (bx, by)
+    __shared__ int pre_s[WALK_WARPS][3 * WB];            // inclusive prefix of the runs of the batch's edges
     double (*er)[EREC] = er_s[threadIdx.x >> 5];
     double (*tr)[8] = tr_s[threadIdx.x >> 5];
+    int *pre = pre_s[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     long long nb = (long long)S.counters[C_BIG];
@@ -358,7 +362,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_kernel(const __grid_c
         long long bnext = 0;
         if (lane == 0) bnext = (long long)atomicAdd(&S.counters[C_WALK], 1ull);
         // ---- lane = triangle: local frame
-        const long long it = b + (long long)lane * nbatch;      // strided: the giant triangles of one star's tiles sit next to each other in the list
+        const long long it = b * WB + lane;
         int status = 0;
         double ry0 = 0.0, ry1 = 0.0, cx1 = 0.0;
         if (lane < WB && it < nb) {
@@ -386,91 +390,133 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 4) walk_kernel(const __grid_c
             if (ed < 3 * WB) {
                 EdgeWalk E;
                 E.n = 0; E.majorY = 1; E.sg = 1.0; E.cf = 0;
-                double *q = er[ed];
+                E.x0 = E.y0 = E.x1 = E.y1 = E.idx = E.idy = E.ta = E.tb = E.g0 = 0.0;
                 if (st == 1) {
                     const int e1 = (e == 2) ? 0 : e + 1;
                     const double *t = tr[ti];
                     edge_setup(E, t[2 * e], t[2 * e + 1], t[2 * e1], t[2 * e1 + 1], r0, r1, c1);
-                    const bool my = E.majorY != 0;                    // stored in (major, other) order: no selects per step
-                    q[0] = my ? E.y0 : E.x0; q[1] = my ? E.x0 : E.y0; q[2] = my ? E.y1 : E.x1; q[3] = my ? E.x1 : E.y1;
-                    q[4] = my ? E.idy : E.idx; q[5] = my ? E.idx : E.idy; q[6] = E.ta; q[7] = E.tb; q[8] = E.g0;
                 }
-                q[9] = __hiloint2double(E.n, E.majorY | (E.sg < 0.0 ? 2 : 0) | (E.cf << 2));
-
+                edge_record(E, er[ed]);
             }
         }
         __syncwarp();
-        // steps per triangle (lane < WB) and their inclusive prefix
+        // steps per triangle (lane < WB); a giant is shared out edge by edge in chunks to walk_giant_kernel
         int ntot = 0;
-        if (lane < WB) ntot = __double2hiint(er[3 * lane][9]) + __double2hiint(er[3 * lane + 1][9]) + __double2hiint(er[3 * lane + 2][9]);
+        if (lane < WB) ntot = edge_record_steps(er[3 * lane]) + edge_record_steps(er[3 * lane + 1]) + edge_record_steps(er[3 * lane + 2]);
         if (ntot > GIANT_STEPS) {
-            // too many steps for one warp (the faint images of the whole map): shared out in chunks to walk_giant_kernel
-            const int nch = (ntot + GIANT_CHUNK - 1) / GIANT_CHUNK;
-            const unsigned long long at = atomicAdd(&S.counters[C_GIANT], (unsigned long long)nch);
+            int nch = 0;
+#pragma unroll
+            for (int e = 0; e < 3; ++e) nch += (edge_record_steps(er[3 * lane + e]) + GIANT_CHUNK - 1) / GIANT_CHUNK;
+            unsigned long long at = atomicAdd(&S.counters[C_GIANT], (unsigned long long)nch);
             if ((long long)(at + nch) <= S.giant_cap) {           // (else it stays here; the skipped slots keep their sentinel)
-                for (int c = 0; c < nch; ++c) S.giant[at + c] = ((unsigned long long)it << 20) | (unsigned long long)c;
-                ntot = 0;
+                for (int e = 0; e < 3; ++e) {
+                    const int ne = (edge_record_steps(er[3 * lane + e]) + GIANT_CHUNK - 1) / GIANT_CHUNK;
+                    for (int c = 0; c < ne; ++c) S.giant[at++] = ((unsigned long long)it << 20) | ((unsigned long long)e << 18) | (unsigned long long)c;
+                }
+                ntot = -1;                                          // gone
             }
         }
-        int inc = ntot;
+        // ---- runs per edge and their inclusive prefix (lane = edge, two passes)
+        int total = 0;
 #pragma unroll
-        for (int o = 1; o < WB; o <<= 1) { int t = __shfl_up_sync(full, inc, o); if (lane >= o) inc += t; }
-        const int total = __shfl_sync(full, inc, WB - 1);
+        for (int ps = 0; ps < 2; ++ps) {
+            const int ed = ps * 32 + lane, tis = min(ed / 3, WB - 1);
+            const int nt = __shfl_sync(full, ntot, tis);
+            int inc = (ed < 3 * WB && nt > 0) ? (edge_record_steps(er[ed]) + RUN - 1) / RUN : 0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(full, inc, o); if (lane >= o) inc += t; }
+            if (ed < 3 * WB) pre[ed] = total + inc;
+            total += __shfl_sync(full, inc, 31);
+        }
+        __syncwarp();
+        int steps = 0;
 #pragma unroll 1
-        for (int k0 = 0; k0 < total; k0 += 32) {
-            const int k = k0 + lane;
-            int i = 0;                                              // first triangle whose inclusive prefix exceeds k
+        for (int r0 = 0; r0 < total; r0 += 32) {
+            const int r = r0 + lane;
+            if (r < total) {
+                int lo = 0, hi = 3 * WB - 1;                        // first edge whose inclusive prefix exceeds r
 #pragma unroll
-            for (int step = WB / 2; step; step >>= 1) {
-                int v = __shfl_sync(full, inc, i + step - 1);
-                if (v <= k) i += step;
-            }
-            i = min(i, WB - 1);
-            const int incl = __shfl_sync(full, inc, i), cnt = __shfl_sync(full, ntot, i);
-            if (k < total) {
-                int m = k - (incl - cnt);
-                const int n0 = __double2hiint(er[3 * i][9]), n1 = __double2hiint(er[3 * i + 1][9]);
-                const int e = (m >= n0 + n1) ? 2 : (m >= n0 ? 1 : 0);
-                m -= (e == 2) ? n0 + n1 : (e == 1 ? n0 : 0);
-                const double *q = er[3 * i + e];
-                const int fl = __double2loint(q[9]);
-                const double pk = tr[i][7];
-                edge_step_mo(S, q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7], q[8], (fl & 2) ? -1.0 : 1.0, (fl & 1) != 0, fl >> 2,
-                             __double2hiint(q[9]), m, tr[i][6], __double2loint(pk), __double2hiint(pk));
+                for (int k = 0; k < 6; ++k) { const int mid = (lo + hi) >> 1; const bool up = pre[mid] <= r; lo = up ? mid + 1 : lo; hi = up ? hi : mid; }
+                const int ed = min(lo, 3 * WB - 1), ti = ed / 3;
+                const double *q = er[ed];
+                const int m0 = (r - (ed ? pre[ed - 1] : 0)) * RUN, m1 = min(m0 + RUN, edge_record_steps(q));
+                const double pk = tr[ti][7];
+                edge_run(S, q, m0, m1, tr[ti][6], __double2loint(pk), __double2hiint(pk));
+                steps += m1 - m0;
             }
         }
         __syncwarp();
-        n_pieces += (unsigned long long)total;
+        n_pieces += (unsigned long long)steps;
         b = __shfl_sync(full, bnext, 0);
     }
+    for (int o = 16; o; o >>= 1) n_pieces += __shfl_xor_sync(full, n_pieces, o);
     if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&S.counters[C_CHUNKS], (unsigned long long)nb);   // walked, all bands
 }
 
-// The giant triangles walk_kernel set aside: one warp per chunk of GIANT_CHUNK steps.
-__global__ void __launch_bounds__(256) walk_giant_kernel(const __grid_constant__ ShootDev S) {
-    __shared__ double scratch_s[8][48];
-    double *scratch = scratch_s[threadIdx.x >> 5];
+// The giant triangles walk_kernel set aside: a warp takes 32 chunks at a time -- lane = chunk for the set-up (its
+// triangle's frame and the one edge the chunk belongs to), then the 32 lanes walk GIANT_RUN consecutive steps each of
+// one chunk after the other.  Every chunk sets the same edge up from the same vertices, so the chunks' end points
+// agree bit for bit.
+static const int GIANT_WARPS = 8;
+__global__ void __launch_bounds__(GIANT_WARPS * 32, 3) walk_giant_kernel(const __grid_constant__ ShootDev S) {
+    __shared__ double rec_s[GIANT_WARPS][32][EREC + 2];  // edge record, cs, (bx, by)
+    double (*rec)[EREC + 2] = rec_s[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     long long n = (long long)S.counters[C_GIANT];
     if (n > S.giant_cap) n = S.giant_cap;
     if (blockIdx.x == 0 && threadIdx.x == 0 && n) atomicAdd(&S.counters[C_ROWS], (unsigned long long)n);    // chunks, all bands
+    Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
     unsigned long long n_pieces = 0;
     while (true) {
-        long long i = 0;
-        if (lane == 0) i = (long long)atomicAdd(&S.counters[C_GWALK], 1ull);
-        i = __shfl_sync(full, i, 0);
-        if (i >= n) break;
-        const unsigned long long ent = S.giant[i];
-        if (ent == ~0ull) continue;                                 // a slot whose triangle stayed with walk_kernel
-        const int c = (int)(ent & 0xfffffull);
-        const double *e = S.queue + (size_t)S.biglist[ent >> 20] * QENT;
-        double v[QENT];
+        long long i0 = 0;
+        if (lane == 0) i0 = 32ll * (long long)atomicAdd(&S.counters[C_GWALK], 1ull);
+        i0 = __shfl_sync(full, i0, 0);
+        if (i0 >= n) break;
+        // ---- lane = chunk: frame of its triangle, record of its edge
+        int c = -1;
+        if (i0 + lane < n) {
+            const unsigned long long ent = S.giant[i0 + lane];
+            if (ent != ~0ull) {                                     // (a slot whose triangle stayed with walk_kernel keeps the sentinel)
+                const int e = (int)((ent >> 18) & 3ull);
+                const double *p = S.queue + (size_t)S.biglist[ent >> 20] * QENT;
+                double v[QENT];
 #pragma unroll
-        for (int k = 0; k < QENT; ++k) v[k] = __ldg(&e[k]);
-        n_pieces += walk_triangle(S, v, scratch, c * GIANT_CHUNK, (c + 1) * GIANT_CHUNK);
+                for (int k = 0; k < QENT; ++k) v[k] = __ldg(&p[k]);
+                TriSetup T;
+                tri_setup(S, W, v, T);
+                if (T.status == 1) {
+                    const double xa = (e == 0) ? T.x[0] : (e == 1) ? T.x[1] : T.x[2], ya = (e == 0) ? T.y[0] : (e == 1) ? T.y[1] : T.y[2];
+                    const double xb = (e == 0) ? T.x[1] : (e == 1) ? T.x[2] : T.x[0], yb = (e == 0) ? T.y[1] : (e == 1) ? T.y[2] : T.y[0];
+                    EdgeWalk E;
+                    edge_setup(E, xa, ya, xb, yb, T.ry0, T.ry1, T.cx1);
+                    edge_record(E, rec[lane]);
+                    rec[lane][EREC] = T.cs; rec[lane][EREC + 1] = __hiloint2double(T.by, T.bx);
+                    c = (int)(ent & 0x3ffffull);
+                }
+            }
+        }
+        __syncwarp();
+        // ---- lane = run of GIANT_RUN consecutive steps of chunk j
+        int steps = 0;
+#pragma unroll 1
+        for (int j = 0; j < 32; ++j) {
+            const int cj = __shfl_sync(full, c, j);
+            if (cj < 0) continue;                                   // warp-uniform
+            const double *q = rec[j];
+            const int nst = edge_record_steps(q);
+            const int m0 = cj * GIANT_CHUNK + lane * GIANT_RUN, m1 = min(m0 + GIANT_RUN, nst);
+            if (m0 < m1) {
+                const double pk = q[EREC + 1];
+                edge_run(S, q, m0, m1, q[EREC], __double2loint(pk), __double2hiint(pk));
+                steps += m1 - m0;
+            }
+        }
+        __syncwarp();
+        n_pieces += (unsigned long long)steps;
     }
+    for (int o = 16; o; o >>= 1) n_pieces += __shfl_xor_sync(full, n_pieces, o);
     if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
 }
 
@@ -868,9 +914,9 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             }
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
             ML_TRY(mark());
-            ML_LAUNCH(walk_kernel, nsm * 4, WALK_WARPS * 32, 0, s, S);
+            ML_LAUNCH(walk_kernel, nsm * 3, WALK_WARPS * 32, 0, s, S);
             ML_TRY(mark());
-            ML_LAUNCH(walk_giant_kernel, nsm * 8, 256, 0, s, S);
+            ML_LAUNCH(walk_giant_kernel, nsm * 3, GIANT_WARPS * 32, 0, s, S);
             ML_TRY(mark());
             launches += 4;
         } else {
