@@ -8,5 +8,5 @@ CPU oracle and the CUDA library.
 """
 from .configs import CONFIGS, LensConfig, get_config, salpeter_moments  # noqa: F401
 from .stars import (  # noqa: F401
-    disc_stars, rect_stars, sample_points_window, sample_points_near_stars,
+    clustered_stars, disc_stars, rect_stars, sample_points_window, sample_points_near_stars,
 )

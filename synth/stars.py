@@ -22,6 +22,27 @@ def disc_stars(n: int, R: float, seed: int, cfg: LensConfig | None = None):
     return r * np.cos(phi), r * np.sin(phi), _masses(rng, n, cfg)
 
 
+def clustered_stars(n: int, R: float, seed: int, n_clumps: int = 6, clump_frac: float = 0.3, sigma: float = 3e-4,
+                    cfg: LensConfig | None = None, r_clumps: float = 0.25):
+    """Clustered star field ("spatial distributions including clustered or uniform random"): (1 - clump_frac) n
+    stars uniform in the disc |z| <= R, the rest in n_clumps tight Gaussian clumps of width sigma R whose centres lie
+    uniformly within r_clumps R of the origin.  The clumps force the quadtree many levels deeper than a uniform field
+    of the same size (cell size ~ sigma R / sqrt(stars per clump / 32))."""
+    rng = np.random.default_rng(seed)
+    n_c = int(round(clump_frac * n / n_clumps)) * n_clumps
+    n_u = n - n_c
+    r = R * np.sqrt(rng.random(n_u))
+    phi = 2.0 * np.pi * rng.random(n_u)
+    x, y = r * np.cos(phi), r * np.sin(phi)
+    rc = r_clumps * R * np.sqrt(rng.random(n_clumps))
+    pc = 2.0 * np.pi * rng.random(n_clumps)
+    cx = np.repeat(rc * np.cos(pc), n_c // n_clumps)
+    cy = np.repeat(rc * np.sin(pc), n_c // n_clumps)
+    x = np.concatenate([x, cx + sigma * R * rng.standard_normal(n_c)])
+    y = np.concatenate([y, cy + sigma * R * rng.standard_normal(n_c)])
+    return x, y, _masses(rng, n, cfg)
+
+
 def rect_stars(n: int, c1: float, c2: float, seed: int, cfg: LensConfig | None = None):
     """n stars uniform in the rectangle |x1| <= c1, |x2| <= c2."""
     rng = np.random.default_rng(seed)
