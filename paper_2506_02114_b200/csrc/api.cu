@@ -269,7 +269,7 @@ int mlens_field_destroy(mlens_field *f) {
     f->sqx.release(s); f->sqy.release(s); f->acc.release(s); f->diff.release(s);
     f->binom.p = nullptr; f->tab.p = nullptr;                     // borrowed from the per-device tables (fmm.cu)
     scratch_park(f, s);
-    f->queue.release(s); f->qcount.release(s); f->biglist.release(s); f->giant.release(s); f->counters.release(s);
+    f->queue.release(s); f->qcount.release(s); f->biglist.release(s); f->giant.release(s); f->giant_sorted.release(s); f->giant_key.release(s); f->giant_hist.release(s); f->counters.release(s);
     f->tree.release(s);
     if (cur != f->device) cudaSetDevice(cur);
     delete f;

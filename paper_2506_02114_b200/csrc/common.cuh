@@ -129,6 +129,9 @@ struct mlens_field {
     ml::DevBuf<int> qcount;              // entries per queue chunk
     ml::DevBuf<unsigned int> biglist;    // queue entries to be walked edge by edge
     ml::DevBuf<unsigned long long> giant; // chunks of the giant triangles among them
+    ml::DevBuf<unsigned long long> giant_sorted;
+    ml::DevBuf<unsigned char> giant_key;
+    ml::DevBuf<unsigned int> giant_hist;
     ml::DevBuf<unsigned long long> counters;
     int device = 0;
     cudaStream_t last_stream = nullptr;   // stream of the most recent call on this field: destroy frees in its order

@@ -364,9 +364,11 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
         // ---- lane = triangle: local frame
         const long long it = b * WB + lane;
         int status = 0;
+        unsigned int qidx = 0;
         double ry0 = 0.0, ry1 = 0.0, cx1 = 0.0;
         if (lane < WB && it < nb) {
-            const double *e = S.queue + (size_t)S.biglist[it] * QENT;
+            qidx = S.biglist[it];
+            const double *e = S.queue + (size_t)qidx * QENT;
             double v[QENT];
 #pragma unroll
             for (int k = 0; k < QENT; ++k) v[k] = __ldg(&e[k]);
@@ -409,9 +411,21 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
             for (int e = 0; e < 3; ++e) nch += (edge_record_steps(er[3 * lane + e]) + GIANT_CHUNK - 1) / GIANT_CHUNK;
             unsigned long long at = atomicAdd(&S.counters[C_GIANT], (unsigned long long)nch);
             if ((long long)(at + nch) <= S.giant_cap) {           // (else it stays here; the skipped slots keep their sentinel)
+                const int by_t = __double2hiint(tr[lane][7]);
                 for (int e = 0; e < 3; ++e) {
-                    const int ne = (edge_record_steps(er[3 * lane + e]) + GIANT_CHUNK - 1) / GIANT_CHUNK;
-                    for (int c = 0; c < ne; ++c) S.giant[at++] = ((unsigned long long)it << 20) | ((unsigned long long)e << 18) | (unsigned long long)c;
+                    const double *q = er[3 * lane + e];
+                    const int nst = edge_record_steps(q);
+                    const int ne = (nst + GIANT_CHUNK - 1) / GIANT_CHUNK;
+                    const int fl = __double2loint(q[9]);
+                    for (int c = 0; c < ne; ++c) {
+                        // the block of map rows around the middle step of the chunk (ordering key only)
+                        const int m = min(c * GIANT_CHUNK + GIANT_CHUNK / 2, nst - 1);
+                        const double ms = q[8] + ((fl & 2) ? -1.0 : 1.0) * (double)(m - 1);
+                        const double y = (fl & 1) ? ms : fma(dmin(dmax((ms - q[0]) * q[4], q[6]), q[7]), q[3] - q[1], q[1]);
+                        const int row = min(max(__double2int_rd(y) + by_t, 0), S.npix2 - 1);
+                        S.giant_key[at] = (unsigned char)min(row >> GIANT_BIN_SHIFT, GIANT_BINS - 2);
+                        S.giant[at++] = ((unsigned long long)qidx << 20) | ((unsigned long long)e << 18) | (unsigned long long)c;
+                    }
                 }
                 ntot = -1;                                          // gone
             }
@@ -454,69 +468,77 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&S.counters[C_CHUNKS], (unsigned long long)nb);   // walked, all bands
 }
 
-// The giant triangles walk_kernel set aside: a warp takes 32 chunks at a time -- lane = chunk for the set-up (its
-// triangle's frame and the one edge the chunk belongs to), then the 32 lanes walk GIANT_RUN consecutive steps each of
-// one chunk after the other.  Every chunk sets the same edge up from the same vertices, so the chunks' end points
-// agree bit for bit.
-static const int GIANT_WARPS = 8;
-__global__ void __launch_bounds__(GIANT_WARPS * 32, 3) walk_giant_kernel(const __grid_constant__ ShootDev S) {
-    __shared__ double rec_s[GIANT_WARPS][32][EREC + 2];  // edge record, cs, (bx, by)
-    double (*rec)[EREC + 2] = rec_s[threadIdx.x >> 5];
-    const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31;
+// The giant triangles walk_kernel set aside, chunk by chunk.  A giant's edges cross the whole map, so its deposits
+// touch `diff` rows 80 KB apart: the chunks are first ORDERED by the block of 256 map rows they fall into (counting
+// sort: giant_hist_kernel, giant_scatter_kernel), and the warps of walk_giant_kernel take consecutive chunks of that
+// order -- at any moment all of them deposit into one or two row blocks (20 MB each), which L2 holds, instead of
+// into the whole 1.6 GB of a 10^4 x 10^4 map.
+__global__ void __launch_bounds__(256) giant_hist_kernel(const __grid_constant__ ShootDev S) {
+    __shared__ unsigned int h[GIANT_BINS];
+    for (int k = threadIdx.x; k < GIANT_BINS; k += blockDim.x) h[k] = 0u;
+    __syncthreads();
     long long n = (long long)S.counters[C_GIANT];
     if (n > S.giant_cap) n = S.giant_cap;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned char key = S.giant_key[i];
+        if (key < GIANT_BINS - 1) atomicAdd(&h[key], 1u);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < GIANT_BINS; k += blockDim.x) if (h[k]) atomicAdd(&S.giant_hist[k], h[k]);
+}
+__global__ void __launch_bounds__(256) giant_scatter_kernel(const __grid_constant__ ShootDev S) {
+    __shared__ unsigned int base[GIANT_BINS];
+    if (threadIdx.x == 0) {
+        unsigned int run = 0;
+        for (int k = 0; k < GIANT_BINS; ++k) { base[k] = run; run += S.giant_hist[k]; }
+        if (blockIdx.x == 0) S.counters[C_GWALK] = run;            // sorted entries (the sentinels are left out)
+    }
+    __syncthreads();
+    long long n = (long long)S.counters[C_GIANT];
+    if (n > S.giant_cap) n = S.giant_cap;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned char key = S.giant_key[i];
+        if (key < GIANT_BINS - 1) S.giant_sorted[base[key] + atomicAdd(&S.giant_hist[GIANT_BINS + key], 1u)] = S.giant[i];
+    }
+}
+
+// One warp per chunk, chunks in sorted order with a grid stride (they cost the same): every lane sets the chunk's
+// triangle and edge up for itself from the same vertices (so the chunks' end points agree bit for bit, and no shared
+// memory is needed), then walks GIANT_RUN consecutive steps of the chunk.
+static const int GIANT_WARPS = 8;
+__global__ void __launch_bounds__(GIANT_WARPS * 32, 3) walk_giant_kernel(const __grid_constant__ ShootDev S) {
+    const int lane = threadIdx.x & 31;
+    const long long n = (long long)S.counters[C_GWALK];
     if (blockIdx.x == 0 && threadIdx.x == 0 && n) atomicAdd(&S.counters[C_ROWS], (unsigned long long)n);    // chunks, all bands
     Win W; W.w32 = nullptr; W.ax = 0; W.ay = 0;
     unsigned long long n_pieces = 0;
-    while (true) {
-        long long i0 = 0;
-        if (lane == 0) i0 = 32ll * (long long)atomicAdd(&S.counters[C_GWALK], 1ull);
-        i0 = __shfl_sync(full, i0, 0);
-        if (i0 >= n) break;
-        // ---- lane = chunk: frame of its triangle, record of its edge
-        int c = -1;
-        if (i0 + lane < n) {
-            const unsigned long long ent = S.giant[i0 + lane];
-            if (ent != ~0ull) {                                     // (a slot whose triangle stayed with walk_kernel keeps the sentinel)
-                const int e = (int)((ent >> 18) & 3ull);
-                const double *p = S.queue + (size_t)S.biglist[ent >> 20] * QENT;
-                double v[QENT];
+    const long long stride = (long long)gridDim.x * GIANT_WARPS;
+    long long i = (long long)blockIdx.x * GIANT_WARPS + (threadIdx.x >> 5);
+    unsigned long long ent_next = (i < n) ? S.giant_sorted[i] : 0ull;
+    for (; i < n; i += stride) {
+        const unsigned long long ent = ent_next;                    // (queue entry << 20 | edge << 18 | chunk)
+        if (i + stride < n) ent_next = S.giant_sorted[i + stride];  // on its way while this chunk is walked
+        const int e = (int)((ent >> 18) & 3ull), c = (int)(ent & 0x3ffffull);
+        const double *p = S.queue + (size_t)(ent >> 20) * QENT;
+        double v[QENT];
 #pragma unroll
-                for (int k = 0; k < QENT; ++k) v[k] = __ldg(&p[k]);
-                TriSetup T;
-                tri_setup(S, W, v, T);
-                if (T.status == 1) {
-                    const double xa = (e == 0) ? T.x[0] : (e == 1) ? T.x[1] : T.x[2], ya = (e == 0) ? T.y[0] : (e == 1) ? T.y[1] : T.y[2];
-                    const double xb = (e == 0) ? T.x[1] : (e == 1) ? T.x[2] : T.x[0], yb = (e == 0) ? T.y[1] : (e == 1) ? T.y[2] : T.y[0];
-                    EdgeWalk E;
-                    edge_setup(E, xa, ya, xb, yb, T.ry0, T.ry1, T.cx1);
-                    edge_record(E, rec[lane]);
-                    rec[lane][EREC] = T.cs; rec[lane][EREC + 1] = __hiloint2double(T.by, T.bx);
-                    c = (int)(ent & 0x3ffffull);
-                }
-            }
+        for (int k = 0; k < QENT; ++k) v[k] = __ldg(&p[k]);
+        TriSetup T;
+        tri_setup(S, W, v, T);
+        if (T.status != 1) continue;                                // (cannot happen: walk_kernel found steps to walk)
+        const double xa = (e == 0) ? T.x[0] : (e == 1) ? T.x[1] : T.x[2], ya = (e == 0) ? T.y[0] : (e == 1) ? T.y[1] : T.y[2];
+        const double xb = (e == 0) ? T.x[1] : (e == 1) ? T.x[2] : T.x[0], yb = (e == 0) ? T.y[1] : (e == 1) ? T.y[2] : T.y[0];
+        EdgeWalk E;
+        edge_setup(E, xa, ya, xb, yb, T.ry0, T.ry1, T.cx1);
+        double q[EREC];
+        edge_record(E, q);
+        const int m0 = c * GIANT_CHUNK + lane * GIANT_RUN, m1 = min(m0 + GIANT_RUN, E.n);
+        if (m0 < m1) {
+            edge_run(S, q, m0, m1, T.cs, T.bx, T.by);
+            n_pieces += (unsigned long long)(m1 - m0);
         }
-        __syncwarp();
-        // ---- lane = run of GIANT_RUN consecutive steps of chunk j
-        int steps = 0;
-#pragma unroll 1
-        for (int j = 0; j < 32; ++j) {
-            const int cj = __shfl_sync(full, c, j);
-            if (cj < 0) continue;                                   // warp-uniform
-            const double *q = rec[j];
-            const int nst = edge_record_steps(q);
-            const int m0 = cj * GIANT_CHUNK + lane * GIANT_RUN, m1 = min(m0 + GIANT_RUN, nst);
-            if (m0 < m1) {
-                const double pk = q[EREC + 1];
-                edge_run(S, q, m0, m1, q[EREC], __double2loint(pk), __double2hiint(pk));
-                steps += m1 - m0;
-            }
-        }
-        __syncwarp();
-        n_pieces += (unsigned long long)steps;
     }
-    for (int o = 16; o; o >>= 1) n_pieces += __shfl_xor_sync(full, n_pieces, o);
+    for (int o = 16; o; o >>= 1) n_pieces += __shfl_xor_sync(0xffffffffu, n_pieces, o);
     if (lane == 0 && n_pieces) atomicAdd(&S.counters[C_PX_EDGE], n_pieces);
 }
 
@@ -783,6 +805,9 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             if (rc == MLENS_OK) rc = f->qcount.reserve((size_t)qcap, s, false);
             if (rc == MLENS_OK) rc = f->biglist.reserve((size_t)qcap * QCHUNK / 4, s, false);
             if (rc == MLENS_OK) rc = f->giant.reserve((size_t)GIANT_CAP, s, false);
+            if (rc == MLENS_OK) rc = f->giant_sorted.reserve((size_t)GIANT_CAP, s, false);
+            if (rc == MLENS_OK) rc = f->giant_key.reserve((size_t)GIANT_CAP, s, false);
+            if (rc == MLENS_OK) rc = f->giant_hist.reserve((size_t)2 * GIANT_BINS, s, false);
             if (rc == MLENS_OK) break;
             if (rc != MLENS_ENOMEM || qmb_env > 0 || qmb <= 256) return rc;
             cudaGetLastError();
@@ -796,7 +821,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     S.colmajor = d->tile_traversal == 1 ? 0 : 1;
     S.ylo1 = g->ylo1; S.ylo2 = g->ylo2; S.p1 = g->p1; S.p2 = g->p2; S.inv_p1 = 1.0 / g->p1; S.inv_p2 = 1.0 / g->p2;
     S.npix1 = d->npix1; S.npix2 = d->npix2;
-    S.acc = f->acc.p; S.diff = f->diff.p; S.queue = f->queue.p; S.qcount = f->qcount.p; S.biglist = f->biglist.p; S.big_cap = qcap * QCHUNK / 4; S.giant = f->giant.p; S.giant_cap = ipm ? GIANT_CAP : 0; S.counters = f->counters.p; S.queue_cap = qcap;
+    S.acc = f->acc.p; S.diff = f->diff.p; S.queue = f->queue.p; S.qcount = f->qcount.p; S.biglist = f->biglist.p; S.big_cap = qcap * QCHUNK / 4; S.giant = f->giant.p; S.giant_cap = ipm ? GIANT_CAP : 0; S.giant_sorted = f->giant_sorted.p; S.giant_key = f->giant_key.p; S.giant_hist = f->giant_hist.p; S.counters = f->counters.p; S.queue_cap = qcap;
     S.dump1 = d->dump_w1; S.dump2 = d->dump_w2;
     S.binom = f->binom.p;
     if ((S.dump1 == nullptr) != (S.dump2 == nullptr)) { set_error("dump_w1 and dump_w2 go together"); return MLENS_EINVAL; }
@@ -896,7 +921,10 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         int grid = (int)((want < resident) ? want : resident);
         ML_CUDA(cudaMemsetAsync(f->counters.p, 0, 16, s));         // queue fill count and tile counter
         ML_CUDA(cudaMemsetAsync(f->counters.p + C_DRAIN, 0, 5 * 8, s));   // drain, big-list, walk and giant counters
-        if (ipm) ML_CUDA(cudaMemsetAsync(f->giant.p, 0xff, (size_t)GIANT_CAP * 8, s));   // sentinels
+        if (ipm) {
+            ML_CUDA(cudaMemsetAsync(f->giant_key.p, 0xff, (size_t)GIANT_CAP, s));        // sentinels: slots reserved but not filled
+            ML_CUDA(cudaMemsetAsync(f->giant_hist.p, 0, (size_t)2 * GIANT_BINS * 4, s));
+        }
         ML_TRY(mark());
         if (ipm) {
             if (f32) ML_LAUNCH(shoot_ipm_kernel<true>, grid, SHOOT_WARPS * 32, smem_ipm, s, S);
@@ -916,9 +944,11 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             ML_TRY(mark());
             ML_LAUNCH(walk_kernel, nsm * 3, WALK_WARPS * 32, 0, s, S);
             ML_TRY(mark());
+            ML_LAUNCH(giant_hist_kernel, nsm, 256, 0, s, S);
+            ML_LAUNCH(giant_scatter_kernel, nsm, 256, 0, s, S);
             ML_LAUNCH(walk_giant_kernel, nsm * 3, GIANT_WARPS * 32, 0, s, S);
             ML_TRY(mark());
-            launches += 4;
+            launches += 6;
         } else {
             if (f32) ML_LAUNCH(shoot_irs_kernel<true>, grid, SHOOT_WARPS * 32, smem_irs, s, S);
             else ML_LAUNCH(shoot_irs_kernel<false>, grid, SHOOT_WARPS * 32, smem_irs, s, S);

@@ -22,6 +22,8 @@ static const int NSLOT = 2;           // leaves a tile keeps a series for (rays 
 static const int WX = 32, WY = 8;     // per-warp shared-memory pixel window
 static const int FOLDJ = WX * WY * 8 / (32 * 16);   // series terms per pass of the star folding (scratch = the window)
 static const int BN = 2 * ML_P1MAX;   // stride of the Pascal triangle
+static const int GIANT_BINS = 128;    // blocks of map rows the giant triangles' chunks are ordered by
+static const int GIANT_BIN_SHIFT = 8; // 256 rows per block (a block of `diff` rows stays in L2 while its chunks are walked)
 
 // slots of ShootDev::counters
 enum { C_QUEUE = 0, C_TILE, C_SINGLE, C_SMALL, C_QUEUED, C_CHUNKS, C_OVERFLOW, C_FALLBACK, C_RAYS, C_NEAR,
@@ -43,8 +45,11 @@ struct ShootDev {
     int *qcount;                       // entries in each chunk
     unsigned int *biglist;             // queue entries whose triangles are walked edge by edge (walk_kernel)
     long long big_cap;
-    unsigned long long *giant;         // (walk-list index << 20 | chunk) of the triangles with too many steps for one warp
+    unsigned long long *giant;         // (queue entry << 20 | edge << 18 | chunk) of the triangles with too many steps for one warp
     long long giant_cap;
+    unsigned long long *giant_sorted;  // the same entries ordered by the block of map rows their steps fall into
+    unsigned char *giant_key;          // that block, per entry (255: none)
+    unsigned int *giant_hist;          // [0, GIANT_BINS): entries per block; [GIANT_BINS, 2 GIANT_BINS): scatter cursors
     unsigned long long *counters;
     long long queue_cap;               // chunks
     double *dump1, *dump2;
