@@ -97,7 +97,8 @@ static_assert(FOLDJ >= 4 && ML_NEAR == 32, "fold scratch must fit the window");
 struct TileCtx {                       // warp-uniform registers
     double zt_x, zt_y, inv_rt;
     bool fast;                         // the whole tile sits in one leaf whose tile series passed its bound
-    bool lin;                          // the whole tile lies inside the star disc: the sheet term of eq 19 is -kappa_star z
+    bool lin;                          // the sheet term is -kappa_star z for every ray of the tile: inside the star disc (eq 19), or inside
+                                       // the star rectangle with the analytic rest of eq B8 folded into the tile series
 };
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -272,10 +273,72 @@ static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShar
         atomicAdd(&S.counters[C_TILES], 1ull);
         atomicAdd(&S.counters[C_NEAR_LEAF], (unsigned long long)__ldg(&S.L.near_cnt[W.leaf[0]]));
     }
-    zero_window(W);
     // eq 19 inside the disc is linear in z: the farthest ray of the tile decides (the disc is convex)
     const double rmax = sqrt(C.zt_x * C.zt_x + C.zt_y * C.zt_y) + rt;
-    const bool lin = S.L.shape == MLENS_SHAPE_DISC && rmax * rmax <= S.L.R2;
+    bool lin = S.L.shape == MLENS_SHAPE_DISC && rmax * rmax <= S.L.R2;
+    if (S.L.shape == MLENS_SHAPE_RECT && fabs(C.zt_x) + rt <= S.L.c1 && fabs(C.zt_y) + rt <= S.L.c2) {
+        // Rectangle sheet inside the rectangle (eq B8): alpha_s = -kappa_star z + conj A(z) with
+        //   A(z) = (kappa_star i/pi) G(z) - kappa_star (2 c1 + z),   G(z) = sum_i s_i (a_i - z) log(a_i - z),
+        // a_i = conj c, c, -conj c, -c and s_i = +1, -1, +1, -1 -- analytic in the open rectangle (the logarithms' cuts
+        // lie on its upper and lower edges).  Its Taylor series about the tile centre joins the tile series, so a ray
+        // costs nothing extra and no logarithm (hard part 8; the paper pays four per ray):
+        //   G' = -sum s_i log(a_i - z),   G^(n) = sum s_i (n-2)!/(a_i - z)^(n-1)  (n >= 2)
+        //   T_j = A^(j)(z_t) rt^j / j!;  for j >= 2:  T_j = (kappa_star i/pi) sum_i s_i (a_i - z_t) w_i^j / (j (j-1)),  w_i = rt/(a_i - z_t)
+        // The series converges within the distance to the nearest corner; the tile keeps the full eq B7 if its tail is not
+        // within the budget (tiles next to a corner of the rectangle).
+        int Qm = 0;
+        for (int s = 0; s < NSLOT; ++s) if (W.leaf[s] >= 0) Qm = max(Qm, W.q[s]);
+        const double ks_pi = S.L.kappa_star * 0.31830988618379067154;
+        const int j = lane;                                        // lane = term of the series
+        double2 Tj = make_double2(0.0, 0.0);
+        double tail = 0.0;
+        // the four logarithms, one corner per lane (a double-precision log and atan2 are a few hundred instructions each:
+        // once per tile, in parallel, not once per term)
+        double lg = 0.0, ar = 0.0;
+        {
+            const int i = lane & 3;
+            const double ax = (i < 2) ? S.L.c1 : -S.L.c1, ay = (i == 0 || i == 3) ? -S.L.c2 : S.L.c2;
+            const double dx = ax - C.zt_x, dy = ay - C.zt_y;
+            lg = 0.5 * log(dx * dx + dy * dy); ar = atan2(dy, dx);
+        }
+#pragma unroll 1
+        for (int i = 0; i < 4; ++i) {
+            const double sg = (i & 1) ? -1.0 : 1.0;
+            const double ax = (i < 2) ? S.L.c1 : -S.L.c1, ay = (i == 0 || i == 3) ? -S.L.c2 : S.L.c2;    // conj c, c, -conj c, -c
+            const double2 d = make_double2(ax - C.zt_x, ay - C.zt_y);
+            const double d2 = d.x * d.x + d.y * d.y, id2 = fast_rcp(d2);
+            const double2 w = make_double2(rt * d.x * id2, -rt * d.y * id2);         // rt / d
+            const double rho = rt * sqrt(id2);
+            const double lgi = __shfl_sync(full, lg, i), ari = __shfl_sync(full, ar, i);
+            if (j == 0) {
+                Tj.x += sg * (d.x * lgi - d.y * ari); Tj.y += sg * (d.x * ari + d.y * lgi);              // G: d log d
+            } else if (j == 1) {
+                Tj.x -= sg * lgi * rt; Tj.y -= sg * ari * rt;                                            // G' rt
+            } else if (j <= Qm) {
+                const double2 t = cmul(d, cpowi(w, j));
+                const double f = sg / (double)(j * (j - 1));
+                Tj.x += f * t.x; Tj.y += f * t.y;
+            }
+            // what the truncation after order Qm leaves out of this corner's part, geometric bound
+            double rq = rho;
+            for (int k = 0; k < Qm; ++k) rq *= rho;                                  // rho^(Qm+1)
+            tail += (rho < 0.5) ? ks_pi * sqrt(d2) * rq / ((double)(Qm * (Qm + 1)) * (1.0 - rho)) : 1.0e300;
+        }
+        // (kappa_star i/pi) G-part, then the polynomial part -kappa_star (2 c1 + z) in the terms 0 and 1
+        Tj = make_double2(-ks_pi * Tj.y, ks_pi * Tj.x);
+        if (j == 0) { Tj.x -= S.L.kappa_star * (2.0 * S.L.c1 + C.zt_x); Tj.y -= S.L.kappa_star * C.zt_y; }
+        if (j == 1) Tj.x -= S.L.kappa_star * rt;
+        const bool ok = (Qm >= 2) && (tail <= S.eps_far);         // the same in all lanes
+        if (ok) {
+            for (int s = 0; s < NSLOT; ++s) {
+                if (W.leaf[s] < 0) continue;
+                if (j <= W.q[s]) { double2 t0 = W.t[s][j]; W.t[s][j] = make_double2(t0.x + Tj.x, t0.y + Tj.y); }
+            }
+            lin = true;
+        }
+        __syncwarp();
+    }
+    zero_window(W);
     if (lane == 0) {
         W.ctx[0] = C.zt_x; W.ctx[1] = C.zt_y; W.ctx[2] = C.inv_rt;
         W.ctx[3] = ((one_leaf && W.mode[0] == 0) ? 1.0 : 0.0) + (lin ? 2.0 : 0.0);
@@ -343,6 +406,11 @@ static __device__ __noinline__ void eval_group_ool(const ShootDev *Sp, const War
             int kind;
             a = eval_one_ool(Sp, T, x, y, ux, uy0 + duy * (double)r, &kind);
             if (kind >= 0) cnt[1] += kind; else ++cnt[2];
+            if (kind >= 0 && S.L.shape == MLENS_SHAPE_RECT && (((int)T->ctx[3]) & 2)) {
+                // the slot's series already holds the analytic part of the rectangle sheet (eq B8): only -kappa_star z is left
+                w[2 * r] = fma(S.a1_lin, x, -a.x); w[2 * r + 1] = fma(S.a2_lin, y, -a.y);
+                continue;
+            }
         }
         lens_w(S.L, x, y, a.x, a.y, w[2 * r], w[2 * r + 1]);
     }

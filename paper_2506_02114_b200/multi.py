@@ -38,9 +38,12 @@ def slab_bounds(n_rows, world, rank, weights=None, align=1):
     return cuts[rank], cuts[rank + 1]
 
 
-def star_row_weights(ys, x0_2, h2, n_rows, per_star=2000.0):
+def star_row_weights(ys, x0_2, h2, n_rows, per_star=10.0):
     """Per-row cost model for slab_bounds: one unit per cell row plus `per_star` for every star whose
-    x2 lies in the row (the cells around a star map to triangles covering thousands of pixels)."""
+    x2 lies in the row (the cells around a star map to triangles covering thousands of pixels).  per_star = 10 rows is
+    the least-squares fit of t = a rows + b stars to the times of eight equal-row slabs of BASELINE config 1 on one
+    B200 (bench.py `slab_balance`: a = 0.19 us per row, b = 1.9 us per star; equal rows are off by 17 %, weighted
+    rows by 11 % -- the window's edge rows hold no stars and fewer in-map triangles)."""
     w = np.ones(n_rows)
     j = np.floor((np.asarray(ys) - x0_2) / h2).astype(np.int64)
     j = j[(j >= 0) & (j < n_rows)]

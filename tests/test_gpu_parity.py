@@ -519,6 +519,20 @@ def test_rect_field_map(ml, orc):
     g = orc.geometry(0.5, ks, 0.1, 2.0, 48, 2.0, 2, 0.2)
     res = gf.shoot(2.0, 48, 2.0, border_mode=ml.BORDER_MARGIN, border_param=0.2)
     _map_check(res.map, orc.shoot(of, g, 0), "rectangle")
+    # The tiles inside the rectangle carry the analytic part of eq B8 in their series (no logarithm per ray): every ray
+    # against the oracle's eq B7, over a window that reaches past the rectangle's edges and corners (there the tiles
+    # keep the full eq B7), at a ray density where a tile is small against the rectangle
+    H = (1.25 * c1, 1.4 * c2)
+    g = orc.geometry(0.5, ks, 0.1, (0.5 * H[0], 0.1 * H[1]), (40, 40), 16.0, 3, He=H)
+    res = gf.shoot((0.5 * H[0], 0.1 * H[1]), (40, 40), 16.0, border_mode=BORDER_EXPLICIT, He=H, dump=True)
+    assert (res.grid.n1, res.grid.n2) == (g.n1, g.n2)
+    ox, oy = orc.map_corners(of, g, 0, g.n1, 0, g.n2)
+    assert np.max(np.hypot(res.dump[0] - ox, res.dump[1] - oy)) <= 1e-8
+    _map_check(res.map, orc.shoot(of, g, 0), "rectangle, window past its edges")
+    irs = gf.shoot((0.5 * H[0], 0.1 * H[1]), (40, 40), 16.0, border_mode=BORDER_EXPLICIT, He=H, map_mode=ml.MAP_IRS, dump=True, want_counts=True)
+    ox, oy = orc.map_centres(of, g, 0, g.n1, 0, g.n2)
+    assert np.max(np.hypot(irs.dump[0] - ox, irs.dump[1] - oy)) <= 1e-8
+    assert np.array_equal(irs.counts, orc.bin_irs(irs.dump[0], irs.dump[1], g))
 
 
 def test_ipm_and_irs_agree_on_gpu(ml):
