@@ -873,12 +873,18 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     long long rows_per_band = band_cells / (ntx * stepx * stepy);
     if (rows_per_band < 1) rows_per_band = 1;
     if (!ipm && !d->band_fixed) rows_per_band = nty;                          // IRS has no queue to bound: one launch
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    // events of a timed call: destroyed on every way out of the function, error returns included
+    struct Events {
+        cudaEvent_t e0 = nullptr, e1 = nullptr;
+        std::vector<cudaEvent_t> list;
+        ~Events() { if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); for (cudaEvent_t e : list) cudaEventDestroy(e); }
+    } evs;
+    cudaEvent_t &e0 = evs.e0, &e1 = evs.e1;
     const bool timed = st && (d->sync || d->ptr_kind == MLENS_PTR_HOST);
     if (timed) { ML_CUDA(cudaEventCreate(&e0)); ML_CUDA(cudaEventCreate(&e1)); ML_CUDA(cudaEventRecord(e0, s)); }
     int launches = 0, bands = 0;
     // per-kernel device times: events between the back-to-back launches of each band (timed calls only)
-    std::vector<cudaEvent_t> ev;
+    std::vector<cudaEvent_t> &ev = evs.list;
     auto mark = [&]() -> int {
         if (!timed) return MLENS_OK;
         cudaEvent_t e; ML_CUDA(cudaEventCreate(&e)); ML_CUDA(cudaEventRecord(e, s)); ev.push_back(e);
@@ -984,7 +990,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         st->tile_order = S.tq;
         st->n_bands = bands; st->gpu_launches = launches; st->n_shoot_launches = bands;
         if (timed) {
-            ML_CUDA(cudaEventElapsedTime(&st->ms_total, e0, e1)); cudaEventDestroy(e0); cudaEventDestroy(e1);
+            ML_CUDA(cudaEventElapsedTime(&st->ms_total, e0, e1));
             const size_t per = ipm ? 5 : 2;              // events per band
             for (int b = 0; b < bands; ++b) {
                 float ms = 0;
@@ -1001,7 +1007,6 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     } else if (d->sync) {
         ML_CUDA(cudaStreamSynchronize(s));
     }
-    for (cudaEvent_t e : ev) cudaEventDestroy(e);
     return MLENS_OK;
 }
 

@@ -76,5 +76,8 @@ def shoot_distributed(field, half_y, npix, k, *, group=None, weights=None, shoot
     if not torch.is_tensor(part):
         part = torch.from_numpy(np.ascontiguousarray(part))
     if world > 1:
+        if dist.get_backend(group) == "nccl" and not part.is_cuda:
+            raise ValueError("shoot_distributed over NCCL needs the partial map on the GPU: pass device=torch.device('cuda', local_rank) "
+                             "or a CUDA tensor as out= (a host map can only be reduced over gloo)")
         dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)      # the one exchange step of the path
     return part, (j0, j1), stats
