@@ -120,6 +120,8 @@ struct EdgeWalk {                     // one triangle edge, clipped to the map r
     int majorY;                       // 1: walk rows (|dy| >= |dx|), 0: walk columns
     int n;                            // steps = crossings of major-axis grid lines + 1, or 0
     int cf;                           // ends cut by a border row of the map: bits 0-1 the start (1: row line ry0, 2: ry1), bits 2-3 the end
+    int bx, by;                       // integer origin of the edge's own frame (edge_setup_canon)
+    int fwd;                          // 1: the canonical direction (smaller end first) is the direction the triangle's boundary runs in
 };
 
 // local coordinates: pixel units relative to the integer point (bx, by); rows [ry0, ry1] and columns <= cx1 are the map
@@ -163,11 +165,27 @@ __device__ __forceinline__ void edge_setup(EdgeWalk &E, double x0, double y0, do
     E.n = ((nc > 0.0) ? (int)fmin(nc, 1.0e7) : 0) + 1;
 }
 
-// One piece of an edge, from (xs, ys) to (xe, ye), inside one pixel, with cover tcov = G(ye) - G(ys), G(y) = rn(cs y),
-// cs = -sign(A) ONE/|A|; (bx, by) = integer origin of the local coordinates.  The covers telescope exactly along the
-// triangle's boundary because consecutive pieces share the value of G at the point where they meet.
-__device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, double ys, double xe, double ye, long long tcov, int bx, int by) {
-    if (tcov == 0) return;
+// An edge is set up in a frame and a direction of ITS OWN -- origin = the integer lower-left of its two end points,
+// direction = smaller end first (by x, then y) -- so that the two triangles that share it compute the very same pieces,
+// bit for bit, whichever of them walks it and whether it is walked once for both or once for each.  (ux0, uy0) ->
+// (ux1, uy1): the end points in GLOBAL pixel units, in the order of the triangle's boundary.
+__device__ __forceinline__ void edge_setup_canon(const ShootDev &S, EdgeWalk &E, double ux0, double uy0, double ux1, double uy1) {
+    const bool fwd = (ux0 < ux1) || (ux0 == ux1 && uy0 <= uy1);
+    const double ax = fwd ? ux0 : ux1, ay = fwd ? uy0 : uy1, cx = fwd ? ux1 : ux0, cy = fwd ? uy1 : uy0;
+    const double fbx = floor(ax), fby = floor(dmin(ay, cy));          // ax <= cx
+    const double hgt = dmax(ay, cy) - fby + 1.0;
+    edge_setup(E, ax - fbx, ay - fby, cx - fbx, cy - fby, fmax(0.0, -fby), fmin(hgt, (double)S.npix2 - fby), (double)S.npix1 - fbx);
+    E.bx = (int)fbx; E.by = (int)fby; E.fwd = fwd ? 1 : 0;
+}
+
+// One piece of an edge, from (xs, ys) to (xe, ye), inside one pixel, with the covers ta, tb it has for the (one or two)
+// triangles on its sides: t = G(ye) - G(ys), G(y) = rn(c y), c = -+ONE/|A| of that triangle; (bx, by) = integer origin
+// of the local coordinates.  The covers telescope exactly along each triangle's boundary because consecutive pieces
+// share the value of G at the point where they meet.  The share that moves to the next column is rounded per triangle,
+// so a piece walked once for two triangles deposits exactly what two walks would.
+__device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, double ys, double xe, double ye, long long ta, long long tb, int bx, int by) {
+    const long long tcov = ta + tb;
+    if ((ta | tb) == 0) return;
     const double ym = 0.5 * (ys + ye), xm = 0.5 * (xs + xe);
     const int jr = __double2int_rd(ym) + by;                   // (coordinates are bounded by 1e9: no saturation)
     if ((unsigned)jr >= (unsigned)S.npix2) return;
@@ -179,7 +197,8 @@ __device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, doub
     int c0 = 0;
     if (ic >= 0) {
         const double m = clamp01(xm - (double)il);
-        r = __double2ll_rn((double)tcov * m);
+        r = __double2ll_rn((double)ta * m);
+        if (tb) r += __double2ll_rn((double)tb * m);
         c0 = ic + 1;
         if (tcov != r) atomicAdd(row + ic, (unsigned long long)(tcov - r));
     }
@@ -190,24 +209,39 @@ __device__ __forceinline__ void piece_deposit(const ShootDev &S, double xs, doub
 // that is walked, oc0 -> o1 along the other, id / oid the reciprocals of the two extents (0 for an extent of 0),
 // [ta, tb] the clipped parameter range, g0 the first grid line; q[9] packs the step count n (high word) with the
 // flags: bit 0 major axis is y, bit 1 walking towards smaller coordinates, bits 2-5 the border-row flags cf.
-static const int EREC = 10;
-__device__ __forceinline__ void edge_record(const EdgeWalk &E, double *q) {
+// q[10], q[11]: weight c1 of the triangle the edge was set up for (signed for the canonical direction) and the offset
+// d1 = by_edge - by_triangle that takes the edge's local y into that triangle's frame (G is taken there, so that the
+// triangle's three edges see the same numbers at the vertices they share).  q[12], q[13]: the same for a SECOND
+// triangle on the other side (walk_kernel pairs the edges two triangles of a batch share), c2 = 0 if there is none.
+// q[14]: the edge's frame origin (by, bx) packed.
+static const int EREC = 16;
+__device__ __forceinline__ void edge_record(const EdgeWalk &E, double cs_tri, int by_tri, double *q) {
     const bool my = E.majorY != 0;
     q[0] = my ? E.y0 : E.x0; q[1] = my ? E.x0 : E.y0; q[2] = my ? E.y1 : E.x1; q[3] = my ? E.x1 : E.y1;
     q[4] = my ? E.idy : E.idx; q[5] = my ? E.idx : E.idy; q[6] = E.ta; q[7] = E.tb; q[8] = E.g0;
     q[9] = __hiloint2double(E.n, E.majorY | (E.sg < 0.0 ? 2 : 0) | (E.cf << 2));
+    q[10] = E.fwd ? cs_tri : -cs_tri; q[11] = (double)(E.by - by_tri);
+    q[12] = 0.0; q[13] = 0.0;
+    q[14] = __hiloint2double(E.by, E.bx); q[15] = 0.0;
 }
 __device__ __forceinline__ int edge_record_steps(const double *q) { return __double2hiint(q[9]); }
+// the same geometric edge (set up from the same two end points): everything but the weights agrees bit for bit
+__device__ __forceinline__ bool edge_record_same(const double *a, const double *b) {
+    return a[0] == b[0] && a[1] == b[1] && a[2] == b[2] && a[3] == b[3] &&
+           __double_as_longlong(a[14]) == __double_as_longlong(b[14]);
+}
 
 // Steps [m0, m1) of an edge, 0 <= m0 < m1 <= n.  Step k runs from major-axis grid line k-1 (or the clipped start) to
 // grid line k (or the clipped end).  End points on a grid line take its exact value, an unclipped end the vertex
 // itself, an end cut by a border row of the map that row line's value: consecutive steps and consecutive edges share
 // their end points bit for bit.  A lane walks CONSECUTIVE steps: the end of a step (its coordinates and G) is carried
 // into the next one, so that every point of the edge is computed once.
-__device__ __forceinline__ void edge_run(const ShootDev &S, const double *q, int m0, int m1, double cs, int bx, int by) {
+__device__ __forceinline__ void edge_run(const ShootDev &S, const double *q, int m0, int m1) {
     const double c0 = q[0], oc0 = q[1], c1 = q[2], o1 = q[3], id = q[4], oid = q[5], ta = q[6], tb = q[7], g0 = q[8];
     const int fl = __double2loint(q[9]), n = __double2hiint(q[9]);
-    const bool my = (fl & 1) != 0;
+    const double ca = q[10], da = q[11], cb = q[12], db = q[13];
+    const int bx = __double2loint(q[14]), by = __double2hiint(q[14]);
+    const bool my = (fl & 1) != 0, two = (cb != 0.0);
     const double sg = (fl & 2) ? -1.0 : 1.0;
     const int cf = fl >> 2;
     const double d = c1 - c0, od = o1 - oc0;
@@ -219,7 +253,7 @@ __device__ __forceinline__ void edge_run(const ShootDev &S, const double *q, int
             if (my) ms = yl; else os = yl;
         }
     } else { ms = g0 + sg * (double)(m0 - 1); ts = dmin(dmax((ms - c0) * id, ta), tb); os = fma(ts, od, oc0); }
-    long long Gs = __double2ll_rn(cs * (my ? ms : os));
+    long long Gas = __double2ll_rn(ca * ((my ? ms : os) + da)), Gbs = two ? __double2ll_rn(cb * ((my ? ms : os) + db)) : 0ll;
 #pragma unroll 1
     for (int k = m0; k < m1; ++k) {
         double me, oe, te;
@@ -233,22 +267,23 @@ __device__ __forceinline__ void edge_run(const ShootDev &S, const double *q, int
                 if (my) me = yl; else oe = yl;
             }
         } else { me = g0 + sg * (double)k; te = dmin(dmax((me - c0) * id, ta), tb); oe = fma(te, od, oc0); }
-        const long long Ge = __double2ll_rn(cs * (my ? me : oe));
+        const long long Gae = __double2ll_rn(ca * ((my ? me : oe) + da)), Gbe = two ? __double2ll_rn(cb * ((my ? me : oe) + db)) : 0ll;
         // at most one grid line of the other axis lies strictly between os and oe
         const double gl = (oe > os) ? floor(os) + 1.0 : ceil(os) - 1.0;
         const bool cross = (od != 0.0) && ((oe > os) ? (gl < oe) : (gl > oe)) && (oe != os);
         double mg = me, og = oe;                               // where the first piece ends
-        long long Gg = Ge;
+        long long Gag = Gae, Gbg = Gbe;
         if (cross) {
             const double tg = dmin(dmax((gl - oc0) * oid, ts), te);
             mg = fma(tg, d, c0); og = gl;
-            Gg = __double2ll_rn(cs * (my ? mg : og));
+            Gag = __double2ll_rn(ca * ((my ? mg : og) + da));
+            if (two) Gbg = __double2ll_rn(cb * ((my ? mg : og) + db));
         }
         // the axes are swapped back before the deposit, so that one copy of it serves all lanes: the first piece,
         // then the second of those that cross
-        piece_deposit(S, my ? os : ms, my ? ms : os, my ? og : mg, my ? mg : og, Gg - Gs, bx, by);
-        if (cross) piece_deposit(S, my ? og : mg, my ? mg : og, my ? oe : me, my ? me : oe, Ge - Gg, bx, by);
-        ms = me; os = oe; ts = te; Gs = Ge;
+        piece_deposit(S, my ? os : ms, my ? ms : os, my ? og : mg, my ? mg : og, Gag - Gas, Gbg - Gbs, bx, by);
+        if (cross) piece_deposit(S, my ? og : mg, my ? mg : og, my ? oe : me, my ? me : oe, Gae - Gag, Gbe - Gbg, bx, by);
+        ms = me; os = oe; ts = te; Gas = Gae; Gbs = Gbe;
     }
 }
 
@@ -435,17 +470,14 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
     const int status = __shfl_sync(full, T.status, 0);
     if (status != 1) return 0ull;
     const double cs = __shfl_sync(full, T.cs, 0);
-    const int bx = __shfl_sync(full, T.bx, 0), by = __shfl_sync(full, T.by, 0);
-    const double fbx = (double)bx, fby = (double)by;
-    const double hgt = fmax(v[1], fmax(v[3], v[5])) - fby + 1.0;
-    const double ry0 = fmax(0.0, -fby), ry1 = fmin(hgt, (double)S.npix2 - fby), cx1 = (double)S.npix1 - fbx;
+    const int by = __shfl_sync(full, T.by, 0);
     __syncwarp();
     if (lane < 3) {
         const double xa = (lane == 0) ? v[0] : (lane == 1) ? v[2] : v[4], ya = (lane == 0) ? v[1] : (lane == 1) ? v[3] : v[5];
         const double xb = (lane == 0) ? v[2] : (lane == 1) ? v[4] : v[0], yb = (lane == 0) ? v[3] : (lane == 1) ? v[5] : v[1];
         EdgeWalk E;
-        edge_setup(E, xa - fbx, ya - fby, xb - fbx, yb - fby, ry0, ry1, cx1);
-        edge_record(E, scratch + EREC * lane);
+        edge_setup_canon(S, E, xa, ya, xb, yb);
+        edge_record(E, cs, by, scratch + EREC * lane);
     }
     __syncwarp();
     unsigned long long total = 0;
@@ -455,7 +487,7 @@ __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, c
         const int n = edge_record_steps(q);
         total += (unsigned long long)n;
 #pragma unroll 1
-        for (int m0 = lane * RUN; m0 < n; m0 += 32 * RUN) edge_run(S, q, m0, min(m0 + RUN, n), cs, bx, by);
+        for (int m0 = lane * RUN; m0 < n; m0 += 32 * RUN) edge_run(S, q, m0, min(m0 + RUN, n));
     }
     __syncwarp();
     return total;

@@ -140,10 +140,12 @@ __device__ __forceinline__ void cell_row(const ShootDev &S, const Win &W, WarpSh
     const bool act1 = cellv && !t1 && !(oa & ob & oc), act2 = cellv && !t2 && !(oa & oc & od);
     const unsigned b1 = __ballot_sync(full, act1), b2 = __ballot_sync(full, act2);
     const unsigned lt = (1u << lane) - 1u;
-    const int n1 = __popc(b1), idb = (prev << 6) | (lane << 1);
-    if (act1) Ws.ids[npend + __popc(b1 & lt)] = idb;
-    if (act2) Ws.ids[npend + n1 + __popc(b2 & lt)] = idb | 1;
-    npend += n1 + __popc(b2);
+    // (the two triangles of a cell next to each other, cells in lane order: neighbours in the mesh stay neighbours in the
+    // queue and in the walk list, where walk_kernel pairs the edges they share)
+    const int idb = (prev << 6) | (lane << 1), at = npend + __popc(b1 & lt) + __popc(b2 & lt);
+    if (act1) Ws.ids[at] = idb;
+    if (act2) Ws.ids[at + (act1 ? 1 : 0)] = idb | 1;
+    npend += __popc(b1) + __popc(b2);
 }
 
 // Apportions the `count` listed triangles of the row group, 32 at a time.  A triangle over two adjacent pixels is
@@ -341,13 +343,18 @@ static const int WB = 16;              // triangles per batch
 static const int GIANT_STEPS = 1024;   // a triangle with more steps than this is not walked by one warp alone
 static const int GIANT_CHUNK = 512;    // but edge by edge in chunks of this many steps: 32 lanes x GIANT_RUN consecutive steps
 static const int GIANT_RUN = GIANT_CHUNK / 32;
+struct WalkShared {                    // per warp (dynamic shared memory: 8 warps x 7.4 KB)
+    double er[3 * WB][EREC];           // edge records
+    double tr[WB][8];                  // global vertices, cs, (by, bx) of the triangle's frame
+    int pre[3 * WB];                   // inclusive prefix of the runs of the batch's edges
+    int pad[3 * WB];
+};
 __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_constant__ ShootDev S) {
-    __shared__ double er_s[WALK_WARPS][3 * WB][EREC];
-    __shared__ double tr_s[WALK_WARPS][WB][8];           // local vertices, cs, (bx, by)
-    __shared__ int pre_s[WALK_WARPS][3 * WB];            // inclusive prefix of the runs of the batch's edges
-    double (*er)[EREC] = er_s[threadIdx.x >> 5];
-    double (*tr)[8] = tr_s[threadIdx.x >> 5];
-    int *pre = pre_s[threadIdx.x >> 5];
+    extern __shared__ __align__(16) unsigned char walk_smem[];
+    WalkShared &Wk = reinterpret_cast<WalkShared *>(walk_smem)[threadIdx.x >> 5];
+    double (*er)[EREC] = Wk.er;
+    double (*tr)[8] = Wk.tr;
+    int *pre = Wk.pre;
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     long long nb = (long long)S.counters[C_BIG];
@@ -361,11 +368,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
     while (b < nbatch) {
         long long bnext = 0;
         if (lane == 0) bnext = (long long)atomicAdd(&S.counters[C_WALK], 1ull);
-        // ---- lane = triangle: local frame
+        // ---- lane = triangle: frame and weight
         const long long it = b * WB + lane;
         int status = 0;
         unsigned int qidx = 0;
-        double ry0 = 0.0, ry1 = 0.0, cx1 = 0.0;
         if (lane < WB && it < nb) {
             qidx = S.biglist[it];
             const double *e = S.queue + (size_t)qidx * QENT;
@@ -377,28 +383,30 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
             status = T.status;
             if (status == 1) {
                 double *q = tr[lane];
-                q[0] = T.x[0]; q[1] = T.y[0]; q[2] = T.x[1]; q[3] = T.y[1]; q[4] = T.x[2]; q[5] = T.y[2];
+#pragma unroll
+                for (int k = 0; k < QENT; ++k) q[k] = v[k];
                 q[6] = T.cs; q[7] = __hiloint2double(T.by, T.bx);
-                ry0 = T.ry0; ry1 = T.ry1; cx1 = T.cx1;
             }
         }
         __syncwarp();
-        // ---- lane = edge (3 WB of them, two passes)
+        // ---- lane = edge (3 WB of them, two passes): every edge in its own frame and canonical direction
 #pragma unroll
         for (int ps = 0; ps < 2; ++ps) {
             const int ed = ps * 32 + lane, ti = ed / 3, e = ed - 3 * ti, tis = min(ti, WB - 1);
             const int st = __shfl_sync(full, status, tis);
-            const double r0 = __shfl_sync(full, ry0, tis), r1 = __shfl_sync(full, ry1, tis), c1 = __shfl_sync(full, cx1, tis);
             if (ed < 3 * WB) {
                 EdgeWalk E;
-                E.n = 0; E.majorY = 1; E.sg = 1.0; E.cf = 0;
+                E.n = 0; E.majorY = 1; E.sg = 1.0; E.cf = 0; E.bx = 0; E.by = 0; E.fwd = 1;
                 E.x0 = E.y0 = E.x1 = E.y1 = E.idx = E.idy = E.ta = E.tb = E.g0 = 0.0;
+                double cs = 0.0;
+                int by_t = 0;
                 if (st == 1) {
                     const int e1 = (e == 2) ? 0 : e + 1;
                     const double *t = tr[ti];
-                    edge_setup(E, t[2 * e], t[2 * e + 1], t[2 * e1], t[2 * e1 + 1], r0, r1, c1);
+                    edge_setup_canon(S, E, t[2 * e], t[2 * e + 1], t[2 * e1], t[2 * e1 + 1]);
+                    cs = t[6]; by_t = __double2hiint(t[7]);
                 }
-                edge_record(E, er[ed]);
+                edge_record(E, cs, by_t, er[ed]);
             }
         }
         __syncwarp();
@@ -411,23 +419,73 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
             for (int e = 0; e < 3; ++e) nch += (edge_record_steps(er[3 * lane + e]) + GIANT_CHUNK - 1) / GIANT_CHUNK;
             unsigned long long at = atomicAdd(&S.counters[C_GIANT], (unsigned long long)nch);
             if ((long long)(at + nch) <= S.giant_cap) {           // (else it stays here; the skipped slots keep their sentinel)
-                const int by_t = __double2hiint(tr[lane][7]);
                 for (int e = 0; e < 3; ++e) {
                     const double *q = er[3 * lane + e];
                     const int nst = edge_record_steps(q);
                     const int ne = (nst + GIANT_CHUNK - 1) / GIANT_CHUNK;
-                    const int fl = __double2loint(q[9]);
+                    const int fl = __double2loint(q[9]), by_e = __double2hiint(q[14]);
                     for (int c = 0; c < ne; ++c) {
                         // the block of map rows around the middle step of the chunk (ordering key only)
                         const int m = min(c * GIANT_CHUNK + GIANT_CHUNK / 2, nst - 1);
                         const double ms = q[8] + ((fl & 2) ? -1.0 : 1.0) * (double)(m - 1);
                         const double y = (fl & 1) ? ms : fma(dmin(dmax((ms - q[0]) * q[4], q[6]), q[7]), q[3] - q[1], q[1]);
-                        const int row = min(max(__double2int_rd(y) + by_t, 0), S.npix2 - 1);
+                        const int row = min(max(__double2int_rd(y) + by_e, 0), S.npix2 - 1);
                         S.giant_key[at] = (unsigned char)min(row >> GIANT_BIN_SHIFT, GIANT_BINS - 2);
                         S.giant[at++] = ((unsigned long long)qidx << 20) | ((unsigned long long)e << 18) | (unsigned long long)c;
                     }
                 }
                 ntot = -1;                                          // gone
+            }
+        }
+        // ---- edges shared by two triangles of the batch are walked ONCE, for both (lane = edge, two passes).  T1 and T2 of
+        // a cell share its diagonal, T2 and the T1 of the cell before it a vertical edge, and the list keeps them next to
+        // each other: about a third of a batch's edges go.  Both triangles set the edge up from the same two end points in
+        // the same frame and direction, so the records agree bit for bit and the lower one takes the other's weight: the
+        // deposits are exactly those of two walks (deposit.cuh), whichever triangles happen to share a batch.
+        {
+            int partner[2] = {-1, -1};
+            // a 32-bit tag of the edge's geometry first (one integer compare per candidate), the full record on a hit;
+            // partners sit within three places of each other in the list
+#pragma unroll
+            for (int ps = 0; ps < 2; ++ps) {
+                const int ed = ps * 32 + lane;
+                if (ed < 3 * WB) {
+                    const double *q = er[ed];
+                    unsigned long long h = (unsigned long long)__double_as_longlong(q[0]) * 0x9E3779B97F4A7C15ull;
+                    h = (h ^ (h >> 29) ^ (unsigned long long)__double_as_longlong(q[1])) * 0xBF58476D1CE4E5B9ull;
+                    h = (h ^ (h >> 32) ^ (unsigned long long)__double_as_longlong(q[14])) * 0x94D049BB133111EBull;
+                    Wk.pad[ed] = (edge_record_steps(q) > 0) ? (int)((h >> 33) | 1ull) : 0;
+                }
+            }
+            __syncwarp();
+#pragma unroll
+            for (int ps = 0; ps < 2; ++ps) {
+                const int ed = ps * 32 + lane, ti = ed / 3;
+                const int tag = (ed < 3 * WB) ? Wk.pad[ed] : 0;
+                if (tag) {
+                    const int j0 = 3 * max(ti - 3, 0), j1 = 3 * min(ti + 4, WB);
+#pragma unroll 1
+                    for (int j = j0; j < j1; ++j)
+                        if (Wk.pad[j] == tag && j != ed && edge_record_same(er[ed], er[j])) partner[ps] = j;
+                }
+            }
+            __syncwarp();
+#pragma unroll
+            for (int ps = 0; ps < 2; ++ps) { const int ed = ps * 32 + lane; if (ed < 3 * WB) Wk.pad[ed] = partner[ps]; }
+            __syncwarp();
+            // a pair is made only if both see each other and neither triangle has left for the giants' list
+#pragma unroll
+            for (int ps = 0; ps < 2; ++ps) {
+                const int ed = ps * 32 + lane, j = partner[ps];
+                const int ntj = __shfl_sync(full, ntot, (j >= 0) ? j / 3 : 0);
+                bool keep = false, drop = false;
+                if (ed < 3 * WB && j >= 0 && ntj > 0 && Wk.pad[j] == ed) { keep = ed < j; drop = !keep; }
+                double c2 = 0.0, d2 = 0.0;
+                if (keep) { c2 = er[j][10]; d2 = er[j][11]; }
+                __syncwarp();
+                if (keep) { er[ed][12] = c2; er[ed][13] = d2; }
+                if (drop) er[ed][9] = __hiloint2double(0, __double2loint(er[ed][9]));
+                __syncwarp();
             }
         }
         // ---- runs per edge and their inclusive prefix (lane = edge, two passes)
@@ -451,11 +509,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
                 int lo = 0, hi = 3 * WB - 1;                        // first edge whose inclusive prefix exceeds r
 #pragma unroll
                 for (int k = 0; k < 6; ++k) { const int mid = (lo + hi) >> 1; const bool up = pre[mid] <= r; lo = up ? mid + 1 : lo; hi = up ? hi : mid; }
-                const int ed = min(lo, 3 * WB - 1), ti = ed / 3;
+                const int ed = min(lo, 3 * WB - 1);
                 const double *q = er[ed];
                 const int m0 = (r - (ed ? pre[ed - 1] : 0)) * RUN, m1 = min(m0 + RUN, edge_record_steps(q));
-                const double pk = tr[ti][7];
-                edge_run(S, q, m0, m1, tr[ti][6], __double2loint(pk), __double2hiint(pk));
+                edge_run(S, q, m0, m1);
                 steps += m1 - m0;
             }
         }
@@ -526,15 +583,15 @@ __global__ void __launch_bounds__(GIANT_WARPS * 32, 3) walk_giant_kernel(const _
         TriSetup T;
         tri_setup(S, W, v, T);
         if (T.status != 1) continue;                                // (cannot happen: walk_kernel found steps to walk)
-        const double xa = (e == 0) ? T.x[0] : (e == 1) ? T.x[1] : T.x[2], ya = (e == 0) ? T.y[0] : (e == 1) ? T.y[1] : T.y[2];
-        const double xb = (e == 0) ? T.x[1] : (e == 1) ? T.x[2] : T.x[0], yb = (e == 0) ? T.y[1] : (e == 1) ? T.y[2] : T.y[0];
+        const double xa = (e == 0) ? v[0] : (e == 1) ? v[2] : v[4], ya = (e == 0) ? v[1] : (e == 1) ? v[3] : v[5];
+        const double xb = (e == 0) ? v[2] : (e == 1) ? v[4] : v[0], yb = (e == 0) ? v[3] : (e == 1) ? v[5] : v[1];
         EdgeWalk E;
-        edge_setup(E, xa, ya, xb, yb, T.ry0, T.ry1, T.cx1);
+        edge_setup_canon(S, E, xa, ya, xb, yb);
         double q[EREC];
-        edge_record(E, q);
+        edge_record(E, T.cs, T.by, q);
         const int m0 = c * GIANT_CHUNK + lane * GIANT_RUN, m1 = min(m0 + GIANT_RUN, E.n);
         if (m0 < m1) {
-            edge_run(S, q, m0, m1, T.cs, T.bx, T.by);
+            edge_run(S, q, m0, m1);
             n_pieces += (unsigned long long)(m1 - m0);
         }
     }
@@ -893,6 +950,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
     const size_t smem_ipm = SHOOT_WARPS * sizeof(WarpSharedIpm), smem_irs = SHOOT_WARPS * sizeof(WarpShared);
     static std::atomic<int> attr_set[ML_MAXDEV];                     // kernel attributes are per device (context)
     if (!attr_set[device_slot()].load()) {
+        ML_CUDA(cudaFuncSetAttribute(walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(WALK_WARPS * sizeof(WalkShared))));
         ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
         ML_CUDA(cudaFuncSetAttribute(shoot_irs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_irs));
         ML_CUDA(cudaFuncSetAttribute(shoot_ipm_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_ipm));
@@ -948,7 +1006,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             }
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
             ML_TRY(mark());
-            ML_LAUNCH(walk_kernel, nsm * 3, WALK_WARPS * 32, 0, s, S);
+            ML_LAUNCH(walk_kernel, nsm * 3, WALK_WARPS * 32, WALK_WARPS * sizeof(WalkShared), s, S);
             ML_TRY(mark());
             ML_LAUNCH(giant_hist_kernel, nsm, 256, 0, s, S);
             ML_LAUNCH(giant_scatter_kernel, nsm, 256, 0, s, S);
