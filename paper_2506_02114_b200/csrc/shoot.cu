@@ -348,6 +348,7 @@ struct WalkShared {                    // per warp (dynamic shared memory: 8 war
     double tr[WB][8];                  // global vertices, cs, (by, bx) of the triangle's frame
     int pre[3 * WB];                   // inclusive prefix of the runs of the batch's edges
     int pad[3 * WB];
+    unsigned int qi[WB];               // queue entry of each triangle
 };
 __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_constant__ ShootDev S) {
     extern __shared__ __align__(16) unsigned char walk_smem[];
@@ -388,6 +389,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
                 q[6] = T.cs; q[7] = __hiloint2double(T.by, T.bx);
             }
         }
+        if (lane < WB) Wk.qi[lane] = qidx;
         __syncwarp();
         // ---- lane = edge (3 WB of them, two passes): every edge in its own frame and canonical direction
 #pragma unroll
@@ -410,33 +412,9 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
             }
         }
         __syncwarp();
-        // steps per triangle (lane < WB); a giant is shared out edge by edge in chunks to walk_giant_kernel
+        // steps per triangle (lane < WB)
         int ntot = 0;
         if (lane < WB) ntot = edge_record_steps(er[3 * lane]) + edge_record_steps(er[3 * lane + 1]) + edge_record_steps(er[3 * lane + 2]);
-        if (ntot > GIANT_STEPS) {
-            int nch = 0;
-#pragma unroll
-            for (int e = 0; e < 3; ++e) nch += (edge_record_steps(er[3 * lane + e]) + GIANT_CHUNK - 1) / GIANT_CHUNK;
-            unsigned long long at = atomicAdd(&S.counters[C_GIANT], (unsigned long long)nch);
-            if ((long long)(at + nch) <= S.giant_cap) {           // (else it stays here; the skipped slots keep their sentinel)
-                for (int e = 0; e < 3; ++e) {
-                    const double *q = er[3 * lane + e];
-                    const int nst = edge_record_steps(q);
-                    const int ne = (nst + GIANT_CHUNK - 1) / GIANT_CHUNK;
-                    const int fl = __double2loint(q[9]), by_e = __double2hiint(q[14]);
-                    for (int c = 0; c < ne; ++c) {
-                        // the block of map rows around the middle step of the chunk (ordering key only)
-                        const int m = min(c * GIANT_CHUNK + GIANT_CHUNK / 2, nst - 1);
-                        const double ms = q[8] + ((fl & 2) ? -1.0 : 1.0) * (double)(m - 1);
-                        const double y = (fl & 1) ? ms : fma(dmin(dmax((ms - q[0]) * q[4], q[6]), q[7]), q[3] - q[1], q[1]);
-                        const int row = min(max(__double2int_rd(y) + by_e, 0), S.npix2 - 1);
-                        S.giant_key[at] = (unsigned char)min(row >> GIANT_BIN_SHIFT, GIANT_BINS - 2);
-                        S.giant[at++] = ((unsigned long long)qidx << 20) | ((unsigned long long)e << 18) | (unsigned long long)c;
-                    }
-                }
-                ntot = -1;                                          // gone
-            }
-        }
         // ---- edges shared by two triangles of the batch are walked ONCE, for both (lane = edge, two passes).  T1 and T2 of
         // a cell share its diagonal, T2 and the T1 of the cell before it a vertical edge, and the list keeps them next to
         // each other: about a third of a batch's edges go.  Both triangles set the edge up from the same two end points in
@@ -473,19 +451,55 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, 3) walk_kernel(const __grid_c
 #pragma unroll
             for (int ps = 0; ps < 2; ++ps) { const int ed = ps * 32 + lane; if (ed < 3 * WB) Wk.pad[ed] = partner[ps]; }
             __syncwarp();
-            // a pair is made only if both see each other and neither triangle has left for the giants' list
+            // a pair is made only if both see each other
 #pragma unroll
             for (int ps = 0; ps < 2; ++ps) {
                 const int ed = ps * 32 + lane, j = partner[ps];
                 const int ntj = __shfl_sync(full, ntot, (j >= 0) ? j / 3 : 0);
                 bool keep = false, drop = false;
-                if (ed < 3 * WB && j >= 0 && ntj > 0 && Wk.pad[j] == ed) { keep = ed < j; drop = !keep; }
+                if (ed < 3 * WB && j >= 0 && ntj > 0 && Wk.pad[j] == ed) {
+                    const long long dq = (long long)Wk.qi[j / 3] - (long long)Wk.qi[ed / 3];
+                    if (dq >= -127 && dq <= 127) { keep = ed < j; drop = !keep; }
+                }
                 double c2 = 0.0, d2 = 0.0;
                 if (keep) { c2 = er[j][10]; d2 = er[j][11]; }
                 __syncwarp();
                 if (keep) { er[ed][12] = c2; er[ed][13] = d2; }
                 if (drop) er[ed][9] = __hiloint2double(0, __double2loint(er[ed][9]));
                 __syncwarp();
+            }
+        }
+        // ---- a triangle that still has more than GIANT_STEPS steps is shared out edge by edge in chunks to walk_giant_kernel;
+        // an edge it walks for a neighbour too takes the neighbour along (its queue entry, as an offset, and its edge)
+        if (lane < WB) ntot = edge_record_steps(er[3 * lane]) + edge_record_steps(er[3 * lane + 1]) + edge_record_steps(er[3 * lane + 2]);
+        if (ntot > GIANT_STEPS) {
+            int nch = 0;
+#pragma unroll
+            for (int e = 0; e < 3; ++e) nch += (edge_record_steps(er[3 * lane + e]) + GIANT_CHUNK - 1) / GIANT_CHUNK;
+            unsigned long long at = atomicAdd(&S.counters[C_GIANT], (unsigned long long)nch);
+            if ((long long)(at + nch) <= S.giant_cap) {           // (else it stays here; the skipped slots keep their sentinel)
+                for (int e = 0; e < 3; ++e) {
+                    const double *q = er[3 * lane + e];
+                    const int nst = edge_record_steps(q);
+                    const int ne = (nst + GIANT_CHUNK - 1) / GIANT_CHUNK;
+                    const int fl = __double2loint(q[9]), by_e = __double2hiint(q[14]);
+                    unsigned long long ent = ((unsigned long long)qidx << 20) | ((unsigned long long)e << 18);
+                    const int j = Wk.pad[3 * lane + e];
+                    if (q[12] != 0.0 && j >= 0) {
+                        const long long delta = (long long)Wk.qi[j / 3] - (long long)qidx;        // within +-127 (checked when paired)
+                        ent |= (1ull << 58) | ((unsigned long long)(j % 3) << 56) | ((unsigned long long)(delta + 128) << 48);
+                    }
+                    for (int c = 0; c < ne; ++c) {
+                        // the block of map rows around the middle step of the chunk (ordering key only)
+                        const int m = min(c * GIANT_CHUNK + GIANT_CHUNK / 2, nst - 1);
+                        const double ms = q[8] + ((fl & 2) ? -1.0 : 1.0) * (double)(m - 1);
+                        const double y = (fl & 1) ? ms : fma(dmin(dmax((ms - q[0]) * q[4], q[6]), q[7]), q[3] - q[1], q[1]);
+                        const int row = min(max(__double2int_rd(y) + by_e, 0), S.npix2 - 1);
+                        S.giant_key[at] = (unsigned char)min(row >> GIANT_BIN_SHIFT, GIANT_BINS - 2);
+                        S.giant[at++] = ent | (unsigned long long)c;
+                    }
+                }
+                ntot = -1;                                          // gone
             }
         }
         // ---- runs per edge and their inclusive prefix (lane = edge, two passes)
@@ -573,13 +587,18 @@ __global__ void __launch_bounds__(GIANT_WARPS * 32, 3) walk_giant_kernel(const _
     long long i = (long long)blockIdx.x * GIANT_WARPS + (threadIdx.x >> 5);
     unsigned long long ent_next = (i < n) ? S.giant_sorted[i] : 0ull;
     for (; i < n; i += stride) {
-        const unsigned long long ent = ent_next;                    // (queue entry << 20 | edge << 18 | chunk)
+        const unsigned long long ent = ent_next;                    // (partner: flag, edge, queue offset | queue entry << 20 | edge << 18 | chunk)
         if (i + stride < n) ent_next = S.giant_sorted[i + stride];  // on its way while this chunk is walked
         const int e = (int)((ent >> 18) & 3ull), c = (int)(ent & 0x3ffffull);
-        const double *p = S.queue + (size_t)(ent >> 20) * QENT;
-        double v[QENT];
+        const unsigned int qa = (unsigned int)((ent >> 20) & 0xfffffffull);
+        const bool two = ((ent >> 58) & 1ull) != 0;
+        const double *p = S.queue + (size_t)qa * QENT;
+        const double *p2 = S.queue + (size_t)((long long)qa + (long long)((ent >> 48) & 0xffull) - 128) * QENT;
+        double v[QENT], v2[QENT];
 #pragma unroll
         for (int k = 0; k < QENT; ++k) v[k] = __ldg(&p[k]);
+#pragma unroll
+        for (int k = 0; k < QENT; ++k) v2[k] = two ? __ldg(&p2[k]) : 0.0;
         TriSetup T;
         tri_setup(S, W, v, T);
         if (T.status != 1) continue;                                // (cannot happen: walk_kernel found steps to walk)
@@ -589,6 +608,18 @@ __global__ void __launch_bounds__(GIANT_WARPS * 32, 3) walk_giant_kernel(const _
         edge_setup_canon(S, E, xa, ya, xb, yb);
         double q[EREC];
         edge_record(E, T.cs, T.by, q);
+        if (two) {
+            // the neighbour across this edge: its weight, signed for the canonical direction, and its frame
+            TriSetup T2;
+            tri_setup(S, W, v2, T2);
+            if (T2.status == 1) {
+                const int e2 = (int)((ent >> 56) & 3ull);
+                const double xa2 = (e2 == 0) ? v2[0] : (e2 == 1) ? v2[2] : v2[4], ya2 = (e2 == 0) ? v2[1] : (e2 == 1) ? v2[3] : v2[5];
+                const double xb2 = (e2 == 0) ? v2[2] : (e2 == 1) ? v2[4] : v2[0], yb2 = (e2 == 0) ? v2[3] : (e2 == 1) ? v2[5] : v2[1];
+                const bool fwd2 = (xa2 < xb2) || (xa2 == xb2 && ya2 <= yb2);
+                q[12] = fwd2 ? T2.cs : -T2.cs; q[13] = (double)(E.by - T2.by);
+            }
+        }
         const int m0 = c * GIANT_CHUNK + lane * GIANT_RUN, m1 = min(m0 + GIANT_RUN, E.n);
         if (m0 < m1) {
             edge_run(S, q, m0, m1);
@@ -855,6 +886,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         if ((double)qmb > need_mb) qmb = (long long)need_mb;
         const long long qmb_env = d->queue_mb > 0 ? d->queue_mb : 0;       // the caller's choice, taken as it is
         if (qmb_env > 0) qmb = qmb_env;
+        if (qmb > 12000) qmb = 12000;                                       // queue entries are named by 28 bits (giant-chunk list)
         scratch_take(f, s);
         for (;;) {
             qcap = qmb * (1ll << 20) / (QCHUNK * QENT * 8);          // chunks
