@@ -286,7 +286,13 @@ __global__ void __launch_bounds__(SHOOT_WARPS * 32, 8) shoot_ipm_kernel(const __
 // large ones (among them the faint images of the whole map that every star in the window produces) are
 // walked edge by edge by the whole warp, cost ~ perimeter.
 static const int DRAIN_WARPS = 8;
-__global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_constant__ ShootDev S) {
+// (the walk list is full: cold, and out of line so that its registers are not the drain's)
+static __device__ __noinline__ unsigned long long walk_triangle_ool(const ShootDev *Sp, double a0, double a1, double a2, double a3, double a4, double a5,
+                                                                    double *scratch) {
+    const double v[QENT] = {a0, a1, a2, a3, a4, a5};
+    return walk_triangle(*Sp, v, scratch);
+}
+__global__ void __launch_bounds__(DRAIN_WARPS * 32, 3) drain_kernel(const __grid_constant__ ShootDev S) {
     __shared__ double rec_s[DRAIN_WARPS][32][10];
     double (*rec)[10] = rec_s[threadIdx.x >> 5];
     const unsigned full = 0xffffffffu;
@@ -323,7 +329,7 @@ __global__ void __launch_bounds__(DRAIN_WARPS * 32) drain_kernel(const __grid_co
                 double v[QENT];
 #pragma unroll
                 for (int k = 0; k < QENT; ++k) v[k] = base[(size_t)(b0 + i) * QENT + k];
-                n_pieces += walk_triangle(S, v, &rec[0][0]);
+                n_pieces += walk_triangle_ool(&S, v[0], v[1], v[2], v[3], v[4], v[5], &rec[0][0]);
             }
         }
     }
