@@ -371,6 +371,7 @@ def run_ours(args):
                             "achieved": rate, "peak": a_l2, "unit": "adds/s", "frac": rate / a_l2,
                             "peak_source": "random u64 atomic adds into a 16 MB (L2-resident) buffer, libmlens_bench, this run",
                             "map_sized_buffer_adds_per_s": a_map, "map_accumulator_bytes": 16 * npix * npix,
+                            "shared_memory_adds_per_s": ml.bench_shared_atomics(),
                             "frac_of_map_sized_rate": rate / a_map,
                             "adds_per_map": adds, "n_px_clipped": st["n_px_clipped"], "n_edge_steps": st["n_edge_steps"],
                             "kernel_ms_per_map": st["ms_drain"], "walk_ms": st["ms_walk"], "giant_ms": st["ms_giant"],

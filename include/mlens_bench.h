@@ -21,6 +21,11 @@ int mlens_bench_dfma(double *flops_per_s, void *stream);
  * according to its size. */
 int mlens_bench_atomics(int64_t n_slots, int32_t use_u64, double *adds_per_s, void *stream);
 
+/* Rate [adds/s] of 64-bit atomic adds at uniformly random slots of a 64 KB tile of SHARED memory per block (as many
+ * blocks per SM as fit): what a per-tile shared-memory accumulator could absorb.  On a B200 it equals the rate of
+ * L2-resident global adds. */
+int mlens_bench_shared_atomics(double *adds_per_s, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -4,7 +4,7 @@ Thin binding over the C ABI of include/mlens.h (libmlens.so, hand-written CUDA f
 Every step of the path runs in the library's kernels; there is no CPU fallback.
 """
 from .mlens import (  # noqa: F401
-    MlensError, Field, ShootResult, lib, version, bench_dfma, bench_atomics, launch_count,
+    MlensError, Field, ShootResult, lib, version, bench_dfma, bench_atomics, bench_shared_atomics, launch_count,
     SHAPE_DISC, SHAPE_RECT, MASS_EQUAL, MASS_POWER, EVAL_FMM, EVAL_DIRECT, EVAL_FMM_F32, MAP_IPM, MAP_IRS,
     BORDER_EQ16, BORDER_A6, BORDER_MARGIN, BORDER_EXPLICIT, MAX_ORDER, MAX_DIRECT,
     light_curve, histogram, INTERP_NEAREST, INTERP_BILINEAR,

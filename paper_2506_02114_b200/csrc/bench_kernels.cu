@@ -26,6 +26,23 @@ __global__ void atomics_kernel(unsigned long long *bu, double *bd, long long n_s
     }
 }
 
+// random 64-bit adds into a 64 KB tile of SHARED memory per block (three blocks per SM): what a per-tile accumulator
+// in shared memory could take in
+__global__ void __launch_bounds__(256) shared_atomics_kernel(unsigned long long *out, int nslots, int per_thread) {
+    extern __shared__ unsigned long long tile[];
+    for (int i = threadIdx.x; i < nslots; i += blockDim.x) tile[i] = 0ull;
+    __syncthreads();
+    unsigned long long h = (blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x + 1) * 0x9E3779B97F4A7C15ull;
+    for (int i = 0; i < per_thread; ++i) {
+        h ^= h >> 29; h *= 0xBF58476D1CE4E5B9ull; h ^= h >> 32;
+        atomicAdd(&tile[(int)(h % (unsigned long long)nslots)], (h >> 20) | (1ull << 34));
+    }
+    __syncthreads();
+    unsigned long long acc = 0ull;
+    for (int i = threadIdx.x; i < nslots; i += blockDim.x) acc += tile[i];
+    if (acc == 12345ull) out[0] = acc;
+}
+
 int sm_count() {
     int dev = 0, nsm = 148;
     cudaGetDevice(&dev);
@@ -93,6 +110,38 @@ out:
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
     if (buf) cudaFreeAsync(buf, s);
+    return rc;
+}
+
+int mlens_bench_shared_atomics(double *adds_per_s, void *stream) {
+    if (!adds_per_s) return -(int)cudaErrorInvalidValue;
+    cudaStream_t s = (cudaStream_t)stream;
+    const int smem = 64 * 1024, nslots = smem / 8, threads = 256, per = 4096;
+    int rc = 0, bps = 0;
+    float best = 1e30f;
+    unsigned long long *d = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int blocks = 0;
+    BK(cudaFuncSetAttribute(shared_atomics_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    BK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, shared_atomics_kernel, threads, smem));
+    blocks = sm_count() * (bps > 0 ? bps : 1);
+    BK(cudaMallocAsync(&d, 8, s));
+    BK(cudaEventCreate(&e0)); BK(cudaEventCreate(&e1));
+    shared_atomics_kernel<<<blocks, threads, smem, s>>>(d, nslots, 64);
+    for (int r = 0; r < 3; ++r) {
+        BK(cudaEventRecord(e0, s));
+        shared_atomics_kernel<<<blocks, threads, smem, s>>>(d, nslots, per);
+        BK(cudaEventRecord(e1, s));
+        BK(cudaEventSynchronize(e1));
+        float ms; BK(cudaEventElapsedTime(&ms, e0, e1));
+        if (ms < best) best = ms;
+    }
+    BK(cudaGetLastError());
+    *adds_per_s = (double)blocks * threads * per / (best * 1e-3);
+out:
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (d) cudaFreeAsync(d, s);
     return rc;
 }
 

@@ -364,6 +364,7 @@ def bench_lib():
         L = C.CDLL(_BENCH_SO)
         L.mlens_bench_dfma.argtypes = [_dp, C.c_void_p]
         L.mlens_bench_atomics.argtypes = [C.c_int64, C.c_int32, _dp, C.c_void_p]
+        L.mlens_bench_shared_atomics.argtypes = [_dp, C.c_void_p]
         _bench_lib = L
     return _bench_lib
 
@@ -382,6 +383,12 @@ def bench_dfma(stream=None):
 def bench_atomics(n_slots, use_u64=True, stream=None):
     v = C.c_double()
     _bench_check(bench_lib().mlens_bench_atomics(n_slots, int(use_u64), C.byref(v), _stream(stream)))
+    return v.value
+
+
+def bench_shared_atomics(stream=None):
+    v = C.c_double()
+    _bench_check(bench_lib().mlens_bench_shared_atomics(C.byref(v), _stream(stream)))
     return v.value
 
 
