@@ -459,7 +459,7 @@ __device__ __forceinline__ unsigned apportion_batch(const ShootDev &S, const Win
 // Warp-cooperative edge walk of one large triangle (v = its 3 vertices in pixel units, same in all lanes): the cold
 // copy, for the triangles that found the walk list or the queue full.  Lanes 0-2 set up one edge each into `scratch`
 // (3 x EREC doubles of the warp's shared memory); then the lanes take runs of consecutive steps of each edge in turn.
-static const int RUN = 8;             // consecutive steps of an edge a lane walks at a time
+static const int RUN = 4;             // consecutive steps of an edge a lane walks at a time
 __device__ __forceinline__ unsigned long long walk_triangle(const ShootDev &S, const double (&v)[QENT], double *scratch) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
