@@ -451,18 +451,6 @@ def run_ours(args):
                     f2 = ml.Field.seeded(c2.kappa_tot, c2.gamma, n_rect, c2.seed, kappa_star=c2.kappa_star, shape=ml.SHAPE_RECT,
                                          rect_aspect=c1r / c2r, mass_law=c2.mass_law, mass_a=c2.mass_a, mass_lo=c2.mass_lo, mass_hi=c2.mass_hi)
                     rec["n_stars_rect"] = n_rect
-                    if rep == 1:
-                        # the cost of the sheet term alone: the SAME stars (hence the same tree, lists and tiles) with the disc
-                        # sheet of eq 19 in place of the rectangle's eq B7/B8 (same area; a timing twin, not a lens model)
-                        xs_, ys_, ms_ = f2.stars()
-                        inf_ = f2.info()
-                        ft = ml.Field.from_stars(c2.kappa_tot, c2.gamma, xs_, ys_, ms_, kappa_star=c2.kappa_star,
-                                                 R=float(np.sqrt(4 * inf_["c1"] * inf_["c2"] / np.pi) * 4.0))
-                        for name, mode in (("ipm", ml.MAP_IPM), ("irs", ml.MAP_IRS)):
-                            for _ in range(2):
-                                rt_ = ft.shoot(c2.half_y, c2.npix, c2.rays_per_pixel_length, out=out2, map_mode=mode, **kw2)
-                            rec["same_stars_disc_sheet_" + name + "_shoot_ms"] = rt_.stats["ms_shoot"]
-                        ft.close()
                 else:
                     f2 = seeded(c2)
                 e1.record(stream); e1.synchronize()

@@ -149,6 +149,7 @@ static int finish_create(mlens_field *f, int order_req, cudaStream_t s) {
         }
         p = (p + 3 > MLENS_MAX_ORDER) ? MLENS_MAX_ORDER : p + 3;
     }
+    if (f->shape == MLENS_SHAPE_RECT) ML_TRY(rect_fold(f, s));
     return MLENS_OK;
 }
 

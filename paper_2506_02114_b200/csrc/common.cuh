@@ -97,6 +97,8 @@ struct Tree {
     DevBuf<int> near_cnt;                        // n_leaves
     DevBuf<double> near_x, near_y, near_m;       // n_leaves * ML_NEAR
     DevBuf<double2> ecoef;                       // n_leaves * P1: (l+1) c_{l+1} theta^2/L, l = 0..p-1
+    DevBuf<double2> ecoef_shoot;                 // rectangle fields: + the sheet's analytic part (fmm.cu rect_fold)
+    DevBuf<unsigned char> leaf_fold;             // n_leaves
     void release(cudaStream_t s);
 };
 
@@ -143,6 +145,7 @@ int build_tree(mlens_field *f, cudaStream_t s);
 // fmm.cu
 int fmm_prepare_tables(mlens_field *f, cudaStream_t s);
 int fmm_passes(mlens_field *f, cudaStream_t s);     // upward + downward + leaf coefficients for f->order
+int rect_fold(mlens_field *f, cudaStream_t s);      // rectangle fields: the sheet's analytic part into a copy of the leaf series
 // eval.cu
 int deflect_points(const mlens_field *f, int64_t n, const double *zx, const double *zy, double *ox_, double *oy_,
                    int eval_mode, int full_lens, cudaStream_t s);

@@ -44,6 +44,8 @@ struct LensDev {
     const int *near_cnt;
     const double *near_x, *near_y, *near_m;
     const double2 *ecoef;
+    const double2 *ecoef_shoot;         // rectangle fields: ecoef + the Taylor series of the sheet's analytic part (else = ecoef)
+    const unsigned char *leaf_fold;     // rectangle fields: 1 where ecoef_shoot holds that part
     int p, p1;                          // order, coefficients per expansion (stride of ecoef)
     // all stars (DIRECT mode and out-of-root fallback)
     const double *sx, *sy, *sm;

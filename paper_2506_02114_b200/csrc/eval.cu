@@ -19,6 +19,8 @@ LensDev make_lens_dev(const mlens_field *f) {
     L.child0 = t.child0.p; L.leaf_id = t.leaf_id.p; L.level = t.level.p; L.ix = t.ix.p; L.iy = t.iy.p;
     L.near_cnt = t.near_cnt.p; L.near_x = t.near_x.p; L.near_y = t.near_y.p; L.near_m = t.near_m.p;
     L.ecoef = t.ecoef.p;
+    L.ecoef_shoot = (f->shape == MLENS_SHAPE_RECT && t.ecoef_shoot.p) ? t.ecoef_shoot.p : t.ecoef.p;
+    L.leaf_fold = (f->shape == MLENS_SHAPE_RECT) ? t.leaf_fold.p : nullptr;
     L.p = f->order; L.p1 = f->order + 1;
     L.sx = f->sx.p; L.sy = f->sy.p; L.sm = f->sm.p;
     L.n_stars = f->n_stars;

@@ -317,6 +317,72 @@ __global__ void leaf_coef_kernel(FmmDev F, int n_leaves) {
     F.ecoef[(size_t)leaf * F.p1 + l] = v;
 }
 
+// Rectangle sheet inside the star rectangle (eq B8):  alpha_s = -kappa_star z + conj A(z),
+//   A(z) = (kappa_star i/pi) G(z) - kappa_star (2 c1 + z),   G(z) = sum_i s_i (a_i - z) log(a_i - z),
+// a_i = conj c, c, -conj c, -c and s_i = +1, -1, +1, -1: analytic in the open rectangle (the logarithms' cuts lie on its
+// upper and lower edges).  Its Taylor series about a leaf's centre z_c, in the leaf's variable zeta = (z - z_c)/L, is
+//   T_0 = A(z_c),  T_1 = A'(z_c) L  with G' = -sum s_i log(a_i - z),
+//   T_l = (kappa_star i/pi) sum_i s_i d_i w_i^l / (l (l-1)),  d_i = a_i - z_c,  w_i = L/d_i        (l >= 2)
+// and is ADDED to a copy of the leaf's derivative series (which sums to conj alpha_far): the shooting kernels' tiles shift
+// that copy to their centres and never see a logarithm.  A leaf whose square is not inside the rectangle, or so close to a
+// corner that the series converges slower than 0.4^l, keeps the plain series (flag 0): its tiles evaluate eq B7.
+__global__ void rect_fold_kernel(FmmDev F, int n_leaves, double c1, double c2, double kappa_star, double2 *ecoef_shoot,
+                                 unsigned char *leaf_fold) {
+    const int leaf = blockIdx.x, l = threadIdx.x;
+    if (leaf >= n_leaves) return;
+    const int node = F.leaf_node[leaf];
+    const double half = F.root_half / (double)(1 << F.level[node]);
+    const double cx = -F.root_half + (2.0 * F.ix[node] + 1.0) * half, cy = -F.root_half + (2.0 * F.iy[node] + 1.0) * half;
+    const double ks_pi = kappa_star * 0.31830988618379067154;
+    bool ok = fabs(cx) + half <= c1 && fabs(cy) + half <= c2;
+    double2 T = make_double2(0.0, 0.0);
+#pragma unroll 1
+    for (int i = 0; i < 4; ++i) {
+        const double sg = (i & 1) ? -1.0 : 1.0;
+        const double ax = (i < 2) ? c1 : -c1, ay = (i == 0 || i == 3) ? -c2 : c2;             // conj c, c, -conj c, -c
+        const double2 d = make_double2(ax - cx, ay - cy);
+        const double d2 = d.x * d.x + d.y * d.y;
+        if (!(2.0 * half * half < 0.16 * d2)) ok = false;                                        // (sqrt2 L / |d|)^2 < 0.4^2
+        if (!ok || l >= F.p) continue;
+        if (l == 0) {
+            const double lg = 0.5 * log(d2), ar = atan2(d.y, d.x);
+            T.x += sg * (d.x * lg - d.y * ar); T.y += sg * (d.x * ar + d.y * lg);
+        } else if (l == 1) {
+            T.x -= sg * 0.5 * log(d2) * half; T.y -= sg * atan2(d.y, d.x) * half;
+        } else {
+            const double2 w = make_double2(half * d.x / d2, -half * d.y / d2);
+            const double2 t = cmul(d, cpowi(w, l));
+            const double f = sg / (double)(l * (l - 1));
+            T.x += f * t.x; T.y += f * t.y;
+        }
+    }
+    T = make_double2(-ks_pi * T.y, ks_pi * T.x);
+    if (l == 0) { T.x -= kappa_star * (2.0 * c1 + cx); T.y -= kappa_star * cy; }
+    if (l == 1) T.x -= kappa_star * half;
+    if (l <= F.p) {
+        double2 e = F.ecoef[(size_t)leaf * F.p1 + l];
+        if (ok && l < F.p) { e.x += T.x; e.y += T.y; }
+        ecoef_shoot[(size_t)leaf * F.p1 + l] = e;
+    }
+    if (l == 0) leaf_fold[leaf] = ok ? 1 : 0;
+}
+
+int rect_fold(mlens_field *f, cudaStream_t s) {
+    Tree &t = f->tree;
+    const int p = f->order, p1 = p + 1;
+    const size_t nl = (size_t)t.n_leaves;
+    if (!nl) return MLENS_OK;
+    ML_TRY(t.ecoef_shoot.reserve(nl * p1, s, false));
+    ML_TRY(t.leaf_fold.reserve(nl, s, false));
+    FmmDev F{t.level.p, t.ix.p, t.iy.p, t.parent.p, t.child0.p, t.lo.p, t.n.p,
+             t.m2l_cnt.p, t.m2l_list.p, t.p2l_cnt.p, t.p2l_list.p, t.leaf_node.p,
+             f->sx.p, f->sy.p, f->sm.p, f->sqx.p, f->sqy.p, t.mp.p, t.loc.p, t.ecoef.p,
+             f->binom.p, f->tab.p, f->root_half, f->theta * f->theta, p, p1};
+    ML_LAUNCH(rect_fold_kernel, (unsigned)nl, 64, 0, s, F, (int)nl, f->c1, f->c2, f->kappa_star, t.ecoef_shoot.p, t.leaf_fold.p);
+    ML_CUDA(cudaGetLastError());
+    return MLENS_OK;
+}
+
 int fmm_passes(mlens_field *f, cudaStream_t s) {
     Tree &t = f->tree;
     const int p = f->order, p1 = p + 1;

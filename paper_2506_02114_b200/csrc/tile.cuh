@@ -108,7 +108,7 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 // Builds slot `s` of the warp's tile: shifted series + folded stars + direct-star list.
-__device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &W, const TileCtx &C, int s, double rt) {
+__device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &W, const TileCtx &C, int s, double rt, bool with_sheet) {
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int p = S.L.p;
@@ -119,7 +119,8 @@ __device__ __forceinline__ void wtile_build_slot(const ShootDev &S, WarpShared &
     const double cx = -S.L.root_half + (2.0 * __ldg(&S.L.ix[node]) + 1.0) * half;
     const double cy = -S.L.root_half + (2.0 * __ldg(&S.L.iy[node]) + 1.0) * half;
     const int cnt = __ldg(&S.L.near_cnt[leaf]);
-    for (int j = lane; j < p; j += 32) W.e[j] = S.L.ecoef[(size_t)leaf * S.L.p1 + j];
+    const double2 *ecoef = with_sheet ? S.L.ecoef_shoot : S.L.ecoef;       // with or without the rectangle sheet's analytic part
+    for (int j = lane; j < p; j += 32) W.e[j] = ecoef[(size_t)leaf * S.L.p1 + j];
     __syncwarp();
     // ---- shift of the derivative series to the tile centre: T_j = rho^j sum_m e_{j+m} C(j+m, j) zeta_t^m   (eq C7)
     const double ih = fast_rcp(half);
@@ -263,9 +264,18 @@ static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShar
         }
     }
     __syncwarp();
+    // Rectangle sheet inside the rectangle (eq B8): alpha_s = -kappa_star z + conj A(z), A analytic in the open
+    // rectangle; the Taylor coefficients of A about every leaf's centre were added to a copy of the leaf's series when the
+    // field was made (fmm.cu rect_fold_kernel), so the shift to the tile centre below carries the sheet along: no
+    // logarithm per ray (the paper pays four), none per tile.  A tile uses that copy if it lies inside the rectangle
+    // and its leaves' copies hold the term (leaves next to the rectangle's border keep eq B7).
+    bool fold = false;
+    if (S.L.shape == MLENS_SHAPE_RECT && S.L.leaf_fold && W.leaf[0] >= 0)
+        fold = fabs(C.zt_x) + rt <= S.L.c1 && fabs(C.zt_y) + rt <= S.L.c2 && __ldg(&S.L.leaf_fold[W.leaf[0]]) != 0 &&
+               (W.leaf[1] < 0 || __ldg(&S.L.leaf_fold[W.leaf[1]]) != 0);
     for (int s = 0; s < NSLOT; ++s) {
         if (W.leaf[s] < 0) continue;                              // warp-uniform
-        wtile_build_slot(S, W, C, s, rt);
+        wtile_build_slot(S, W, C, s, rt, fold);
         if (lane == 0 && W.mode[s] == 1 && full_counter) atomicAdd(full_counter, 1ull);
     }
     if (lane == 0 && W.leaf[0] >= 0) {
@@ -275,69 +285,7 @@ static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShar
     }
     // eq 19 inside the disc is linear in z: the farthest ray of the tile decides (the disc is convex)
     const double rmax = sqrt(C.zt_x * C.zt_x + C.zt_y * C.zt_y) + rt;
-    bool lin = S.L.shape == MLENS_SHAPE_DISC && rmax * rmax <= S.L.R2;
-    if (S.L.shape == MLENS_SHAPE_RECT && fabs(C.zt_x) + rt <= S.L.c1 && fabs(C.zt_y) + rt <= S.L.c2) {
-        // Rectangle sheet inside the rectangle (eq B8): alpha_s = -kappa_star z + conj A(z) with
-        //   A(z) = (kappa_star i/pi) G(z) - kappa_star (2 c1 + z),   G(z) = sum_i s_i (a_i - z) log(a_i - z),
-        // a_i = conj c, c, -conj c, -c and s_i = +1, -1, +1, -1 -- analytic in the open rectangle (the logarithms' cuts
-        // lie on its upper and lower edges).  Its Taylor series about the tile centre joins the tile series, so a ray
-        // costs nothing extra and no logarithm (hard part 8; the paper pays four per ray):
-        //   G' = -sum s_i log(a_i - z),   G^(n) = sum s_i (n-2)!/(a_i - z)^(n-1)  (n >= 2)
-        //   T_j = A^(j)(z_t) rt^j / j!;  for j >= 2:  T_j = (kappa_star i/pi) sum_i s_i (a_i - z_t) w_i^j / (j (j-1)),  w_i = rt/(a_i - z_t)
-        // The series converges within the distance to the nearest corner; the tile keeps the full eq B7 if its tail is not
-        // within the budget (tiles next to a corner of the rectangle).
-        int Qm = 0;
-        for (int s = 0; s < NSLOT; ++s) if (W.leaf[s] >= 0) Qm = max(Qm, W.q[s]);
-        const double ks_pi = S.L.kappa_star * 0.31830988618379067154;
-        const int j = lane;                                        // lane = term of the series
-        double2 Tj = make_double2(0.0, 0.0);
-        double tail = 0.0;
-        // the four logarithms, one corner per lane (a double-precision log and atan2 are a few hundred instructions each:
-        // once per tile, in parallel, not once per term)
-        double lg = 0.0, ar = 0.0;
-        {
-            const int i = lane & 3;
-            const double ax = (i < 2) ? S.L.c1 : -S.L.c1, ay = (i == 0 || i == 3) ? -S.L.c2 : S.L.c2;
-            const double dx = ax - C.zt_x, dy = ay - C.zt_y;
-            lg = 0.5 * log(dx * dx + dy * dy); ar = atan2(dy, dx);
-        }
-#pragma unroll 1
-        for (int i = 0; i < 4; ++i) {
-            const double sg = (i & 1) ? -1.0 : 1.0;
-            const double ax = (i < 2) ? S.L.c1 : -S.L.c1, ay = (i == 0 || i == 3) ? -S.L.c2 : S.L.c2;    // conj c, c, -conj c, -c
-            const double2 d = make_double2(ax - C.zt_x, ay - C.zt_y);
-            const double d2 = d.x * d.x + d.y * d.y, id2 = fast_rcp(d2);
-            const double2 w = make_double2(rt * d.x * id2, -rt * d.y * id2);         // rt / d
-            const double rho = rt * sqrt(id2);
-            const double lgi = __shfl_sync(full, lg, i), ari = __shfl_sync(full, ar, i);
-            if (j == 0) {
-                Tj.x += sg * (d.x * lgi - d.y * ari); Tj.y += sg * (d.x * ari + d.y * lgi);              // G: d log d
-            } else if (j == 1) {
-                Tj.x -= sg * lgi * rt; Tj.y -= sg * ari * rt;                                            // G' rt
-            } else if (j <= Qm) {
-                const double2 t = cmul(d, cpowi(w, j));
-                const double f = sg / (double)(j * (j - 1));
-                Tj.x += f * t.x; Tj.y += f * t.y;
-            }
-            // what the truncation after order Qm leaves out of this corner's part, geometric bound
-            double rq = rho;
-            for (int k = 0; k < Qm; ++k) rq *= rho;                                  // rho^(Qm+1)
-            tail += (rho < 0.5) ? ks_pi * sqrt(d2) * rq / ((double)(Qm * (Qm + 1)) * (1.0 - rho)) : 1.0e300;
-        }
-        // (kappa_star i/pi) G-part, then the polynomial part -kappa_star (2 c1 + z) in the terms 0 and 1
-        Tj = make_double2(-ks_pi * Tj.y, ks_pi * Tj.x);
-        if (j == 0) { Tj.x -= S.L.kappa_star * (2.0 * S.L.c1 + C.zt_x); Tj.y -= S.L.kappa_star * C.zt_y; }
-        if (j == 1) Tj.x -= S.L.kappa_star * rt;
-        const bool ok = (Qm >= 2) && (tail <= S.eps_far);         // the same in all lanes
-        if (ok) {
-            for (int s = 0; s < NSLOT; ++s) {
-                if (W.leaf[s] < 0) continue;
-                if (j <= W.q[s]) { double2 t0 = W.t[s][j]; W.t[s][j] = make_double2(t0.x + Tj.x, t0.y + Tj.y); }
-            }
-            lin = true;
-        }
-        __syncwarp();
-    }
+    const bool lin = (S.L.shape == MLENS_SHAPE_DISC && rmax * rmax <= S.L.R2) || fold;
     zero_window(W);
     if (lane == 0) {
         W.ctx[0] = C.zt_x; W.ctx[1] = C.zt_y; W.ctx[2] = C.inv_rt;

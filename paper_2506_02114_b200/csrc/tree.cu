@@ -351,7 +351,7 @@ void Tree::release(cudaStream_t s) {
     level.release(s); ix.release(s); iy.release(s); parent.release(s); child0.release(s); lo.release(s); n.release(s);
     leaf_id.release(s); nbr.release(s); m2l_cnt.release(s); m2l_list.release(s); p2l_cnt.release(s); p2l_list.release(s);
     mp.release(s); loc.release(s); leaf_node.release(s); near_cnt.release(s); near_x.release(s); near_y.release(s);
-    near_m.release(s); ecoef.release(s);
+    near_m.release(s); ecoef.release(s); ecoef_shoot.release(s); leaf_fold.release(s);
 }
 
 static int reserve_nodes(Tree &t, size_t n, cudaStream_t s) {
