@@ -439,15 +439,18 @@ def run_ours(args):
             kw2 = dict(border_mode=c2.border_mode, border_param=c2.border_param)
             out2 = torch.zeros((c2.npix, c2.npix), dtype=torch.float64, device=dev)
             rec = {}
+            if rect:
+                # the same lens with a RECTANGULAR star region sized for the same map (eq 20/21): side ratio
+                # of the shooting window, area from the rectangle's own corner formula, stars at the same density
+                f_tmp = seeded(c2)
+                g2 = f_tmp.grid(c2.half_y, c2.npix, c2.rays_per_pixel_length, **kw2)
+                f_tmp.close()
+                c1r, c2r = 1.2 * g2.H1 + 10.0, 1.2 * g2.H2 + 10.0
+                n_rect = int(round(c2.kappa_star * 4 * c1r * c2r / np.pi))
             for rep in range(2):
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record(stream)
                 if rect:
-                    # the same lens with a RECTANGULAR star region sized for the same map (eq 20/21): side ratio
-                    # of the shooting window, area from the rectangle's own corner formula, stars at the same density
-                    g2 = seeded(c2).grid(c2.half_y, c2.npix, c2.rays_per_pixel_length, **kw2)
-                    c1r, c2r = 1.2 * g2.H1 + 10.0, 1.2 * g2.H2 + 10.0
-                    n_rect = int(round(c2.kappa_star * 4 * c1r * c2r / np.pi))
                     f2 = ml.Field.seeded(c2.kappa_tot, c2.gamma, n_rect, c2.seed, kappa_star=c2.kappa_star, shape=ml.SHAPE_RECT,
                                          rect_aspect=c1r / c2r, mass_law=c2.mass_law, mass_a=c2.mass_a, mass_lo=c2.mass_lo, mass_hi=c2.mass_hi)
                     rec["n_stars_rect"] = n_rect
