@@ -170,7 +170,8 @@ typedef struct {
     int64_t n_near_terms;          /* near-field star terms summed directly over all rays (eq 23 direct part) */
     int64_t n_px_strip;            /* pixel deposits of the strips */
     int64_t n_px_clipped;          /* (triangle, pixel) pairs clipped exactly by the drain kernel */
-    int64_t n_edge_steps;          /* major-axis steps of the edge walk */
+    int64_t n_edge_steps;          /* major-axis steps of the edge walk (an edge walked once for the two triangles that share
+                                      it counts once) */
     int64_t reserved_;
     int64_t n_tiles_full;          /* tile slots whose truncation bound failed (evaluated with the leaf's full series) */
     int32_t tile_order;            /* order of the per-tile series */

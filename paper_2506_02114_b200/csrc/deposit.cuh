@@ -15,7 +15,8 @@
 //     with G(y) = round(c y) evaluated on values shared by consecutive pieces (vertices, grid lines, and the exact
 //     row line where the first or last row of the map cuts an edge).
 //     Cost is proportional to the triangle's perimeter in pixels, never to its area, and the result is the same
-//     area of intersection as clipping every pixel, up to rounding.
+//     area of intersection as clipping every pixel, up to rounding.  An edge is set up in a frame and direction of
+//     its own, so the two triangles that share it see identical pieces and walk_kernel walks it once for both.
 #pragma once
 #include "tile.cuh"
 
