@@ -419,6 +419,8 @@ def test_full_size_config1_in_bench_configuration(ml, orc):
     whole = f.shoot(*args, **kw)
     g = whole.grid
     assert whole.stats["n_queue_overflow"] == 0 and whole.stats["n_cells"] == g.n1 * g.n2
+    # every apportioning route is on this path: clipped boxes, walked triangles (shared edges paired), giants in chunks
+    assert whole.stats["n_px_clipped"] > 0 and whole.stats["n_tri_walked"] > 0 and whole.stats["n_giant_chunks"] > 0
     again = f.shoot(*args, **kw)
     assert torch.equal(whole.map, again.map)
     cuts = [0, g.n2 // 5, g.n2 // 2 + 7, g.n2]
