@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define MLENS_VERSION 100 /* 0.1.0 */
+#define MLENS_VERSION 200 /* 0.2.0: tuning fields in mlens_shoot_desc, more mlens_stats, benchmarks moved to mlens_bench.h */
 
 enum { MLENS_OK = 0, MLENS_EINVAL = -1, MLENS_ENOMEM = -2, MLENS_ECUDA = -3,
        MLENS_ERANGE = -4 /* requested accuracy not attainable with order <= MLENS_MAX_ORDER, or tree depth exhausted */,
