@@ -762,3 +762,41 @@ def test_f32_mode_cluster_regime(ml, orc):
         # the paper's FP32 maps underestimate locally by ~20 %; here the means agree to 1e-4 and no more than
         # 1 % of the pixels (those on caustics, where 1e-7 theta moves a fold by a fraction of a pixel) differ by 1e-3
         assert abs(stats[3] - 1.0) <= 1e-4 and stats[1] <= 1e-2 and stats[2] <= 1e-4, (name, stats)
+
+
+def test_full_size_config4_in_bench_configuration(ml):
+    """BASELINE configs[4] whole (1e7 stars, 10^4 x 10^4 pixels, 2.4e11 rays), launched exactly as bench.py launches it:
+    the properties that hold at any size.  Two runs give the same bits (integer accumulation; shared edges paired by
+    whatever triangles share a batch must not show); two row slabs add up to the whole map; no queue overflow, every
+    apportioning route taken; the mean magnification lies within eq 16's 1 % deficit of 1/|(1-kappa)^2-gamma^2| (plus the
+    sampling scatter of one seed over a 200 x 200 theta_E map); the IRS map carries the same flux.  The oracle's
+    pixel-by-pixel word on this configuration is test_ipm_patches_big_configs[4-*] and test_deflection_parity[4-*]."""
+    import torch
+    cfg = synth.get_config(4)
+    dev = torch.device("cuda")
+    f = ml.Field.seeded(cfg.kappa_tot, cfg.gamma, cfg.n_stars, cfg.seed, kappa_star=cfg.kappa_star, mass_law=cfg.mass_law,
+                        mass_a=cfg.mass_a, mass_lo=cfg.mass_lo, mass_hi=cfg.mass_hi)
+    kw = dict(border_mode=cfg.border_mode, border_param=cfg.border_param)
+    args = (cfg.half_y, cfg.npix, cfg.rays_per_pixel_length)
+    whole = f.shoot(*args, device=dev, **kw)
+    g, st = whole.grid, whole.stats
+    assert st["n_queue_overflow"] == 0 and st["n_cells"] == g.n1 * g.n2 and st["n_bands"] > 100
+    assert st["n_px_clipped"] > 0 and st["n_tri_walked"] > 0 and st["n_giant_chunks"] > 0
+    assert st["n_tri_single"] + st["n_tri_strip"] + st["n_tri_queued"] <= 2 * st["n_cells"]
+    mu_th = 1.0 / abs((1 - cfg.kappa_tot) ** 2 - cfg.gamma ** 2)
+    mean_ipm = float(whole.map.mean())
+    assert 0.975 * mu_th <= mean_ipm <= 1.01 * mu_th, (mean_ipm, mu_th)
+    assert float(whole.map.min()) >= 0.0
+    ref = whole.map.clone()
+    again = f.shoot(*args, out=whole.map, **kw)
+    assert torch.equal(again.map, ref)
+    vmax = float(ref.max())
+    cut = int(g.n2) // 2 + 13
+    acc = torch.zeros_like(ref)
+    for a, b in ((0, cut), (cut, int(g.n2))):
+        f.shoot(*args, sub=(0, int(g.n1), a, b), out=acc, accumulate=True, **kw)
+    assert float((acc - ref).abs().max()) <= 4e-16 * vmax + 8 * g.weight * 2.0 ** -36
+    del acc
+    irs = f.shoot(*args, map_mode=ml.MAP_IRS, out=whole.map, **kw)
+    assert float(irs.map.mean()) == pytest.approx(mean_ipm, rel=2e-3)
+    f.close()
