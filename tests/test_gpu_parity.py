@@ -800,3 +800,39 @@ def test_full_size_config4_in_bench_configuration(ml):
     irs = f.shoot(*args, map_mode=ml.MAP_IRS, out=whole.map, **kw)
     assert float(irs.map.mean()) == pytest.approx(mean_ipm, rel=2e-3)
     f.close()
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13, 14, 15, 16])
+def test_walk_everything_random_fields(ml, orc, seed):
+    """The edge walk under varied geometry: random small fields (positive and negative parity, with and without smooth
+    matter, mass spectrum or not, off-centre non-square maps) with EVERY general triangle walked (small_px = 1: shared
+    edges paired, map-border clips, giants in chunks) against the same map with every one clipped pixel by pixel, and
+    against the oracle pixel by pixel."""
+    rng = np.random.default_rng(seed)
+    n = int(rng.integers(40, 400))
+    ks = float(rng.uniform(0.05, 0.5))
+    kt = ks + float(rng.uniform(0.0, 0.3))
+    gam = float(rng.uniform(0.0, 0.5)) * (1 if rng.random() < 0.5 else -1)
+    if abs((1 - kt) ** 2 - gam ** 2) < 0.05:
+        gam *= 0.5
+    R = math.sqrt(n / ks)
+    xs, ys, ms = synth.disc_stars(n, R, 100 + seed, synth.get_config(2) if seed % 2 else None)
+    gf = ml.Field.from_stars(kt, gam, xs, ys, ms, kappa_star=ks, R=R)
+    of = orc.Field.make(kt, ks, gam, xs, ys, ms, R=R)
+    half = (float(rng.uniform(1.0, 3.0)), float(rng.uniform(1.0, 3.0)))
+    npix = (int(rng.integers(40, 90)), int(rng.integers(40, 90)))
+    Y = (float(rng.uniform(-1, 1)), float(rng.uniform(-1, 1)))
+    k = float(rng.choice([1.0, 2.0, 3.0]))
+    g = orc.geometry(kt, ks, gam, half, npix, k, 0, Y=Y, m2_over_m=float(np.mean(ms ** 2) / np.mean(ms)))
+    kw = dict(border_mode=ml.BORDER_EQ16, center=Y)
+    walk = gf.shoot(half, npix, k, small_px=1, **kw)
+    clip = gf.shoot(half, npix, k, small_px=100000000, **kw)
+    assert (walk.grid.n1, walk.grid.n2) == (g.n1, g.n2)
+    assert walk.stats["n_tri_walked"] > 0 and clip.stats["n_tri_walked"] == 0 and walk.stats["n_queue_overflow"] == 0
+    ref = orc.shoot(of, g, 0)
+    _map_check(walk.map, ref, f"walk-all seed {seed}")
+    _map_check(clip.map, ref, f"clip-all seed {seed}")
+    assert np.max(np.abs(walk.map - clip.map)) <= 1e-9 * ref.max()
+    assert walk.map.sum() == pytest.approx(ref.sum(), rel=1e-9)
+    again = gf.shoot(half, npix, k, small_px=1, **kw)
+    assert np.array_equal(again.map, walk.map)
