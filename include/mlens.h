@@ -254,6 +254,29 @@ int mlens_map_light_curve(const double *map, int32_t npix1, int32_t npix2, doubl
 int mlens_map_histogram(const double *map, int64_t n, double mu_ref, double lo, double hi, int32_t nbins,
                         uint64_t *counts, int32_t ptr_kind, void *stream);
 
+/* The same histogram (Fig 5, Fig 10; same bins, same counts to the last unit) for callers that cannot let
+ * the library allocate device memory.  That is the case in a process whose memory manager has claimed the whole GPU up
+ * front (an inference server, a framework's caching allocator at its cap: any allocation of ours would fail there), and
+ * on paths where an allocation's hidden costs are not acceptable (it can serialise against work on other streams, and
+ * it can fail at a moment the caller cannot recover from).  mlens_map_histogram takes the device copy of its bin-edge
+ * table from the device's memory pool on every call; this entry point keeps that table in a fixed array inside the
+ * library image instead and calls no cudaMalloc / cudaMallocAsync / cudaFree or other allocating routine.
+ *   - map (n values) and counts (nbins + 2, overwritten) are DEVICE pointers owned by the caller; host pointers are
+ *     refused with MLENS_EINVAL (copying them over would need a buffer).
+ *   - nbins <= MLENS_HIST_STATIC_MAXBINS; more is refused with MLENS_EINVAL and a message naming the limit.  The table
+ *     costs (MLENS_HIST_STATIC_MAXBINS + 1) * 8 bytes = 32 KB on every GPU the library is loaded on, until the process ends.
+ *   - the first call on each device looks the table's device address up (with that device current) and sets the
+ *     kernel's attributes; make that first call before any stream capture starts.
+ *   - all calls on a device share the one table.  A call overwrites the entries it uses before its kernel reads them,
+ *     so leftovers of earlier calls are never seen and nothing needs clearing; calls on the same stream are ordered
+ *     and safe, but two calls whose work can overlap on the GPU (different streams, different host threads) race on
+ *     the table and may count with each other's edges: serialise them.
+ *   - work is enqueued on `stream`; the call returns without waiting for the kernel (its copy of the edges from
+ *     pageable host memory may wait for earlier work on that stream). */
+#define MLENS_HIST_STATIC_MAXBINS 4096
+int mlens_map_histogram_static(const double *map, int64_t n, double mu_ref, double lo, double hi, int32_t nbins,
+                               uint64_t *counts, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -113,3 +113,62 @@ int map_light_curve(const double *map, int npix1, int npix2, double ylo1, double
 }
 
 }  // namespace ml
+
+// ---- mlens_map_histogram_static: the histogram for callers that must not allocate device memory -------------------
+// histogram_kernel reads its bin edges from global memory.  mlens_map_histogram gets that table from the device's
+// memory pool on every call; here it lives in the library's own image instead: one fixed array per GPU, there from the
+// moment the library is loaded on that GPU until the process ends, shared by every call of this entry point.
+static __device__ __align__(256) double g_static_hist_edges[MLENS_HIST_STATIC_MAXBINS + 1];
+
+namespace ml {
+// In host code `g_static_hist_edges` is only a handle for the runtime's symbol calls, not somewhere a kernel can read:
+// the array's address on the CURRENT device is asked for once per device and kept here.
+static int static_hist_edges(double **out) {
+    static std::atomic<double *> addr[ML_MAXDEV];                   // zero-initialised; one slot per device
+    int dev = 0;
+    ML_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= ML_MAXDEV) { set_error("device ordinal %d beyond the %d this table holds", dev, ML_MAXDEV); return MLENS_EINVAL; }
+    double *p = addr[dev].load();
+    if (!p) {
+        ML_CUDA(cudaGetSymbolAddress((void **)&p, g_static_hist_edges));
+        if (!p) { set_error("cudaGetSymbolAddress gave a null address for the static edge table"); return MLENS_ECUDA; }
+        addr[dev].store(p);                                         // two threads racing here store the same value
+    }
+    *out = p;
+    return MLENS_OK;
+}
+
+static int must_be_device_memory(const void *p, const char *what) {
+    cudaPointerAttributes a;
+    ML_CUDA(cudaPointerGetAttributes(&a, p));
+    if (a.type != cudaMemoryTypeDevice && a.type != cudaMemoryTypeManaged) {
+        set_error("%s must be device memory: this entry point stages nothing (it may not allocate)", what);
+        return MLENS_EINVAL;
+    }
+    return MLENS_OK;
+}
+}  // namespace ml
+
+extern "C" int mlens_map_histogram_static(const double *map, int64_t n, double mu_ref, double lo, double hi, int32_t nbins,
+                                          uint64_t *counts, void *stream) {
+    using namespace ml;
+    if (nbins > MLENS_HIST_STATIC_MAXBINS) {
+        set_error("nbins = %d is more than the static edge table holds (MLENS_HIST_STATIC_MAXBINS = %d); "
+                  "use mlens_map_histogram, which allocates", nbins, MLENS_HIST_STATIC_MAXBINS);
+        return MLENS_EINVAL;
+    }
+    if (!counts || n < 0 || (n > 0 && !map) || nbins < 1 || !(mu_ref > 0) || !(hi > lo)) { set_error("bad arguments"); return MLENS_EINVAL; }
+    ML_TRY(must_be_device_memory(counts, "counts"));
+    if (n > 0) ML_TRY(must_be_device_memory(map, "map"));
+    // the same expression as mlens_map_histogram (api.cu), so the two entry points decide every pixel alike
+    double edges[MLENS_HIST_STATIC_MAXBINS + 1];                     // 32 KB of stack, no heap
+    for (int j = 0; j <= nbins; ++j) edges[j] = mu_ref * pow(10.0, lo + (double)j * (hi - lo) / (double)nbins);
+    for (int j = 1; j <= nbins; ++j) if (!(edges[j] > edges[j - 1])) { set_error("bins too narrow for float64 edges"); return MLENS_EINVAL; }
+    double *dedges = nullptr;
+    ML_TRY(static_hist_edges(&dedges));                              // first call on a device: looks the array up
+    cudaStream_t s = (cudaStream_t)stream;
+    // Entries 0..nbins are overwritten, the kernel reads no others: whatever an earlier call left behind is never seen
+    // and nothing has to be zeroed.  `edges` is pageable, so the runtime has taken its copy when this returns.
+    ML_CUDA(cudaMemcpyAsync(dedges, edges, (size_t)(nbins + 1) * sizeof(double), cudaMemcpyHostToDevice, s));
+    return map_histogram(map, n, dedges, nbins, reinterpret_cast<unsigned long long *>(counts), s);
+}

@@ -120,6 +120,7 @@ def lib():
         dbl = C.c_double
         L.mlens_map_light_curve.argtypes = [vp, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, dbl, dbl, i64, i32, vp, i32, vp]
         L.mlens_map_histogram.argtypes = [vp, i64, dbl, dbl, dbl, i32, vp, i32, vp]
+        L.mlens_map_histogram_static.argtypes = [vp, i64, dbl, dbl, dbl, i32, vp, vp]
         _lib = L
     return _lib
 
@@ -428,3 +429,23 @@ def histogram(map_, mu_ref, lo, hi, nbins, stream=None):
                                      C.c_int32(nbins), _ptr(out)[0], C.c_int32(kind), _stream(stream)))
     return out
 
+
+
+HIST_STATIC_MAXBINS = 4096
+
+
+def histogram_static(map_, mu_ref, lo, hi, nbins, out, stream=None):
+    """mlens_map_histogram_static: histogram() for callers that cannot let the library allocate device memory (a
+    process whose own memory manager holds the whole GPU, or a path where an allocation's stall or failure is not
+    acceptable).  The bin edges go into a fixed 32 KB table inside the library instead of a pool allocation, so:
+    nbins <= HIST_STATIC_MAXBINS; `map_` and `out` are contiguous torch CUDA tensors the caller made beforehand (`out`:
+    nbins + 2 int64, overwritten with [below, bins..., above]); nothing here allocates, not even the result.  Calls share
+    the table: keep them on one stream or otherwise from overlapping.  The first call on a device does a one-time
+    set-up and belongs before any stream capture.  Returns `out`."""
+    if not (_is_torch(map_) and _is_torch(out)):
+        raise MlensError("histogram_static takes torch CUDA tensors only (host arrays would need a staging allocation)")
+    if not map_.is_contiguous() or int(out.numel()) != nbins + 2 or out.element_size() != 8:
+        raise MlensError("histogram_static: map_ must be contiguous and out must hold nbins + 2 64-bit integers")
+    _check(lib().mlens_map_histogram_static(_ptr(map_)[0], C.c_int64(int(map_.numel())), C.c_double(mu_ref), C.c_double(lo),
+                                            C.c_double(hi), C.c_int32(nbins), _ptr(out)[0], _stream(stream)))
+    return out
