@@ -318,12 +318,12 @@ def run_ours(args):
     except OSError:
         pass
 
-    # ---- roofline of the fused evaluate + IPM deposit kernel: bound by plain FP64 ALU work.
-    # Work = SURVEY 8(d)'s algorithmic flops of the paper's per-ray scheme x the UNIQUE rays of the map (tile-border
-    # corners that the kernel evaluates twice are not counted): the mean near-field list of a ray's leaf (measured in
-    # the run, per tile) summed directly + the leaf's order-p series by Horner + the macro and sheet terms.
-    # The kernel itself executes less (series re-expanded per 32 x 32-ray tile at order 6-15, distant near-field stars
-    # folded into it): `achieved_executed` counts what it really issues for the evaluation.
+    # ---- roofline of the fused evaluate + IPM deposit kernel, DESIGN.md s7.
+    # `achieved` = the FP64 flops the kernel ISSUES for the evaluation (series re-expanded per 32 x 32-ray tile at order
+    # 6-15, the near-field stars it sums directly, macro and sheet terms) / its time, against the measured DFMA rate.
+    # Beside it, for context: SURVEY 8(d)'s algorithmic flops of the paper's per-ray scheme x the UNIQUE rays of the map
+    # (tile-border corners that the kernel evaluates twice are not counted): the mean near-field list of a ray's leaf
+    # (measured in the run, per tile) summed directly + the leaf's order-p series by Horner + the macro terms.
     st = state["ipm"]
     p = state["info"]["order"]
     n_near_leaf = st["n_near_leaf_sum"] / max(1, st["n_tiles"])
@@ -337,21 +337,31 @@ def run_ours(args):
     nsm = torch.cuda.get_device_properties(dev).multi_processor_count
     peak_derived = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     peak_dfma = ml.bench_dfma() / 1e12
-    achieved_tf = flop_alg / t_shoot / 1e12 if t_shoot > 0 else 0.0
+    # `achieved` and `frac` count the flops the kernel really ISSUES for the evaluation (tile series of order
+    # 6-15 + the near stars it sums directly + macro terms), against the measured DFMA rate: hardware utilisation.
+    # The paper's per-ray scheme would need `flop_per_eval_algorithmic` per ray; what that scheme's work divided by this
+    # kernel's time comes to is kept as `achieved_paper_equivalent` (an algorithmic speed-up figure, not utilisation).
+    # The kernel is bound by instruction issue (bookkeeping around the evaluation), not by the FP64 pipe: DESIGN.md s7.
+    paper_tf = flop_alg / t_shoot / 1e12 if t_shoot > 0 else 0.0
+    achieved_tf = flop_exec / t_shoot / 1e12 if t_shoot > 0 else 0.0
     # DRAM traffic of the launches, from the run's own counters: every queued triangle is written once (48 B) by this
     # kernel; the per-tile leaf data and the map windows are L2 hits
     traffic = st["n_tri_queued"] * QUEUE_ENTRY_BYTES / n_l
     roofline = {"bound": "alu", "kernel": "shoot_ipm_kernel", "achieved": achieved_tf, "peak": peak_dfma,
                 "unit": "TFLOP/s", "frac": achieved_tf / peak_dfma if peak_dfma > 0 else None,
+                "achieved_source": "FP64 flops the kernel issues for the evaluation (mlens_stats: n_near_terms, tile_order, n_rays) / summed CUDA-event time of its launches",
                 "traffic": traffic,
                 "traffic_source": "n_tri_queued x 48 B of queue writes / launches (mlens_stats of the timed run); ncu dram bytes of a capture are in profiles/",
                 "peak_source": "FP64 FMA rate measured by libmlens_bench (mlens_bench_dfma) in this run",
                 "peak_derived": peak_derived,
                 "peak_derived_source": f"{nsm} SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {sm_max:.0f} MHz",
+                "achieved_paper_equivalent": paper_tf,
+                "frac_paper_equivalent": paper_tf / peak_dfma if peak_dfma > 0 else None,
+                "paper_equivalent_source": "SURVEY 8(d) flops of the paper's per-ray scheme (leaf near list + order-p Horner) x unique rays / the same time: not utilisation",
+                "limiter": "instruction issue (ncu: profiles/r02_ncu_full.md), not the FP64 pipe",
                 "flop_per_eval_algorithmic": flop_per_eval, "near_stars_per_leaf_mean": n_near_leaf, "order_p": p,
                 "unique_rays": rays_unique, "rays_evaluated": st["n_rays"],
-                "flop_per_launch": flop_alg / n_l, "flop_executed_per_launch": flop_exec / n_l,
-                "achieved_executed": flop_exec / t_shoot / 1e12 if t_shoot > 0 else 0.0,
+                "flop_per_launch": flop_exec / n_l, "flop_paper_equivalent_per_launch": flop_alg / n_l,
                 "launch_ms": t_shoot * 1e3 / n_l, "launches_per_map": n_l, "kernel_ms_per_map": st["ms_shoot"],
                 "share_of_step": t_shoot / sec}
 
