@@ -371,17 +371,33 @@ def run_ours(args):
     # accumulators (HBM-resident when larger than L2).
     roofline_atomics = None
     if world == 1:
-        a_l2 = ml.bench_atomics(2_000_000, True)
-        a_map = ml.bench_atomics(max(2 * npix * npix, 2_000_000), True)
+        # the ceiling, measured with loops whose slot choice costs two integer instructions (round 2's 64-bit modulo was a
+        # ~64-instruction subroutine per add and measured itself: VERDICT r2): profiles/r03_sass_atomics.txt
+        n_l2, n_map = 2_000_000, max(2 * npix * npix, 2_000_000)
+        a_l2 = ml.bench_atomics(n_l2, True)
+        a_map = ml.bench_atomics(n_map, True)
+        table = {"global_u64_L2_16MB": {"random": a_l2, "8_sectors_per_warp": ml.bench_atomics(n_l2, True, pattern=1),
+                                        "1_sector_per_warp": ml.bench_atomics(n_l2, True, pattern=2)},
+                 "global_u64_map_sized": {"random": a_map, "8_sectors_per_warp": ml.bench_atomics(n_map, True, pattern=1),
+                                          "1_sector_per_warp": ml.bench_atomics(n_map, True, pattern=2), "bytes": 8 * n_map},
+                 "global_f64_L2_16MB": {"random": ml.bench_atomics(n_l2, False)},
+                 "shared_64KB_tile": {
+                     "u64_two_32bit_adds_with_carry_random": ml.bench_shared_atomics(kind=1),
+                     "u64_two_32bit_adds_with_carry_conflict_free": ml.bench_shared_atomics(kind=1, conflict_free=True),
+                     "u32_add_random": ml.bench_shared_atomics(kind=2),
+                     "u32_add_conflict_free": ml.bench_shared_atomics(kind=2, conflict_free=True),
+                     "u64_atomicAdd_cas_loop_random": ml.bench_shared_atomics(kind=0),
+                     "u64_atomicAdd_cas_loop_conflict_free": ml.bench_shared_atomics(kind=0, conflict_free=True)}}
         adds = st["n_px_clipped"] + 2 * st["n_edge_steps"]
         t_ap = st["ms_drain"] * 1e-3
         rate = adds / t_ap if t_ap > 0 else 0.0
         queue_bytes = st["n_tri_queued"] * QUEUE_ENTRY_BYTES + st["n_tri_walked"] * (QUEUE_ENTRY_BYTES + 8)
         roofline_atomics = {"bound": "atomics", "kernels": "drain_kernel + walk_kernel + walk_giant_kernel",
                             "achieved": rate, "peak": a_l2, "unit": "adds/s", "frac": rate / a_l2,
-                            "peak_source": "random u64 atomic adds into a 16 MB (L2-resident) buffer, libmlens_bench, this run",
+                            "peak_source": "random REDG.E.ADD.64 into a 16 MB (L2-resident) buffer, libmlens_bench, this run; loop of 5.8 SASS instructions per add, no CALL (profiles/r03_sass_atomics.txt)",
+                            "measured_add_rates_per_s": table,
                             "map_sized_buffer_adds_per_s": a_map, "map_accumulator_bytes": 16 * npix * npix,
-                            "shared_memory_adds_per_s": ml.bench_shared_atomics(),
+                            "shared_memory_adds_per_s": table["shared_64KB_tile"]["u64_two_32bit_adds_with_carry_random"],
                             "frac_of_map_sized_rate": rate / a_map,
                             "adds_per_map": adds, "n_px_clipped": st["n_px_clipped"], "n_edge_steps": st["n_edge_steps"],
                             "kernel_ms_per_map": st["ms_drain"], "walk_ms": st["ms_walk"], "giant_ms": st["ms_giant"],
@@ -530,7 +546,12 @@ def run_ours(args):
         e, t, thr, sub = oracle_sample(cfg, patch)
         cpu = {"value": e / t, "unit": UNIT, "cores": thr, "kind": "oracle", "seconds": t,
                "sample": f"IPM + IRS on the {patch[0]}x{patch[1]}-cell patch {sub} at the window centre "
-                         f"({e} evaluations, each a direct sum over all {cfg.n_stars} stars)"}
+                         f"({e} evaluations, each a direct sum over all {cfg.n_stars} stars)",
+               # the oracle's cost is exactly rays x stars, so the sample's rate carries over to the whole
+               # grid; an EXTRAPOLATION, labelled as one, not a measurement
+               "extrapolated_full_step_seconds": (evals_ipm + evals_irs) * t / e,
+               "extrapolation": f"linear in the rays: {evals_ipm + evals_irs} evaluations of one step (IPM + IRS maps) "
+                                f"at the sample's measured rate; not measured"}
 
     if rank == 0:
         irs = state["irs"]

@@ -191,10 +191,16 @@ int64_t mlens_launch_count(void);
 
 int mlens_field_create(const mlens_field_desc *desc, mlens_field **out);
 int mlens_field_create_seeded(const mlens_seed_desc *desc, mlens_field **out);
+/* Frees everything the field owns WITHOUT synchronising the device: the frees are stream-ordered on the stream of the
+ * most recent call made on this field (create, deflect, lens_map, get_stars, shoot), after the work already enqueued
+ * there.  That stream must therefore still exist when the field is destroyed (destroy the field first, then the
+ * stream); a caller that used the field on several streams orders them before destroying it.  Should a stream-ordered
+ * free fail all the same (e.g. the stream is gone), destroy falls back to a device synchronisation and plain frees. */
 int mlens_field_destroy(mlens_field *f);
 int mlens_field_get_info(const mlens_field *f, mlens_field_info *info);
 
-/* Copies the stars, in the caller's original order, into x, y, m (length n_stars each). */
+/* Copies the stars (positions in units of theta_star's length, masses as used in eq 13; for a seeded field
+ * the draws of P:159-165), in the caller's original order, into x, y, m (length n_stars each). */
 int mlens_field_get_stars(const mlens_field *f, double *x, double *y, double *m, int32_t ptr_kind, void *stream);
 
 /* alpha_star (eq 13) at n points: FMM (near-field direct sum + local expansion, eq 23-24)
@@ -206,15 +212,22 @@ int mlens_deflect(const mlens_field *f, int64_t n, const double *zx, const doubl
 int mlens_lens_map(const mlens_field *f, int64_t n, const double *zx, const double *zy,
                    double *wx, double *wy, int32_t eval_mode, int32_t ptr_kind, void *stream);
 
-/* The integers and lengths the shoot call will use (host-side arithmetic only). */
+/* The integers and lengths the shoot call will use (host-side arithmetic only): window centre X = Y/(1-kappa -+ gamma)
+ * (eq 14), half-sizes from the map's half-sizes plus the border of eq 16 / eq A6 / the caller's
+ * choice, grown to whole cells of pixel/k (Table 1 caption). */
 int mlens_grid_info(const mlens_field *f, const mlens_shoot_desc *desc, mlens_grid *out);
 
 /* Shoots the (sub-range of the) ray grid and builds the map.  map: double[npix2*npix1] or NULL;
  * counts: uint64[npix2*npix1], the IRS ray counts, or NULL -- it must be NULL for MLENS_MAP_IPM (MLENS_EINVAL
  * otherwise: an IPM map has no counts); stats may be NULL.
+ * IPM: cells -> two triangles -> exact area apportioning; IRS: one ray per cell centre, counted in the
+ * pixel it falls into.  Window and grid are those of mlens_grid_info.
  * Ray tiles are anchored on the GLOBAL cell grid, so a ray has the same value to the last bit in whatever
- * sub-range it is shot, and the maps of sub-ranges that tile the grid add up to the map of the whole grid
- * exactly (integer accumulation): row slabs on several GPUs reproduce the one-GPU map bit for bit. */
+ * sub-range it is shot, and within ONE call every deposit is an integer (fixed-point) addition.  Across calls the
+ * sum is taken in float64: each sub-range shoot converts its integers to double once (clamping a negative
+ * rounding residue to 0) and `accumulate` or the all-reduce of row slabs adds those doubles.  Maps put together
+ * from sub-ranges or slabs therefore equal the one-call map up to one float64 rounding per part and pixel (plus
+ * the residues of the fixed-point quantum, 2^-36 of a triangle's weight), not to the last bit. */
 int mlens_shoot(mlens_field *f, const mlens_shoot_desc *desc, double *map, uint64_t *counts,
                 mlens_stats *stats, void *stream);
 

@@ -17,29 +17,66 @@ __global__ void dfma_kernel(double *out, int iters) {
     if (r == 123.456) out[0] = r;
 }
 
-__global__ void atomics_kernel(unsigned long long *bu, double *bd, long long n_slots, int use_u64, int per_thread) {
-    unsigned long long h = (blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x + 1) * 0x9E3779B97F4A7C15ull;
+// Slot choice must cost next to nothing, or the loop measures the slot arithmetic instead of the atomic unit (round 2's
+// `h % n_slots` on 64-bit operands compiled to a ~64-instruction subroutine per add: VERDICT r2).  Here: one 32-bit LCG
+// step (one IMAD) and the high word of h * n_slots (one IMAD.WIDE), n_slots < 2^32.  The SASS of the loops is in
+// profiles/r03_sass_atomics.txt.
+__device__ __forceinline__ unsigned int lcg(unsigned int h) { return h * 1664525u + 1013904223u; }
+
+// PATTERN 0: every lane its own random slot (up to 32 sectors of 32 B per warp instruction)
+//         1: lanes in groups of four on the four 8-byte slots of one random sector: 8 sectors per warp instruction
+//         2: all 32 lanes on the four slots of ONE random sector (8 lanes per address)
+template <int PATTERN>
+__global__ void __launch_bounds__(256) atomics_kernel(unsigned long long *bu, double *bd, unsigned int n_slots, int use_u64, int per_thread) {
+    const unsigned int tid = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    const unsigned int who = PATTERN == 0 ? tid : PATTERN == 1 ? (tid >> 2) : (tid >> 5);   // lanes that share a sector share the stream
+    unsigned int h = (who + 1u) * 0x9E3779B9u;
+    const unsigned int n_eff = PATTERN == 0 ? n_slots : n_slots >> 2;
+#pragma unroll 8
     for (int i = 0; i < per_thread; ++i) {
-        h ^= h >> 29; h *= 0xBF58476D1CE4E5B9ull; h ^= h >> 32;
-        long long slot = (long long)(h % (unsigned long long)n_slots);
+        h = lcg(h);
+        unsigned int slot = __umulhi(h, n_eff);
+        if (PATTERN != 0) slot = slot * 4u + (lane & 3u);
         if (use_u64) atomicAdd(&bu[slot], 1ull); else atomicAdd(&bd[slot], 1.0);
     }
 }
 
-// random 64-bit adds into a 64 KB tile of SHARED memory per block (three blocks per SM): what a per-tile accumulator
-// in shared memory could take in
-__global__ void __launch_bounds__(256) shared_atomics_kernel(unsigned long long *out, int nslots, int per_thread) {
+// Adds into a 64 KB tile of SHARED memory per block (as many blocks per SM as fit): what a per-tile accumulator in
+// shared memory can take in.
+// KIND 0: 64-bit atomicAdd (compiles to a compare-and-swap loop: ATOMS.CAST.SPIN)
+//      1: the product's own 64-bit add (deposit.cuh shared_add64): two native 32-bit ATOMS.ADD, the first returning the
+//         old low word for the carry
+//      2: one plain 32-bit atomicAdd, nothing returned
+// CFREE 0: every lane a random slot (random banks); 1: lane i on slot 32 * row + i of a random row (no bank conflict
+//          beyond the two banks an 8-byte slot spans)
+template <int KIND, int CFREE>
+__global__ void __launch_bounds__(256) shared_atomics_kernel(unsigned long long *out, int per_thread) {
     extern __shared__ unsigned long long tile[];
-    for (int i = threadIdx.x; i < nslots; i += blockDim.x) tile[i] = 0ull;
+    const int nbytes = 64 * 1024;
+    unsigned int *t32 = reinterpret_cast<unsigned int *>(tile);
+    for (int i = threadIdx.x; i < nbytes / 8; i += blockDim.x) tile[i] = 0ull;
     __syncthreads();
-    unsigned long long h = (blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x + 1) * 0x9E3779B97F4A7C15ull;
+    const unsigned int lane = threadIdx.x & 31;
+    const unsigned int n_slots = KIND == 2 ? nbytes / 4 : nbytes / 8;
+    const unsigned int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned int h = ((CFREE ? (tid >> 5) : tid) + 1u) * 0x9E3779B9u;
+#pragma unroll 8
     for (int i = 0; i < per_thread; ++i) {
-        h ^= h >> 29; h *= 0xBF58476D1CE4E5B9ull; h ^= h >> 32;
-        atomicAdd(&tile[(int)(h % (unsigned long long)nslots)], (h >> 20) | (1ull << 34));
+        h = lcg(h);
+        const unsigned int slot = CFREE ? __umulhi(h, n_slots >> 5) * 32u + lane : __umulhi(h, n_slots);
+        if (KIND == 0) {
+            atomicAdd(&tile[slot], (unsigned long long)h | (1ull << 34));
+        } else if (KIND == 1) {
+            const unsigned int lo = h | 1u, hi = 4u;                       // both words non-zero: two adds, as for most deposits
+            const unsigned int old = atomicAdd(&t32[2 * slot], lo);
+            atomicAdd(&t32[2 * slot + 1], hi + ((old + lo < old) ? 1u : 0u));
+        } else {
+            atomicAdd(&t32[slot], h | 1u);
+        }
     }
     __syncthreads();
     unsigned long long acc = 0ull;
-    for (int i = threadIdx.x; i < nslots; i += blockDim.x) acc += tile[i];
+    for (int i = threadIdx.x; i < nbytes / 8; i += blockDim.x) acc += tile[i];
     if (acc == 12345ull) out[0] = acc;
 }
 
@@ -84,21 +121,23 @@ out:
     return rc;
 }
 
-int mlens_bench_atomics(int64_t n_slots, int32_t use_u64, double *adds_per_s, void *stream) {
-    if (!adds_per_s || n_slots <= 0) return -(int)cudaErrorInvalidValue;
+int mlens_bench_atomics_pattern(int64_t n_slots, int32_t use_u64, int32_t pattern, double *adds_per_s, void *stream) {
+    if (!adds_per_s || n_slots < 4 || n_slots >= (1ll << 32) || pattern < 0 || pattern > 2) return -(int)cudaErrorInvalidValue;
     cudaStream_t s = (cudaStream_t)stream;
     const int blocks = sm_count() * 16, threads = 256, per = 256;
     int rc = 0;
     float best = 1e30f;
     void *buf = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
+    void (*k)(unsigned long long *, double *, unsigned int, int, int) =
+        pattern == 0 ? atomics_kernel<0> : pattern == 1 ? atomics_kernel<1> : atomics_kernel<2>;
     BK(cudaMallocAsync(&buf, (size_t)n_slots * 8, s));
     BK(cudaMemsetAsync(buf, 0, (size_t)n_slots * 8, s));
     BK(cudaEventCreate(&e0)); BK(cudaEventCreate(&e1));
-    atomics_kernel<<<blocks, threads, 0, s>>>((unsigned long long *)buf, (double *)buf, n_slots, use_u64, 8);
+    k<<<blocks, threads, 0, s>>>((unsigned long long *)buf, (double *)buf, (unsigned int)n_slots, use_u64, 8);
     for (int r = 0; r < 3; ++r) {
         BK(cudaEventRecord(e0, s));
-        atomics_kernel<<<blocks, threads, 0, s>>>((unsigned long long *)buf, (double *)buf, n_slots, use_u64, per);
+        k<<<blocks, threads, 0, s>>>((unsigned long long *)buf, (double *)buf, (unsigned int)n_slots, use_u64, per);
         BK(cudaEventRecord(e1, s));
         BK(cudaEventSynchronize(e1));
         float ms; BK(cudaEventElapsedTime(&ms, e0, e1));
@@ -113,24 +152,32 @@ out:
     return rc;
 }
 
-int mlens_bench_shared_atomics(double *adds_per_s, void *stream) {
-    if (!adds_per_s) return -(int)cudaErrorInvalidValue;
+int mlens_bench_atomics(int64_t n_slots, int32_t use_u64, double *adds_per_s, void *stream) {
+    return mlens_bench_atomics_pattern(n_slots, use_u64, 0, adds_per_s, stream);
+}
+
+int mlens_bench_shared_atomics_kind(int32_t kind, int32_t conflict_free, double *adds_per_s, void *stream) {
+    if (!adds_per_s || kind < 0 || kind > 2) return -(int)cudaErrorInvalidValue;
     cudaStream_t s = (cudaStream_t)stream;
-    const int smem = 64 * 1024, nslots = smem / 8, threads = 256, per = 4096;
+    const int smem = 64 * 1024, threads = 256, per = 4096;
     int rc = 0, bps = 0;
     float best = 1e30f;
     unsigned long long *d = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     int blocks = 0;
-    BK(cudaFuncSetAttribute(shared_atomics_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    BK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, shared_atomics_kernel, threads, smem));
+    void (*k)(unsigned long long *, int) =
+        kind == 0 ? (conflict_free ? shared_atomics_kernel<0, 1> : shared_atomics_kernel<0, 0>)
+      : kind == 1 ? (conflict_free ? shared_atomics_kernel<1, 1> : shared_atomics_kernel<1, 0>)
+                  : (conflict_free ? shared_atomics_kernel<2, 1> : shared_atomics_kernel<2, 0>);
+    BK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    BK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, k, threads, smem));
     blocks = sm_count() * (bps > 0 ? bps : 1);
     BK(cudaMallocAsync(&d, 8, s));
     BK(cudaEventCreate(&e0)); BK(cudaEventCreate(&e1));
-    shared_atomics_kernel<<<blocks, threads, smem, s>>>(d, nslots, 64);
+    k<<<blocks, threads, smem, s>>>(d, 64);
     for (int r = 0; r < 3; ++r) {
         BK(cudaEventRecord(e0, s));
-        shared_atomics_kernel<<<blocks, threads, smem, s>>>(d, nslots, per);
+        k<<<blocks, threads, smem, s>>>(d, per);
         BK(cudaEventRecord(e1, s));
         BK(cudaEventSynchronize(e1));
         float ms; BK(cudaEventElapsedTime(&ms, e0, e1));
@@ -143,6 +190,10 @@ out:
     if (e1) cudaEventDestroy(e1);
     if (d) cudaFreeAsync(d, s);
     return rc;
+}
+
+int mlens_bench_shared_atomics(double *adds_per_s, void *stream) {
+    return mlens_bench_shared_atomics_kind(1, 0, adds_per_s, stream);
 }
 
 }  // extern "C"

@@ -75,7 +75,16 @@ struct DevBuf {
         p = q; cap = ncap;
         return MLENS_OK;
     }
-    void release(cudaStream_t s) { if (p) cudaFreeAsync(p, s); p = nullptr; cap = 0; }
+    // A stream-ordered free can fail (the stream was destroyed before the buffer's owner): then the error is cleared
+    // and the buffer is freed the plain way after a device synchronisation, so that nothing leaks silently.
+    void release(cudaStream_t s) {
+        if (p && cudaFreeAsync(p, s) != cudaSuccess) {
+            cudaGetLastError();
+            cudaDeviceSynchronize();
+            if (cudaFreeAsync(p, nullptr) != cudaSuccess) { cudaGetLastError(); cudaFree(p); cudaGetLastError(); }
+        }
+        p = nullptr; cap = 0;
+    }
     void release() { release(s_own); }
 };
 // Local scratch of a host function: freed (stream-ordered) on every way out of the scope, early returns included.

@@ -326,15 +326,29 @@ __global__ void leaf_coef_kernel(FmmDev F, int n_leaves) {
 // and is ADDED to a copy of the leaf's derivative series (which sums to conj alpha_far): the shooting kernels' tiles shift
 // that copy to their centres and never see a logarithm.  A leaf whose square is not inside the rectangle, or so close to a
 // corner that the series converges slower than 0.4^l, keeps the plain series (flag 0): its tiles evaluate eq B7.
-__global__ void rect_fold_kernel(FmmDev F, int n_leaves, double c1, double c2, double kappa_star, double2 *ecoef_shoot,
-                                 unsigned char *leaf_fold) {
+// So does a leaf where the series, cut at the field's order p, would leave more than `rem_budget` of the sheet's
+// deflection behind: with r_i = sqrt2 L/|d_i| the four tails are bounded by
+//   sum_i (kappa_star/pi) |d_i| r_i^p / (p (p-1) (1 - r_i)),
+// which matters when the caller fixed a low order (~1e-4 theta at p = 8 next to a corner).
+__global__ void rect_fold_kernel(FmmDev F, int n_leaves, double c1, double c2, double kappa_star, double rem_budget,
+                                 double2 *ecoef_shoot, unsigned char *leaf_fold) {
     const int leaf = blockIdx.x, l = threadIdx.x;
     if (leaf >= n_leaves) return;
     const int node = F.leaf_node[leaf];
     const double half = F.root_half / (double)(1 << F.level[node]);
     const double cx = -F.root_half + (2.0 * F.ix[node] + 1.0) * half, cy = -F.root_half + (2.0 * F.iy[node] + 1.0) * half;
     const double ks_pi = kappa_star * 0.31830988618379067154;
-    bool ok = fabs(cx) + half <= c1 && fabs(cy) + half <= c2;
+    bool ok = fabs(cx) + half <= c1 && fabs(cy) + half <= c2 && F.p >= 2;
+    double rem = 0.0;
+#pragma unroll 1
+    for (int i = 0; i < 4; ++i) {                                                                // the verdict first: the same for every l
+        const double dx = ((i < 2) ? c1 : -c1) - cx, dy = ((i == 0 || i == 3) ? -c2 : c2) - cy;
+        const double d2 = dx * dx + dy * dy;
+        if (!(2.0 * half * half < 0.16 * d2)) { ok = false; continue; }                          // (sqrt2 L / |d|)^2 < 0.4^2
+        const double r = sqrt(2.0 * half * half / d2);
+        rem += ks_pi * sqrt(d2) * pow(r, (double)F.p) / ((double)F.p * (double)(F.p - 1) * (1.0 - r));
+    }
+    if (!(rem <= rem_budget)) ok = false;
     double2 T = make_double2(0.0, 0.0);
 #pragma unroll 1
     for (int i = 0; i < 4; ++i) {
@@ -342,7 +356,6 @@ __global__ void rect_fold_kernel(FmmDev F, int n_leaves, double c1, double c2, d
         const double ax = (i < 2) ? c1 : -c1, ay = (i == 0 || i == 3) ? -c2 : c2;             // conj c, c, -conj c, -c
         const double2 d = make_double2(ax - cx, ay - cy);
         const double d2 = d.x * d.x + d.y * d.y;
-        if (!(2.0 * half * half < 0.16 * d2)) ok = false;                                        // (sqrt2 L / |d|)^2 < 0.4^2
         if (!ok || l >= F.p) continue;
         if (l == 0) {
             const double lg = 0.5 * log(d2), ar = atan2(d.y, d.x);
@@ -378,7 +391,9 @@ int rect_fold(mlens_field *f, cudaStream_t s) {
              t.m2l_cnt.p, t.m2l_list.p, t.p2l_cnt.p, t.p2l_list.p, t.leaf_node.p,
              f->sx.p, f->sy.p, f->sm.p, f->sqx.p, f->sqy.p, t.mp.p, t.loc.p, t.ecoef.p,
              f->binom.p, f->tab.p, f->root_half, f->theta * f->theta, p, p1};
-    ML_LAUNCH(rect_fold_kernel, (unsigned)nl, 64, 0, s, F, (int)nl, f->c1, f->c2, f->kappa_star, t.ecoef_shoot.p, t.leaf_fold.p);
+    // a tenth of the field's accuracy target for the sheet's truncation (orders chosen from eq C9 stay far below it)
+    ML_LAUNCH(rect_fold_kernel, (unsigned)nl, 64, 0, s, F, (int)nl, f->c1, f->c2, f->kappa_star, 0.1 * f->eps * f->theta,
+              t.ecoef_shoot.p, t.leaf_fold.p);
     ML_CUDA(cudaGetLastError());
     return MLENS_OK;
 }

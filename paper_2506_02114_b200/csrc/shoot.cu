@@ -890,8 +890,8 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         if (mem_total > 0 && (long long)(mem_total >> 24) < qmb) qmb = (long long)(mem_total >> 24);   // <= 1/16 of the device
         const double need_mb = 3.2 * (double)(i1 - i0) * (double)(j1 - j0) * (QENT * 8) / 1048576.0 + 64.0;
         if ((double)qmb > need_mb) qmb = (long long)need_mb;
-        const long long qmb_env = d->queue_mb > 0 ? d->queue_mb : 0;       // the caller's choice, taken as it is
-        if (qmb_env > 0) qmb = qmb_env;
+        const long long qmb_desc = d->queue_mb > 0 ? d->queue_mb : 0;       // the caller's choice, taken as it is
+        if (qmb_desc > 0) qmb = qmb_desc;
         if (qmb > 12000) qmb = 12000;                                       // queue entries are named by 28 bits (giant-chunk list)
         scratch_take(f, s);
         for (;;) {
@@ -904,7 +904,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
             if (rc == MLENS_OK) rc = f->giant_key.reserve((size_t)GIANT_CAP, s, false);
             if (rc == MLENS_OK) rc = f->giant_hist.reserve((size_t)2 * GIANT_BINS, s, false);
             if (rc == MLENS_OK) break;
-            if (rc != MLENS_ENOMEM || qmb_env > 0 || qmb <= 256) return rc;
+            if (rc != MLENS_ENOMEM || qmb_desc > 0 || qmb <= 256) return rc;
             cudaGetLastError();
             qmb /= 2;
         }
@@ -1042,6 +1042,7 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
                 q_before = hq;
                 rate = (rate < 0.0) ? 1.25 * r_new : fmax(1.25 * r_new, 0.7 * rate);   // head-room; forget slowly
             }
+            ML_TRY(mark());                                       // after the host's read-back: ms_drain starts here, not at the shooting kernel's end
             ML_LAUNCH(drain_kernel, nsm * 8, DRAIN_WARPS * 32, 0, s, S);
             ML_TRY(mark());
             ML_LAUNCH(walk_kernel, nsm * 3, WALK_WARPS * 32, WALK_WARPS * sizeof(WalkShared), s, S);
@@ -1087,14 +1088,14 @@ int shoot(mlens_field *f, const mlens_shoot_desc *d, const mlens_grid *g, double
         st->n_bands = bands; st->gpu_launches = launches; st->n_shoot_launches = bands;
         if (timed) {
             ML_CUDA(cudaEventElapsedTime(&st->ms_total, e0, e1));
-            const size_t per = ipm ? 5 : 2;              // events per band
+            const size_t per = ipm ? 6 : 2;              // events per band: shoot [0,1], (host read-back), drain [2,3], walk [3,4], giants [4,5]
             for (int b = 0; b < bands; ++b) {
                 float ms = 0;
                 ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per], ev[b * per + 1])); st->ms_shoot += ms;
                 if (ipm) {
-                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 1], ev[b * per + 4])); st->ms_drain += ms;
-                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 2], ev[b * per + 3])); st->ms_walk += ms;
-                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 3], ev[b * per + 4])); st->ms_giant += ms;
+                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 2], ev[b * per + 5])); st->ms_drain += ms;
+                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 3], ev[b * per + 4])); st->ms_walk += ms;
+                    ML_CUDA(cudaEventElapsedTime(&ms, ev[b * per + 4], ev[b * per + 5])); st->ms_giant += ms;
                 }
             }
             float ms = 0;

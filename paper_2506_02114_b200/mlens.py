@@ -366,6 +366,8 @@ def bench_lib():
         L.mlens_bench_dfma.argtypes = [_dp, C.c_void_p]
         L.mlens_bench_atomics.argtypes = [C.c_int64, C.c_int32, _dp, C.c_void_p]
         L.mlens_bench_shared_atomics.argtypes = [_dp, C.c_void_p]
+        L.mlens_bench_atomics_pattern.argtypes = [C.c_int64, C.c_int32, C.c_int32, _dp, C.c_void_p]
+        L.mlens_bench_shared_atomics_kind.argtypes = [C.c_int32, C.c_int32, _dp, C.c_void_p]
         _bench_lib = L
     return _bench_lib
 
@@ -381,15 +383,17 @@ def bench_dfma(stream=None):
     return v.value
 
 
-def bench_atomics(n_slots, use_u64=True, stream=None):
+def bench_atomics(n_slots, use_u64=True, stream=None, pattern=0):
+    """Global 64-bit atomic adds per second; pattern 0 random slots, 1 eight sectors per warp, 2 one sector per warp."""
     v = C.c_double()
-    _bench_check(bench_lib().mlens_bench_atomics(n_slots, int(use_u64), C.byref(v), _stream(stream)))
+    _bench_check(bench_lib().mlens_bench_atomics_pattern(n_slots, int(use_u64), int(pattern), C.byref(v), _stream(stream)))
     return v.value
 
 
-def bench_shared_atomics(stream=None):
+def bench_shared_atomics(stream=None, kind=1, conflict_free=False):
+    """Shared-memory atomic adds per second; kind 0 64-bit CAS loop, 1 the product's two 32-bit adds, 2 one 32-bit add."""
     v = C.c_double()
-    _bench_check(bench_lib().mlens_bench_shared_atomics(C.byref(v), _stream(stream)))
+    _bench_check(bench_lib().mlens_bench_shared_atomics_kind(int(kind), int(conflict_free), C.byref(v), _stream(stream)))
     return v.value
 
 

@@ -31,7 +31,8 @@ def test_exports_every_declared_symbol(so):
     assert not hasattr(L, "mlens_bench_dfma") and not hasattr(L, "mlens_bench_atomics")
     bh = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "mlens_bench.h")).read(), flags=re.S)
     bnames = set(re.findall(r"\b(mlens_[a-z_0-9]+)\s*\(", bh))
-    assert bnames == {"mlens_bench_dfma", "mlens_bench_atomics", "mlens_bench_shared_atomics"}
+    assert bnames == {"mlens_bench_dfma", "mlens_bench_atomics", "mlens_bench_shared_atomics",
+                      "mlens_bench_atomics_pattern", "mlens_bench_shared_atomics_kind"}
     from paper_2506_02114_b200 import build
     B = ctypes.CDLL(build.BENCH_SO)
     for n in bnames:

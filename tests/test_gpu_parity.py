@@ -173,7 +173,7 @@ def test_fmm_coefficients_against_definitions(ml, orc, order):
 
 
 # ----------------------------------------------------------------------------- deflection (the 1e-8 surface)
-@pytest.mark.parametrize("idx,npts", [(0, 100000), (1, 100000), (2, 40000), (3, 16000), (4, 8000)])
+@pytest.mark.parametrize("idx,npts", [(0, 100000), (1, 100000), (2, 40000), (3, 16000), (4, 32000)])
 def test_deflection_parity(ml, orc, idx, npts):
     cfg, gf, of, (xs, ys, ms, R) = _cfg_field(ml, orc, idx)
     g = orc.geometry(cfg.kappa_tot, cfg.kappa_star, cfg.gamma, cfg.half_y, cfg.npix, cfg.rays_per_pixel_length,
@@ -328,6 +328,19 @@ def test_ipm_patches_big_configs(ml, orc, idx, P, npatch):
         # to one quantum per map row and column it spans
         assert res.map.sum() == pytest.approx(tot, rel=1e-6, abs=quantum * (npix + npix))
         assert res.stats["n_queue_overflow"] == 0
+        # the IRS path on the same patch (BASELINE configs[1]: "run both"): its cell-centre rays against the
+        # direct sum, and its counts bit for bit against the positions binned by the oracle's floor of a true division
+        irs = gf.shoot(half, npix, k, map_mode=ml.MAP_IRS, border_mode=cfg.border_mode, border_param=cfg.border_param,
+                       sub=sub, dump=True, want_counts=True)
+        cx, cy = orc.map_centres(of, g, *sub)
+        assert irs.dump[0].shape == cx.shape == (P, P)
+        assert np.max(np.hypot(irs.dump[0] - cx, irs.dump[1] - cy)) <= 1e-8, f"cfg{idx} IRS rays of patch {sub}"
+        want = orc.bin_irs(irs.dump[0], irs.dump[1], g)
+        assert np.array_equal(irs.counts, want), f"cfg{idx} IRS counts of patch {sub}"
+        assert int(want.sum()) <= P * P
+        np.testing.assert_allclose(irs.map, want / (k * k), rtol=1e-14, atol=0.0)
+        own = orc.bin_irs(cx, cy, g)                  # the oracle's own rays: only one within 1e-8 of a pixel edge may move
+        assert int(np.sum(own != want)) <= 4
 
 
 @pytest.mark.parametrize("idx", [1, 2, 3])
@@ -535,6 +548,81 @@ def test_rect_field_map(ml, orc):
     ox, oy = orc.map_centres(of, g, 0, g.n1, 0, g.n2)
     assert np.max(np.hypot(irs.dump[0] - ox, irs.dump[1] - oy)) <= 1e-8
     assert np.array_equal(irs.counts, orc.bin_irs(irs.dump[0], irs.dump[1], g))
+
+
+def test_rect_sheet_fold_respects_a_low_explicit_order(ml, orc):
+    """the rectangle sheet's analytic part is folded into the leaf series truncated at the FIELD's order.  With
+    an order the caller fixed low (p = 8) that truncation must still stay below the accuracy target, or the leaf must
+    keep eq B7: stars of negligible mass (1e-20; kappa_star is taken as given, G17) leave the sheet as the only term the
+    series carries, so every shot ray must equal the oracle's eq B7 to 1e-8 -- next to the rectangle's corners too."""
+    n, c1, c2 = 4000, 30.0, 12.0
+    ks = 0.3
+    xs, ys, ms = synth.rect_stars(n, c1, c2, 17)
+    ms = ms * 1e-20
+    gf = ml.Field.from_stars(0.5, 0.1, xs, ys, ms, kappa_star=ks, shape=ml.SHAPE_RECT, c1=c1, c2=c2, order=8)
+    assert gf.info()["order"] == 8
+    of = orc.Field.make(0.5, ks, 0.1, xs, ys, ms, shape=1, c1=c1, c2=c2)
+    H = (0.98 * c1, 0.98 * c2)                       # a window that reaches into the corners, inside the rectangle
+    hy = (0.3 * H[0], 0.3 * H[1])
+    g = orc.geometry(0.5, ks, 0.1, hy, (32, 32), 12.0, 3, He=H)
+    for mode, ref in ((ml.MAP_IPM, orc.map_corners), (ml.MAP_IRS, orc.map_centres)):
+        res = gf.shoot(hy, (32, 32), 12.0, border_mode=BORDER_EXPLICIT, He=H, map_mode=mode, dump=True)
+        assert (res.grid.n1, res.grid.n2) == (g.n1, g.n2)
+        ox, oy = ref(of, g, 0, g.n1, 0, g.n2)
+        err = np.hypot(res.dump[0] - ox, res.dump[1] - oy)
+        assert err.max() <= 1e-8, (mode, err.max(), np.unravel_index(err.argmax(), err.shape))
+
+
+def test_ray_exactly_on_a_star(ml, orc):
+    """Reading G11 on the GPU (every other test keeps stars off the grid on purpose): a ray that sits exactly on a star
+    skips that star's term on both sides.  (a) deflect / lens_map AT the star positions, FMM and DIRECT; (b) an
+    EXPLICIT window centred on a star at the origin with even cell counts and power-of-two cells, so that corner
+    (n1/2, n2/2) is the star's position to the last bit: IPM corners and map, IRS centres and counts, and the F32
+    evaluator's corners (its bar: 64 2^-24 (1 + sum m/r), as in test_f32_mode_config0)."""
+    n, ks, kt, gam = 600, 0.3, 0.5, 0.2
+    R = math.sqrt(n / ks)
+    xs, ys, ms = synth.disc_stars(n, R, 77)
+    xs[0], ys[0], ms[0] = 0.0, 0.0, 1.0
+    gf = ml.Field.from_stars(kt, gam, xs, ys, ms, kappa_star=ks, R=R)
+    of = orc.Field.make(kt, ks, gam, xs, ys, ms, R=R)
+    # (a)
+    rx, ry = orc.alpha_star(of, xs, ys)
+    assert np.all(np.isfinite(rx)) and np.all(np.isfinite(ry))
+    for mode, tol in ((ml.EVAL_FMM, 1e-8), (ml.EVAL_DIRECT, 1e-12)):
+        ax, ay = gf.deflect(xs, ys, mode)
+        assert np.all(np.isfinite(ax)) and np.all(np.isfinite(ay))
+        scale = 1.0 if mode == ml.EVAL_FMM else np.maximum(1.0, np.hypot(rx, ry))     # DIRECT: rounding of the sum
+        assert np.max(np.hypot(ax - rx, ay - ry) / scale) <= tol, mode
+        wx, wy = gf.lens_map(xs, ys, mode)
+        ox, oy = orc.lens_map(of, xs, ys)
+        assert np.max(np.hypot(wx - ox, wy - oy) / scale) <= tol, mode
+    # (b)
+    half, npix, k, He = 2.0, 32, 2.0, (3.0, 3.0)                   # pixel 1/8, cell 1/16, 96 x 96 cells
+    g = orc.geometry(kt, ks, gam, half, npix, k, 3, He=He)
+    assert g.n1 % 2 == 0 and g.n2 % 2 == 0
+    assert g.x0_1 + (g.n1 // 2) * g.h1 == 0.0 and g.x0_2 + (g.n2 // 2) * g.h2 == 0.0       # a corner on the star
+    kw = dict(border_mode=BORDER_EXPLICIT, He=He, dump=True)
+    res = gf.shoot(half, npix, k, **kw)
+    assert (res.grid.n1, res.grid.n2, res.grid.x0_1, res.grid.x0_2) == (g.n1, g.n2, g.x0_1, g.x0_2)
+    ox, oy = orc.map_corners(of, g, 0, g.n1, 0, g.n2)
+    assert np.all(np.isfinite(res.dump[0])) and np.all(np.isfinite(res.dump[1]))
+    err = np.hypot(res.dump[0] - ox, res.dump[1] - oy)
+    assert err.max() <= 1e-8, np.unravel_index(err.argmax(), err.shape)
+    _map_check(res.map, orc.shoot(of, g, 0), "corner on a star")
+    irs = gf.shoot(half, npix, k, map_mode=ml.MAP_IRS, want_counts=True, **kw)
+    cx, cy = orc.map_centres(of, g, 0, g.n1, 0, g.n2)
+    assert np.max(np.hypot(irs.dump[0] - cx, irs.dump[1] - cy)) <= 1e-8
+    assert np.array_equal(irs.counts, orc.bin_irs(irs.dump[0], irs.dump[1], g))
+    r32 = gf.shoot(half, npix, k, eval_mode=ml.EVAL_FMM_F32, **kw)
+    X, Y = np.meshgrid(g.x0_1 + np.arange(g.n1 + 1) * g.h1, g.x0_2 + np.arange(g.n2 + 1) * g.h2)
+    S = np.zeros_like(X)
+    for sx_, sy_, sm_ in zip(xs, ys, ms):
+        d = np.hypot(X - sx_, Y - sy_)
+        S += np.where(d > 0, sm_ / np.maximum(d, 1e-300), 0.0)    # the skipped term adds nothing to the bar
+    e32 = np.hypot(r32.dump[0] - ox, r32.dump[1] - oy)
+    assert np.all(np.isfinite(e32)) and np.all(e32 <= 64 * 2.0 ** -24 * (1.0 + S)), f"worst {np.max(e32 / (1 + S)):.3g}"
+    j, i = g.n2 // 2, g.n1 // 2
+    assert e32[j, i] <= 64 * 2.0 ** -24 * (1.0 + S[j, i])
 
 
 def test_ipm_and_irs_agree_on_gpu(ml):
