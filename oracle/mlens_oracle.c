@@ -22,7 +22,9 @@
  * Parity pins (tests/test_oracle_*.py): point-lens magnification, Chang-Refsdal
  * caustic cusps, rectangle sheet vs 2-D quadrature of eq B1, affine-map
  * exactness of IPM, area conservation, mean magnification, Monte-Carlo area on
- * tiny inputs, RNG uniformity and closed-form moments.  Unpinned: the paper's
+ * tiny inputs, RNG uniformity and closed-form moments; the second-order macro
+ * terms (reading G23) by the closed-form fold map (image positions, flux per
+ * pixel column, pixel means) and a finite-difference Jacobian.  Unpinned: the paper's
  * own absolute map values (its figures and star files are not available).
  */
 #include <complex.h>
@@ -43,6 +45,10 @@ typedef struct {
     double R, c1, c2;
     int64_t n_stars;
     const double *x, *y, *m;
+    /* Macro model beyond linear (App. D, P:694-702 gives the idea -- "the chosen order to which the potential is Taylor
+     * expanded" -- and no formula; reading G23): third derivatives psi_111, psi_112, psi_122, psi_222 of the
+     * macro potential at the origin.  All zero = the paper's constant kappa, gamma. */
+    double t111, t112, t122, t222;
 } orc_field;
 
 int orc_num_threads(void)
@@ -127,15 +133,21 @@ void orc_alpha_smooth(const orc_field *f, int64_t n, const double *zx, const dou
     }
 }
 
-/* Lens equation, eq 12: w = (1-kappa) z + gamma conj(z) - alpha_star - alpha_s */
+/* Lens equation, eq 12: w = (1-kappa) z + gamma conj(z) - alpha_star - alpha_s
+ * and, reading G23 (App. D: the macro potential Taylor-expanded one order further), minus the second-order term
+ * of the macro deflection grad(psi):  alpha_i += (1/2) sum_jk psi_ijk x_j x_k, i.e.
+ *   alpha_1 += (psi_111 x1^2 + 2 psi_112 x1 x2 + psi_122 x2^2)/2,  alpha_2 += (psi_112 x1^2 + 2 psi_122 x1 x2 + psi_222 x2^2)/2. */
 static void lens_map_1(const orc_field *f, double zx, double zy, double *wx, double *wy)
 {
     ld asx, asy, amx, amy;
     alpha_star_1(f, zx, zy, &asx, &asy);
     alpha_smooth_1(f, zx, zy, &amx, &amy);
     ld k = f->kappa_tot, g = f->gamma;
-    *wx = (double)((1 - k) * zx + g * zx - asx - amx);
-    *wy = (double)((1 - k) * zy - g * zy - asy - amy);
+    ld x1 = zx, x2 = zy;
+    ld q1 = (f->t111 * x1 * x1 + 2 * f->t112 * x1 * x2 + f->t122 * x2 * x2) / 2;
+    ld q2 = (f->t112 * x1 * x1 + 2 * f->t122 * x1 * x2 + f->t222 * x2 * x2) / 2;
+    *wx = (double)((1 - k) * zx + g * zx - asx - amx - q1);
+    *wy = (double)((1 - k) * zy - g * zy - asy - amy - q2);
 }
 
 void orc_lens_map(const orc_field *f, int64_t n, const double *zx, const double *zy,

@@ -22,12 +22,14 @@ class Field(C.Structure):
     _fields_ = [("kappa_tot", C.c_double), ("kappa_star", C.c_double), ("gamma", C.c_double),
                 ("theta_star", C.c_double), ("shape", C.c_int32), ("pad_", C.c_int32),
                 ("R", C.c_double), ("c1", C.c_double), ("c2", C.c_double),
-                ("n_stars", C.c_int64), ("x", _dp), ("y", _dp), ("m", _dp)]
+                ("n_stars", C.c_int64), ("x", _dp), ("y", _dp), ("m", _dp),
+                ("t111", C.c_double), ("t112", C.c_double), ("t122", C.c_double), ("t222", C.c_double)]
 
     @classmethod
     def make(cls, kappa_tot, kappa_star, gamma, x, y, m, *, shape=0, R=0.0, c1=0.0, c2=0.0,
-             theta_star=1.0):
+             theta_star=1.0, macro_quad=(0.0, 0.0, 0.0, 0.0)):
         f = cls()
+        f.t111, f.t112, f.t122, f.t222 = macro_quad      # reading G23: third derivatives of the macro potential at 0
         f.kappa_tot, f.kappa_star, f.gamma, f.theta_star = kappa_tot, kappa_star, gamma, theta_star
         f.shape, f.R, f.c1, f.c2 = shape, R, c1, c2
         f._x = np.ascontiguousarray(x, dtype=np.float64)
