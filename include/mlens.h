@@ -199,6 +199,17 @@ int mlens_field_create_seeded(const mlens_seed_desc *desc, mlens_field **out);
 int mlens_field_destroy(mlens_field *f);
 int mlens_field_get_info(const mlens_field *f, mlens_field_info *info);
 
+/* Macro model beyond linear, for maps next to a macro-caustic (App. D: "the chosen order to which the
+ * potential is Taylor expanded"; the paper prints no formula, reading G23).  The macro deflection grad(psi)
+ * gets its second-order Taylor term about the origin, from the four third derivatives of the macro potential there:
+ *   w1 -= (psi_111 x1^2 + 2 psi_112 x1 x2 + psi_122 x2^2) / 2,   w2 -= (psi_112 x1^2 + 2 psi_122 x1 x2 + psi_222 x2^2) / 2
+ * in eq 12 (mlens_lens_map and every ray of mlens_shoot; mlens_deflect, the stars' part, is untouched).  All four zero
+ * (the state after create) is the paper's constant kappa and gamma, to the last bit.  With any of them non-zero the
+ * shooting window of eq 14-16 no longer encloses the macro-images, so mlens_shoot / mlens_grid_info then take
+ * MLENS_BORDER_EXPLICIT only (MLENS_EINVAL otherwise): choosing the window is the part the paper leaves to other work.
+ * Host-side state only (no device work); affects the calls made after it. */
+int mlens_field_set_macro_quadratic(mlens_field *f, double psi_111, double psi_112, double psi_122, double psi_222);
+
 /* Copies the stars (positions in units of theta_star's length, masses as used in eq 13; for a seeded field
  * the draws of P:159-165), in the caller's original order, into x, y, m (length n_stars each). */
 int mlens_field_get_stars(const mlens_field *f, double *x, double *y, double *m, int32_t ptr_kind, void *stream);

@@ -277,6 +277,14 @@ int mlens_field_destroy(mlens_field *f) {
     return MLENS_OK;
 }
 
+int mlens_field_set_macro_quadratic(mlens_field *f, double psi_111, double psi_112, double psi_122, double psi_222) {
+    if (!f) { set_error("null argument"); return MLENS_EINVAL; }
+    const double t[4] = {psi_111, psi_112, psi_122, psi_222};
+    for (int i = 0; i < 4; ++i) if (!(t[i] == t[i]) || fabs(t[i]) > 1e300) { set_error("macro coefficients must be finite"); return MLENS_EINVAL; }
+    for (int i = 0; i < 4; ++i) f->quad[i] = t[i];
+    return MLENS_OK;
+}
+
 int mlens_field_get_info(const mlens_field *f, mlens_field_info *o) {
     if (!f || !o) { set_error("null argument"); return MLENS_EINVAL; }
     memset(o, 0, sizeof(*o));

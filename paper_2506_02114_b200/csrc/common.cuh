@@ -119,6 +119,7 @@ struct mlens_field {
     int shape = 0;
     double R = 0, c1 = 0, c2 = 0;
     double eps = 1e-8;
+    double quad[4] = {0, 0, 0, 0};  // psi_111, psi_112, psi_122, psi_222 of the macro potential (reading G23); all zero = off
     int max_direct = 32;
     int order = 0;                 // p
     int64_t n_stars = 0;

@@ -36,6 +36,8 @@ __device__ __forceinline__ double fast_rcp(double a) {
 // ---- everything a kernel needs to evaluate the lens equation (eq 12)
 struct LensDev {
     double one_minus_kappa, gamma, kappa_star, theta2;
+    double q111, q112, q122, q222;      // macro potential's third derivatives at the origin (App. D, reading G23)
+    int has_quad;                       // 0: constant kappa, gamma (the terms are not even touched)
     int shape;
     double R2, c1, c2;
     // tree
@@ -187,6 +189,15 @@ static __device__ __noinline__ double2 direct_all_ool(const LensDev *L, double x
     return make_double2(ax * L->theta2, ay * L->theta2);
 }
 
+// Second-order term of the macro deflection (App. D; reading G23): w -= (1/2) psi_ijk x_j x_k.  A uniform
+// branch: fields without it (every BASELINE config) execute one predicate.
+__device__ __forceinline__ void macro_quad(const LensDev &L, double x, double y, double &wx, double &wy) {
+    if (L.has_quad) {
+        wx -= 0.5 * (L.q111 * x * x + 2.0 * L.q112 * x * y + L.q122 * y * y);
+        wy -= 0.5 * (L.q112 * x * x + 2.0 * L.q122 * x * y + L.q222 * y * y);
+    }
+}
+
 // w of eq 12 from alpha_star: w = (1-kappa) z + gamma conj z - alpha_star - alpha_s
 __device__ __forceinline__ void lens_w(const LensDev &L, double x, double y, double ax, double ay,
                                        double &wx, double &wy) {
@@ -194,6 +205,7 @@ __device__ __forceinline__ void lens_w(const LensDev &L, double x, double y, dou
     sheet(L, x, y, sx_, sy_);
     wx = (L.one_minus_kappa + L.gamma) * x - ax - sx_;
     wy = (L.one_minus_kappa - L.gamma) * y - ay - sy_;
+    macro_quad(L, x, y, wx, wy);
 }
 
 LensDev make_lens_dev(const mlens_field *f);

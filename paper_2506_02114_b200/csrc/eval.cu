@@ -8,6 +8,8 @@ LensDev make_lens_dev(const mlens_field *f) {
     LensDev L;
     L.one_minus_kappa = 1.0 - f->kappa_tot;
     L.gamma = f->gamma;
+    L.q111 = f->quad[0]; L.q112 = f->quad[1]; L.q122 = f->quad[2]; L.q222 = f->quad[3];
+    L.has_quad = (f->quad[0] != 0.0 || f->quad[1] != 0.0 || f->quad[2] != 0.0 || f->quad[3] != 0.0) ? 1 : 0;
     L.kappa_star = f->kappa_star;
     L.theta2 = f->theta * f->theta;
     L.shape = f->shape;
@@ -19,8 +21,10 @@ LensDev make_lens_dev(const mlens_field *f) {
     L.child0 = t.child0.p; L.leaf_id = t.leaf_id.p; L.level = t.level.p; L.ix = t.ix.p; L.iy = t.iy.p;
     L.near_cnt = t.near_cnt.p; L.near_x = t.near_x.p; L.near_y = t.near_y.p; L.near_m = t.near_m.p;
     L.ecoef = t.ecoef.p;
-    L.ecoef_shoot = (f->shape == MLENS_SHAPE_RECT && t.ecoef_shoot.p) ? t.ecoef_shoot.p : t.ecoef.p;
-    L.leaf_fold = (f->shape == MLENS_SHAPE_RECT) ? t.leaf_fold.p : nullptr;
+    // (with macro terms beyond linear every ray goes through lens_w, sheet included: no folded series then)
+    const bool fold_ok = f->shape == MLENS_SHAPE_RECT && !L.has_quad;
+    L.ecoef_shoot = (fold_ok && t.ecoef_shoot.p) ? t.ecoef_shoot.p : t.ecoef.p;
+    L.leaf_fold = fold_ok ? t.leaf_fold.p : nullptr;
     L.p = f->order; L.p1 = f->order + 1;
     L.sx = f->sx.p; L.sy = f->sy.p; L.sm = f->sm.p;
     L.n_stars = f->n_stars;

@@ -793,6 +793,11 @@ int geometry(const mlens_field *f, const mlens_shoot_desc *d, mlens_grid *g) {
         set_error("bad map description"); return MLENS_EINVAL;
     }
     if (d->npix1 > 30000 || d->npix2 > 30000) { set_error("maps are limited to 30000 pixels per side"); return MLENS_EINVAL; }
+    if ((f->quad[0] != 0.0 || f->quad[1] != 0.0 || f->quad[2] != 0.0 || f->quad[3] != 0.0) && d->border_mode != MLENS_BORDER_EXPLICIT) {
+        set_error("a field with macro terms beyond linear (mlens_field_set_macro_quadratic) needs an explicit window: "
+                  "eq 14-16 enclose the macro-images of a constant kappa, gamma only (MLENS_BORDER_EXPLICIT)");
+        return MLENS_EINVAL;
+    }
     g->p1 = 2.0 * d->half_y1 / d->npix1;
     g->p2 = 2.0 * d->half_y2 / d->npix2;
     g->h1 = g->p1 / d->rays_per_pixel_length;

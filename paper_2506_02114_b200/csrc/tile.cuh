@@ -285,7 +285,9 @@ static __device__ __noinline__ void wtile_setup_ool(const ShootDev *Sp, WarpShar
     }
     // eq 19 inside the disc is linear in z: the farthest ray of the tile decides (the disc is convex)
     const double rmax = sqrt(C.zt_x * C.zt_x + C.zt_y * C.zt_y) + rt;
-    const bool lin = (S.L.shape == MLENS_SHAPE_DISC && rmax * rmax <= S.L.R2) || fold;
+    // (a field with macro terms beyond linear, reading G23, is never `lin`: its rays take lens_w, which holds that term;
+    // make_lens_dev switches the rectangle fold off for such a field, so `fold` is false then)
+    const bool lin = !S.L.has_quad && ((S.L.shape == MLENS_SHAPE_DISC && rmax * rmax <= S.L.R2) || fold);
     zero_window(W);
     if (lane == 0) {
         W.ctx[0] = C.zt_x; W.ctx[1] = C.zt_y; W.ctx[2] = C.inv_rt;

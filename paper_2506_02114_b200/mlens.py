@@ -121,6 +121,7 @@ def lib():
         L.mlens_map_light_curve.argtypes = [vp, i32, i32, dbl, dbl, dbl, dbl, dbl, dbl, dbl, dbl, i64, i32, vp, i32, vp]
         L.mlens_map_histogram.argtypes = [vp, i64, dbl, dbl, dbl, i32, vp, i32, vp]
         L.mlens_map_histogram_static.argtypes = [vp, i64, dbl, dbl, dbl, i32, vp, vp]
+        L.mlens_field_set_macro_quadratic.argtypes = [vp, dbl, dbl, dbl, dbl]
         _lib = L
     return _lib
 
@@ -262,6 +263,13 @@ class Field:
     def deflect(self, zx, zy, eval_mode=EVAL_FMM, stream=None):
         """alpha_star (eq 13) at the given points."""
         return self._points(lib().mlens_deflect, zx, zy, eval_mode, stream)
+
+    def set_macro_quadratic(self, psi_111, psi_112, psi_122, psi_222):
+        """mlens_field_set_macro_quadratic: second-order Taylor term of the macro deflection (App. D; maps next to a
+        macro-caustic).  Shooting then needs border_mode=BORDER_EXPLICIT.  All zero switches it off."""
+        _check(lib().mlens_field_set_macro_quadratic(self._h, C.c_double(psi_111), C.c_double(psi_112),
+                                                     C.c_double(psi_122), C.c_double(psi_222)))
+        return self
 
     def lens_map(self, zx, zy, eval_mode=EVAL_FMM, stream=None):
         """w of eq 12 at the given points."""

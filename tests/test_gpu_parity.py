@@ -625,6 +625,66 @@ def test_ray_exactly_on_a_star(ml, orc):
     assert e32[j, i] <= 64 * 2.0 ** -24 * (1.0 + S[j, i])
 
 
+def test_macro_terms_beyond_linear(ml, orc):
+    """SURVEY 8(f) NEXT-3 remainder (App. D; reading G23): second-order Taylor term of the macro deflection.
+    (a) no stars, a fold (psi_111 alone): the GPU's IPM map against the oracle's (itself pinned to the closed form) and
+    against the closed-form pixel means; (b) stars + all four coefficients: points, every corner and centre of an
+    EXPLICIT window to 1e-8, the IPM map under the north_star rule, IRS counts bit for bit, the F32 evaluator's bar;
+    (c) zero coefficients are today's bits; any other window mode is refused."""
+    kt, gam, g_ = 0.3, 0.1, 0.08
+    a, b = 1 - kt + gam, 1 - kt - gam
+    z = np.zeros(0)
+    f = ml.Field.from_stars(kt, gam, z, z, z, kappa_star=0.0, R=1e9).set_macro_quadratic(g_, 0.0, 0.0, 0.0)
+    of = orc.Field.make(kt, 0.0, gam, z, z, z, R=1e9, macro_quad=(g_, 0.0, 0.0, 0.0))
+    He = (4.0, 4.0)
+    geo = orc.geometry(kt, 0.0, gam, 2.0, 32, 8.0, 3, He=He)
+    res = f.shoot(2.0, 32, 8.0, border_mode=BORDER_EXPLICIT, He=He)
+    ref = orc.shoot(of, geo, 0)
+    assert np.max(np.abs(res.map - ref)) <= 1e-9 * ref.max()
+    ylo = geo.ylo1 + geo.p1 * np.arange(32)
+    want = (np.sqrt(a * a - 2 * g_ * ylo) - np.sqrt(a * a - 2 * g_ * (ylo + geo.p1))) / (g_ * geo.p1 * abs(b))
+    assert np.max(np.abs(res.map[16] / want - 1)) <= 2e-3 and abs(res.map[16].mean() * a * abs(b) - 1) > 1e-3
+    with pytest.raises(ml.MlensError, match="explicit window"):
+        f.shoot(2.0, 32, 8.0, border_mode=ml.BORDER_EQ16)
+    # (b)
+    n, ks, kt, gam = 500, 0.2, 0.45, 0.2
+    R = math.sqrt(n / ks)
+    xs, ys, ms = synth.disc_stars(n, R, 123)
+    t = (0.004, -0.003, 0.002, 0.005)
+    gf = ml.Field.from_stars(kt, gam, xs, ys, ms, kappa_star=ks, R=R)
+    of0 = orc.Field.make(kt, ks, gam, xs, ys, ms, R=R)
+    of = orc.Field.make(kt, ks, gam, xs, ys, ms, R=R, macro_quad=t)
+    He, half, npix, k = (9.0, 12.0), 3.0, 48, 3.0
+    kw = dict(border_mode=BORDER_EXPLICIT, He=He, dump=True)
+    base = gf.shoot(half, npix, k, **kw)
+    gf.set_macro_quadratic(*t)
+    zx, zy = synth.sample_points_window(20000, 0.0, 0.0, He[0], He[1], 8)
+    wx, wy = gf.lens_map(zx, zy)
+    ox, oy = orc.lens_map(of, zx, zy)
+    assert np.max(np.hypot(wx - ox, wy - oy)) <= 1e-8
+    o0x, o0y = orc.lens_map(of0, zx, zy)
+    assert np.max(np.hypot(ox - o0x, oy - o0y)) > 0.1          # the term is not small here
+    ax, ay = gf.deflect(zx[:2000], zy[:2000])
+    rx, ry = orc.alpha_star(of, zx[:2000], zy[:2000])
+    assert np.max(np.hypot(ax - rx, ay - ry)) <= 1e-8          # the stars' part is untouched
+    geo = orc.geometry(kt, ks, gam, half, npix, k, 3, He=He)
+    res = gf.shoot(half, npix, k, **kw)
+    cx, cy = orc.map_corners(of, geo, 0, geo.n1, 0, geo.n2)
+    assert np.max(np.hypot(res.dump[0] - cx, res.dump[1] - cy)) <= 1e-8
+    _map_check(res.map, orc.shoot(of, geo, 0), "macro terms beyond linear")
+    irs = gf.shoot(half, npix, k, map_mode=ml.MAP_IRS, want_counts=True, **kw)
+    mx, my = orc.map_centres(of, geo, 0, geo.n1, 0, geo.n2)
+    assert np.max(np.hypot(irs.dump[0] - mx, irs.dump[1] - my)) <= 1e-8
+    assert np.array_equal(irs.counts, orc.bin_irs(irs.dump[0], irs.dump[1], geo))
+    r32 = gf.shoot(half, npix, k, eval_mode=ml.EVAL_FMM_F32, **kw)
+    e32 = np.hypot(r32.dump[0] - cx, r32.dump[1] - cy)
+    assert np.median(e32) <= 3e-7 and np.max(e32) > 1e-9
+    # (c)
+    gf.set_macro_quadratic(0.0, 0.0, 0.0, 0.0)
+    again = gf.shoot(half, npix, k, **kw)
+    assert np.array_equal(again.map, base.map) and np.array_equal(again.dump[0], base.dump[0]) and np.array_equal(again.dump[1], base.dump[1])
+
+
 def test_ipm_and_irs_agree_on_gpu(ml):
     # P:288 "we do not find any differences": IRS at high density converges to the IPM map within Poisson error
     cfg = synth.get_config(0)
